@@ -1,0 +1,18 @@
+"""Seeded synthetic inputs for the Benincasa-Dowker action hot path.
+
+This package serves BOTH the oracle-side tests and the CUDA-side tests/bench and therefore holds none of
+the method's arithmetic (no interval counts, no histogram, no action): only the seeded sprinkling, the
+time sort, the relation test and the packed-matrix layout.  Recipe: DESIGN.md "Input recipe" (A17).
+It imports neither ``oracle`` nor ``paper_1709_03013_b200``.
+"""
+from .generate import (  # noqa: F401
+    CONFIGS,
+    build,
+    stride_words,
+    sprinkle,
+    relations_from_coords,
+    make_causet,
+    pack_dense,
+    bits_hash,
+    random_poset_bits,
+)

@@ -1,0 +1,19 @@
+"""ORACLE package -- test infrastructure only.
+
+Plain CPU restatement of the paper's hot path (PAPER.md:395 naive action algorithm; Eq. 4 / Eq. 5;
+Algorithm 5).  Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package.  It never imports ``paper_1709_03013_b200``.
+"""
+from .oracle import (  # noqa: F401
+    build,
+    expand,
+    counts_plain,
+    counts_from_bits,
+    pair_interval,
+    action_local,
+    f2,
+    action_smeared_2d,
+    alg5_counts,
+    alg5_counts_rows,
+    alg5_threads,
+)

@@ -1,0 +1,141 @@
+"""ctypes front end of the C oracle (oracle/csg_oracle.c, oracle/alg5_packed.c).
+
+Test infrastructure only (see oracle/__init__.py).  Every function cites the PAPER.md passage its C body
+follows; the arithmetic lives in the C files, this module only marshals numpy arrays.
+"""
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "liboracle.so")
+_SRCS = [os.path.join(_HERE, "csg_oracle.c"), os.path.join(_HERE, "alg5_packed.c")]
+_lib = None
+
+_i64 = ctypes.c_int64
+_p_u64 = np.ctypeslib.ndpointer(dtype=np.uint64, flags="C_CONTIGUOUS")
+_p_u8 = np.ctypeslib.ndpointer(dtype=np.uint8, flags="C_CONTIGUOUS")
+_p_i64 = np.ctypeslib.ndpointer(dtype=np.int64, flags="C_CONTIGUOUS")
+
+
+def build(force=False):
+    """Compile the oracle with gcc (plain -O2; OpenMP only drives Algorithm 5's pair loop)."""
+    newest = max(os.path.getmtime(s) for s in _SRCS)
+    if not force and os.path.exists(_LIB_PATH) and os.path.getmtime(_LIB_PATH) >= newest:
+        return _LIB_PATH
+    cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-o", _LIB_PATH] + _SRCS + ["-lm"]
+    subprocess.run(cmd, check=True)
+    return _LIB_PATH
+
+
+def _load():
+    global _lib
+    if _lib is not None:
+        return _lib
+    build()
+    lib = ctypes.CDLL(_LIB_PATH)
+    lib.csg_oracle_expand.argtypes = [_p_u64, _i64, _i64, _p_u8]
+    lib.csg_oracle_expand.restype = None
+    lib.csg_oracle_counts.argtypes = [_p_u8, _i64, _i64, _p_i64]
+    lib.csg_oracle_counts.restype = None
+    lib.csg_oracle_pair.argtypes = [_p_u64, _i64, _i64, _i64, _i64]
+    lib.csg_oracle_pair.restype = _i64
+    lib.csg_oracle_action_local.argtypes = [ctypes.c_int, _i64, _p_i64]
+    lib.csg_oracle_action_local.restype = ctypes.c_double
+    lib.csg_oracle_f2.argtypes = [_i64, ctypes.c_double]
+    lib.csg_oracle_f2.restype = ctypes.c_double
+    lib.csg_oracle_action_smeared_2d.argtypes = [_i64, _i64, _p_i64, ctypes.c_double,
+                                                 ctypes.POINTER(ctypes.c_double)]
+    lib.csg_oracle_action_smeared_2d.restype = ctypes.c_double
+    lib.csg_alg5_counts.argtypes = [_p_u64, _i64, _i64, _i64, _p_i64]
+    lib.csg_alg5_counts.restype = None
+    lib.csg_alg5_counts_rows.argtypes = [_p_u64, _i64, _i64, _i64, _i64, _i64, _p_i64,
+                                         ctypes.POINTER(_i64)]
+    lib.csg_alg5_counts_rows.restype = None
+    lib.csg_alg5_threads.argtypes = []
+    lib.csg_alg5_threads.restype = ctypes.c_int
+    _lib = lib
+    return lib
+
+
+def _check_bits(bits, N):
+    bits = np.ascontiguousarray(bits, dtype=np.uint64)
+    assert bits.ndim == 2 and bits.shape[0] >= N and bits.shape[1] * 64 >= N, bits.shape
+    return bits
+
+
+def expand(bits, N):
+    """Packed relation matrix -> N x N byte matrix (PAPER.md:163-169 layout)."""
+    bits = _check_bits(bits, N)
+    B = np.zeros((N, N), dtype=np.uint8)
+    if N > 0:
+        _load().csg_oracle_expand(bits, N, bits.shape[1], B)
+    return B
+
+
+def counts_plain(B, kmax):
+    """Naive action algorithm on a byte matrix: counts[0..kmax]."""
+    B = np.ascontiguousarray(B, dtype=np.uint8)
+    N = B.shape[0]
+    assert B.shape == (N, N)
+    counts = np.zeros(kmax + 1, dtype=np.int64)
+    _load().csg_oracle_counts(B, N, kmax, counts)
+    return counts
+
+
+def counts_from_bits(bits, N, kmax):
+    """expand() then counts_plain(): the oracle on the same packed bitset the GPU gets."""
+    return counts_plain(expand(bits, N), kmax)
+
+
+def pair_interval(bits, N, i, j):
+    """n_ij for one pair, bit by bit from the packed matrix; -1 if unrelated."""
+    bits = _check_bits(bits, N)
+    return int(_load().csg_oracle_pair(bits, N, bits.shape[1], int(i), int(j)))
+
+
+def action_local(dim, N, counts):
+    """Eq. 4 (dim=2) or the d=4 BD combination (reading A8)."""
+    counts = np.ascontiguousarray(counts, dtype=np.int64)
+    need = 3 if dim == 2 else 4
+    if counts.shape[0] < need:
+        counts = np.concatenate([counts, np.zeros(need - counts.shape[0], dtype=np.int64)])
+    return float(_load().csg_oracle_action_local(int(dim), int(N), counts))
+
+
+def f2(k, eps):
+    """Smearing weight f_2(k, eps) of Eq. 5."""
+    return float(_load().csg_oracle_f2(int(k), float(eps)))
+
+
+def action_smeared_2d(N, counts, eps):
+    """Eq. 5 over counts[0..len-1]; returns (S_eps, abs_scale)."""
+    counts = np.ascontiguousarray(counts, dtype=np.int64)
+    scale = ctypes.c_double(0.0)
+    s = _load().csg_oracle_action_smeared_2d(int(N), counts.shape[0] - 1, counts, float(eps),
+                                             ctypes.byref(scale))
+    return float(s), float(scale.value)
+
+
+def alg5_counts(bits, N, kmax):
+    """Algorithm 5 on the packed matrix, all host threads."""
+    bits = _check_bits(bits, N)
+    counts = np.zeros(kmax + 1, dtype=np.int64)
+    _load().csg_alg5_counts(bits, N, bits.shape[1], kmax, counts)
+    return counts
+
+
+def alg5_counts_rows(bits, N, kmax, row_begin, row_end):
+    """Algorithm 5 restricted to first elements i in [row_begin,row_end); returns (counts, triple_tests)."""
+    bits = _check_bits(bits, N)
+    counts = np.zeros(kmax + 1, dtype=np.int64)
+    tests = _i64(0)
+    _load().csg_alg5_counts_rows(bits, N, bits.shape[1], kmax, int(row_begin), int(row_end), counts,
+                                 ctypes.byref(tests))
+    return counts, int(tests.value)
+
+
+def alg5_threads():
+    return int(_load().csg_alg5_threads())
