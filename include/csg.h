@@ -1,0 +1,119 @@
+/*
+ * csg.h -- C ABI of libcsg: Benincasa-Dowker action of a causal set on one B200 (sm_100a).
+ *
+ * The library computes the O(N^3) hot path of Cunningham & Krioukov, "Causal Set Generator and Action
+ * Computer" (arXiv:1709.03013; citations below are /root/reference/PAPER.md:<line>):
+ *   for every related pair i<j of a time-sorted causal set, the number n_ij of elements k with
+ *   i < k < j related to both (Sec. 4.1; Fig. 2 caption; Algorithm 5,
+ *   PAPER.md:407), the histogram N_k of those interval sizes, and the action built from it
+ *   (Eq. 4; Eq. 5).
+ *
+ * Relation-matrix layout (FastBitset rows): N rows of csg_row_stride_words(N) 64-bit
+ * words; bit c of row r is bit (c % 64), LSB first, of word r*stride + c/64.  The matrix
+ * is symmetric (bit (r,c) == bit (c,r) == 1 iff the two elements are related), has a zero diagonal and zero
+ * padding bits, and rows are sorted so that "r precedes c" implies r < c.  For a pair i<j the
+ * library reads bit (i,j), bits (i,k) and bits (j,k) for i<k<j -- both triangles are used.
+ *
+ * No function throws; every function returns a CSG_* code (0 = success) unless stated otherwise.
+ * There is no CPU fallback: without a CUDA device every compute entry point returns CSG_E_CUDA.
+ * Pointers are tagged DEVICE or HOST.  The caller owns every buffer it passes; the library keeps a small
+ * cached device workspace (tile schedule, counters) that csg_shutdown() frees.  Inputs are never modified.
+ */
+#ifndef CSG_H_
+#define CSG_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#ifndef __DRIVER_TYPES_H__
+typedef struct CUstream_st *cudaStream_t;
+#endif
+
+enum {
+    CSG_OK = 0,
+    CSG_E_NULL = -1,        /* a required pointer is NULL */
+    CSG_E_SIZE = -2,        /* N < 1, N > CSG_MAX_N, or npairs < 0 */
+    CSG_E_ALIGN = -3,       /* rel_bits not 16-byte aligned, counts/S not 8-byte aligned */
+    CSG_E_DIM = -4,         /* dim not in {2, 4} */
+    CSG_E_EPS = -5,         /* eps NaN or outside (0, 1] */
+    CSG_E_KMAX = -6,        /* kmax < 0, kmax > CSG_MAX_KMAX, or too small for the local action */
+    CSG_E_UNSUPPORTED = -7, /* smeared action in 4D (not defined by the paper) */
+    CSG_E_CUDA = -8,        /* a CUDA call failed; csg_strerror(CSG_E_CUDA) carries its text */
+    CSG_E_VARIANT = -9      /* unknown variant id */
+};
+
+#define CSG_MAX_N (1 << 22)
+#define CSG_MAX_KMAX (1 << 22)
+
+enum {
+    CSG_VARIANT_AUTO = 0,   /* tensor variant when N >= 2048, else bitset */
+    CSG_VARIANT_BITSET = 1, /* LOP3 AND + POPC over packed 32-bit words, register micro-tiles */
+    CSG_VARIANT_TENSOR = 2  /* bits unpacked to 0/1 u8 in shared memory, tcgen05.mma kind::i8 into TMEM */
+};
+
+/* Row stride of the relation matrix in 64-bit words: 4*ceil(N/256) (rows 256-bit aligned). */
+int64_t csg_row_stride_words(int64_t N);
+
+/*
+ * Interval abundances and action of one causal set.  All work is enqueued on `stream`; no host
+ * synchronisation happens inside (the first call for a new N also builds the cached tile schedule).
+ *
+ *   rel_bits DEVICE, N*csg_row_stride_words(N) words, layout above, 16-byte aligned, read only.
+ *   N        number of elements, 1 <= N <= CSG_MAX_N (N = 1, 2 are valid: no triples).
+ *   dim      2 or 4: which combination of abundances gives S.
+ *   eps      1.0 -> local action: dim 2: S = 2(N - 2N_0 + 4N_1 - 2N_2) (Eq. 4 with n_i = N_{i-1});
+ *                   dim 4: S = (4/sqrt 6)(N - N_0 + 9N_1 - 16N_2 + 8N_3) (not in the paper; A8).
+ *                   Needs kmax >= 2 (dim 2) or >= 3 (dim 4).
+ *            0 < eps < 1 -> smeared action, dim 2 only (Eq. 5):
+ *                   S = 2 eps [N - 2 eps sum_{k=0..kmax} N_k f_2(k, eps)]; pass kmax = N-2 for the full sum.
+ *   kmax     highest interval size that is histogrammed; related pairs with n_ij > kmax are not counted.
+ *   counts   DEVICE, kmax+1 int64, overwritten: counts[k] = N_k = number of related pairs i<j with exactly
+ *            k elements strictly between (0-based; the paper's n_i is counts[i-1]).
+ *   S        DEVICE, 1 double, overwritten.
+ */
+int csg_action(const uint64_t *rel_bits, int64_t N, int dim, double eps, int kmax, int64_t *counts,
+               double *S, cudaStream_t stream);
+
+/*
+ * Same computation with HOST buffers (the end-to-end call): copies rel_bits to the device (pinned or
+ * pageable host memory), runs csg_action on an internal stream, copies counts and S back and
+ * synchronises.  rel_bits_host: N*stride words; counts_host: kmax+1 int64; S_host: 1 double.
+ */
+int csg_action_host(const uint64_t *rel_bits_host, int64_t N, int dim, double eps, int kmax,
+                    int64_t *counts_host, double *S_host);
+
+/*
+ * Test hook: interval sizes of listed pairs.  pairs_ij DEVICE, 2*npairs int64 (i0, j0, i1, j1, ...);
+ * n_out DEVICE, npairs int32: n_ij if 0 <= i < j < N and bit (i,j) is set, else -1.
+ */
+int csg_interval_sizes(const uint64_t *rel_bits, int64_t N, const int64_t *pairs_ij, int64_t npairs,
+                       int32_t *n_out, cudaStream_t stream);
+
+/* Choose the kernel variant for later csg_action calls (CSG_VARIANT_*); returns CSG_E_VARIANT if unknown. */
+int csg_set_variant(int variant);
+/* The variant csg_action would run for this N under the current setting (CSG_VARIANT_BITSET or _TENSOR). */
+int csg_effective_variant(int64_t N);
+
+/*
+ * Measurement aids.  csg_set_kernel_timing(1) makes csg_action bracket its dominant kernel (the interval
+ * kernel, not the memsets or the finishing kernel) with CUDA events on the caller's stream;
+ * csg_last_kernel_ms waits for those events and returns the elapsed milliseconds of the latest call.
+ * csg_launch_count returns how many kernels this library has launched in this process.
+ */
+int csg_set_kernel_timing(int enable);
+int csg_last_kernel_ms(float *ms);
+int64_t csg_launch_count(void);
+
+/* Text for a code; for CSG_E_CUDA it includes the text of the last CUDA error the library saw. */
+const char *csg_strerror(int code);
+
+/* Free the cached device workspace and internal stream/events.  Safe to call more than once. */
+int csg_shutdown(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CSG_H_ */

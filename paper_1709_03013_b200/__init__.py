@@ -1,0 +1,176 @@
+"""paper_1709_03013_b200 -- thin Python binding of libcsg (include/csg.h).
+
+Argument marshalling only: every step of the hot path (interval sizes, histogram, action) runs in the
+hand-written sm_100a kernels behind the C ABI.  PyTorch is used for device memory and streams.
+There is no CPU fallback: if libcsg.so is missing, importing the compute entry points fails loudly.
+
+Functions carry the C names: csg_action, csg_action_host, csg_interval_sizes, csg_row_stride_words,
+csg_set_variant, csg_effective_variant, csg_set_kernel_timing, csg_last_kernel_ms, csg_launch_count,
+csg_strerror, csg_shutdown.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+from . import _build
+
+VARIANT_AUTO, VARIANT_BITSET, VARIANT_TENSOR = 0, 1, 2
+LIB_PATH = _build.LIB_PATH
+
+EXPORTS = [
+    "csg_row_stride_words", "csg_action", "csg_action_host", "csg_interval_sizes", "csg_set_variant",
+    "csg_effective_variant", "csg_set_kernel_timing", "csg_last_kernel_ms", "csg_launch_count",
+    "csg_strerror", "csg_shutdown",
+]
+
+_lib = None
+
+
+class CsgError(RuntimeError):
+    def __init__(self, code, text):
+        super().__init__("libcsg error %d: %s" % (code, text))
+        self.code = code
+
+
+def build(force=False, verbose=False):
+    """Compile libcsg.so in-tree (nvcc, sm_100a)."""
+    return _build.build(force=force, verbose=verbose)
+
+
+def load():
+    """dlopen libcsg.so and declare the prototypes of include/csg.h.  Raises if the library is absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError("%s not built: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                          "(there is no CPU fallback)" % LIB_PATH)
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, i64, ci, dbl = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_double
+    lib.csg_row_stride_words.argtypes = [i64]
+    lib.csg_row_stride_words.restype = i64
+    lib.csg_action.argtypes = [vp, i64, ci, dbl, ci, vp, vp, vp]
+    lib.csg_action.restype = ci
+    lib.csg_action_host.argtypes = [vp, i64, ci, dbl, ci, vp, vp]
+    lib.csg_action_host.restype = ci
+    lib.csg_interval_sizes.argtypes = [vp, i64, vp, i64, vp, vp]
+    lib.csg_interval_sizes.restype = ci
+    lib.csg_set_variant.argtypes = [ci]
+    lib.csg_set_variant.restype = ci
+    lib.csg_effective_variant.argtypes = [i64]
+    lib.csg_effective_variant.restype = ci
+    lib.csg_set_kernel_timing.argtypes = [ci]
+    lib.csg_set_kernel_timing.restype = ci
+    lib.csg_last_kernel_ms.argtypes = [ctypes.POINTER(ctypes.c_float)]
+    lib.csg_last_kernel_ms.restype = ci
+    lib.csg_launch_count.argtypes = []
+    lib.csg_launch_count.restype = i64
+    lib.csg_strerror.argtypes = [ci]
+    lib.csg_strerror.restype = ctypes.c_char_p
+    lib.csg_shutdown.argtypes = []
+    lib.csg_shutdown.restype = ci
+    _lib = lib
+    return lib
+
+
+def _check(code):
+    if code != 0:
+        raise CsgError(code, csg_strerror(code))
+
+
+def csg_strerror(code):
+    return load().csg_strerror(int(code)).decode()
+
+
+def csg_row_stride_words(N):
+    return int(load().csg_row_stride_words(int(N)))
+
+
+def _stream_handle(stream):
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream))
+
+
+def to_device(bits, device="cuda"):
+    """numpy (N, stride) uint64 relation matrix -> CUDA int64 tensor holding the same words."""
+    import torch
+    b = np.ascontiguousarray(bits, dtype=np.uint64)
+    return torch.from_numpy(b.view(np.int64)).to(device)
+
+
+def csg_action(rel_bits, N, dim, eps, kmax, counts=None, S=None, stream=None):
+    """int csg_action(rel_bits, N, dim, eps, kmax, counts, S, stream) -- see include/csg.h.
+
+    rel_bits: CUDA tensor of 64-bit words, N rows of csg_row_stride_words(N).  counts (int64, kmax+1) and
+    S (float64, 1) are allocated on the same device when not given.  Returns (counts, S) device tensors;
+    nothing is synchronised."""
+    import torch
+    lib = load()
+    assert rel_bits.is_cuda and rel_bits.element_size() == 8 and rel_bits.is_contiguous()
+    assert rel_bits.numel() >= int(N) * csg_row_stride_words(N)
+    if counts is None:
+        counts = torch.empty(max(int(kmax), 0) + 1, dtype=torch.int64, device=rel_bits.device)
+    if S is None:
+        S = torch.empty(1, dtype=torch.float64, device=rel_bits.device)
+    _check(lib.csg_action(rel_bits.data_ptr(), int(N), int(dim), float(eps), int(kmax), counts.data_ptr(),
+                          S.data_ptr(), _stream_handle(stream)))
+    return counts, S
+
+
+def csg_action_host(rel_bits, N, dim, eps, kmax):
+    """int csg_action_host(...) with HOST buffers: rel_bits is a numpy uint64 array or a (pinned) CPU torch
+    tensor of 64-bit words.  Returns (counts numpy int64[kmax+1], S float)."""
+    lib = load()
+    if isinstance(rel_bits, np.ndarray):
+        assert rel_bits.dtype in (np.uint64, np.int64) and rel_bits.flags["C_CONTIGUOUS"]
+        ptr, nwords = rel_bits.ctypes.data, rel_bits.size
+    else:
+        assert not rel_bits.is_cuda and rel_bits.element_size() == 8 and rel_bits.is_contiguous()
+        ptr, nwords = rel_bits.data_ptr(), rel_bits.numel()
+    assert nwords >= int(N) * csg_row_stride_words(N)
+    counts = np.empty(max(int(kmax), 0) + 1, dtype=np.int64)
+    S = np.empty(1, dtype=np.float64)
+    _check(lib.csg_action_host(ptr, int(N), int(dim), float(eps), int(kmax), counts.ctypes.data, S.ctypes.data))
+    return counts, float(S[0])
+
+
+def csg_interval_sizes(rel_bits, N, pairs_ij, n_out=None, stream=None):
+    """Test hook: n_ij for listed pairs.  pairs_ij: CUDA int64 tensor (npairs, 2).  Returns int32 tensor."""
+    import torch
+    lib = load()
+    assert rel_bits.is_cuda and pairs_ij.is_cuda and pairs_ij.dtype == torch.int64 and pairs_ij.is_contiguous()
+    npairs = pairs_ij.numel() // 2
+    if n_out is None:
+        n_out = torch.empty(npairs, dtype=torch.int32, device=rel_bits.device)
+    _check(lib.csg_interval_sizes(rel_bits.data_ptr(), int(N), pairs_ij.data_ptr(), npairs, n_out.data_ptr(),
+                                  _stream_handle(stream)))
+    return n_out
+
+
+def csg_set_variant(variant):
+    _check(load().csg_set_variant(int(variant)))
+
+
+def csg_effective_variant(N):
+    return int(load().csg_effective_variant(int(N)))
+
+
+def csg_set_kernel_timing(enable):
+    _check(load().csg_set_kernel_timing(1 if enable else 0))
+
+
+def csg_last_kernel_ms():
+    ms = ctypes.c_float(0.0)
+    _check(load().csg_last_kernel_ms(ctypes.byref(ms)))
+    return float(ms.value)
+
+
+def csg_launch_count():
+    return int(load().csg_launch_count())
+
+
+def csg_shutdown():
+    _check(load().csg_shutdown())

@@ -1,0 +1,358 @@
+// libcsg: C-ABI entry points (include/csg.h), argument validation, cached device workspace, tile
+// schedule, finishing kernel.  Every step of the hot path runs in the kernels of this directory; there is
+// no CPU fallback.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <vector>
+
+#include "../../include/csg.h"
+#include "bitset_kernel.cuh"
+#include "tensor_kernel.cuh"
+
+namespace csg {
+
+// ---------------------------------------------------------------------------------------------- finishing
+// counts -> S.  One CTA.
+//   eps == 1, dim 2: Eq. 4 with n_i = counts[i-1]:  S = 2 (N - 2 N_0 + 4 N_1 - 2 N_2)
+//   eps == 1, dim 4: S = (4/sqrt 6)(N - N_0 + 9 N_1 - 16 N_2 + 8 N_3)   (not in the paper; A8)
+//   eps <  1, dim 2: Eq. 5: S = 2 eps [N - 2 eps sum_k N_k f_2(k, eps)],
+//                    f_2(k,e) = (1-e)^k - 2 e k (1-e)^(k-1) + e^2 k(k-1)/2 (1-e)^(k-2)   (bracket multiplied out)
+// The integer combinations are exact in int64 and below 2^53, so the local S is one exact product.
+// The smeared sum is a fixed-order (thread-strided, compensated, then tree) double reduction: deterministic.
+constexpr int FIN_THREADS = 1024;
+
+__global__ void __launch_bounds__(FIN_THREADS, 1)
+finish_action_kernel(const long long* __restrict__ counts, long long N, int dim, double eps, int kmax,
+                     double* __restrict__ S) {
+    __shared__ double red[FIN_THREADS];
+    const int tid = threadIdx.x;
+    if (eps == 1.0) {
+        if (tid == 0) {
+            if (dim == 2) {
+                const long long I2 = N - 2 * counts[0] + 4 * counts[1] - 2 * counts[2];
+                *S = 2.0 * (double)I2;
+            } else {
+                const long long I4 = N - counts[0] + 9 * counts[1] - 16 * counts[2] + 8 * counts[3];
+                *S = (4.0 / sqrt(6.0)) * (double)I4;
+            }
+        }
+        return;
+    }
+    const double x = 1.0 - eps;
+    double sum = 0.0, comp = 0.0;
+    for (long long k = tid; k <= kmax; k += FIN_THREADS) {
+        const long long c = counts[k];
+        if (c == 0) continue;
+        const double dk = (double)k;
+        double w = pow(x, dk);
+        if (k >= 1) w -= 2.0 * eps * dk * pow(x, dk - 1.0);
+        if (k >= 2) w += 0.5 * eps * eps * dk * (dk - 1.0) * pow(x, dk - 2.0);
+        const double term = (double)c * w;
+        const double y = term - comp;
+        const double t = sum + y;
+        comp = (t - sum) - y;
+        sum = t;
+    }
+    red[tid] = sum;
+    __syncthreads();
+    for (int s = FIN_THREADS / 2; s > 0; s >>= 1) {
+        if (tid < s) red[tid] += red[tid + s];
+        __syncthreads();
+    }
+    if (tid == 0) *S = 2.0 * eps * ((double)N - 2.0 * eps * red[0]);
+}
+
+// ---------------------------------------------------------------------------------------------- host state
+struct State {
+    std::mutex mu;
+    int variant = CSG_VARIANT_AUTO;
+    bool timing = false;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    bool ev_valid = false;
+    long long launches = 0;
+    char cuda_msg[256] = "no CUDA error recorded";
+    // cached tile schedule of the tensor variant
+    long long tiles_N = -1;
+    int2* d_tiles = nullptr;
+    int ntiles = 0;
+    std::vector<int2> h_tiles;
+    int sm_count = 0;
+    bool attr_set = false;
+    // end-to-end (host buffer) path
+    cudaStream_t host_stream = nullptr;
+    uint64_t* d_bits = nullptr;
+    size_t d_bits_bytes = 0;
+    long long* d_counts = nullptr;
+    size_t d_counts_bytes = 0;
+    double* d_S = nullptr;
+};
+static State g;
+
+static int cuda_fail(cudaError_t e, const char* what) {
+    snprintf(g.cuda_msg, sizeof(g.cuda_msg), "%s: %s", what, cudaGetErrorString(e));
+    cudaGetLastError();  // clear the sticky-less error state
+    return CSG_E_CUDA;
+}
+#define CSG_CUDA(call)                                   \
+    do {                                                 \
+        cudaError_t e_ = (call);                         \
+        if (e_ != cudaSuccess) return cuda_fail(e_, #call); \
+    } while (0)
+
+static int ensure_device() {
+    if (g.sm_count > 0) return CSG_OK;
+    int dev = 0;
+    CSG_CUDA(cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    CSG_CUDA(cudaGetDeviceProperties(&prop, dev));
+    if (prop.major != 10) {
+        snprintf(g.cuda_msg, sizeof(g.cuda_msg), "device is sm_%d%d; libcsg is built for sm_100a only", prop.major,
+                 prop.minor);
+        return CSG_E_CUDA;
+    }
+    g.sm_count = prop.multiProcessorCount;
+    return CSG_OK;
+}
+
+static int effective_variant(long long N) {
+    if (g.variant != CSG_VARIANT_AUTO) return g.variant;
+    return N >= 2048 ? CSG_VARIANT_TENSOR : CSG_VARIANT_BITSET;
+}
+
+// Tiles (I, J) of the tensor variant: I = block of 128 rows i, J = block of 256 rows j; a tile is needed
+// iff it holds some pair i<j.  K-depth in 128-column stages = 2J+2-I.  Sorted longest first.
+static int ensure_tiles(long long N, cudaStream_t stream) {
+    if (g.tiles_N == N && g.d_tiles) return CSG_OK;
+    const int nI = (int)((N + TC_TM - 1) / TC_TM), nJ = (int)((N + TC_TN - 1) / TC_TN);
+    g.h_tiles.clear();
+    for (int J = 0; J < nJ; ++J)
+        for (int I = 0; I < nI && I <= 2 * J + 1; ++I) g.h_tiles.push_back(make_int2(I, J));
+    std::stable_sort(g.h_tiles.begin(), g.h_tiles.end(), [](const int2& a, const int2& b) {
+        return (2 * a.y + 2 - a.x) > (2 * b.y + 2 - b.x);
+    });
+    if (g.d_tiles) {
+        CSG_CUDA(cudaStreamSynchronize(stream));
+        CSG_CUDA(cudaFree(g.d_tiles));
+        g.d_tiles = nullptr;
+    }
+    g.ntiles = (int)g.h_tiles.size();
+    CSG_CUDA(cudaMalloc(&g.d_tiles, std::max<size_t>(1, g.h_tiles.size()) * sizeof(int2)));
+    CSG_CUDA(cudaMemcpyAsync(g.d_tiles, g.h_tiles.data(), g.h_tiles.size() * sizeof(int2), cudaMemcpyHostToDevice,
+                             stream));
+    g.tiles_N = N;
+    return CSG_OK;
+}
+
+static int validate(const void* rel_bits, long long N, int dim, double eps, int kmax, const void* counts,
+                    const void* S) {
+    if (!rel_bits || !counts || !S) return CSG_E_NULL;
+    if (N < 1 || N > CSG_MAX_N) return CSG_E_SIZE;
+    if (dim != 2 && dim != 4) return CSG_E_DIM;
+    if (!(eps > 0.0 && eps <= 1.0)) return CSG_E_EPS;  // also rejects NaN
+    if (kmax < 0 || kmax > CSG_MAX_KMAX) return CSG_E_KMAX;
+    if (eps == 1.0 && kmax < (dim == 2 ? 2 : 3)) return CSG_E_KMAX;
+    if (eps < 1.0 && dim == 4) return CSG_E_UNSUPPORTED;
+    return CSG_OK;
+}
+
+static int action_device(const uint64_t* rel_bits, long long N, int dim, double eps, int kmax, long long* counts,
+                         double* S, cudaStream_t stream) {
+    int rc = ensure_device();
+    if (rc) return rc;
+    const long long stride = csg_row_stride_words(N);
+    CSG_CUDA(cudaMemsetAsync(counts, 0, (size_t)(kmax + 1) * sizeof(long long), stream));
+    const int variant = effective_variant(N);
+    if (variant == CSG_VARIANT_TENSOR) {
+        rc = ensure_tiles(N, stream);
+        if (rc) return rc;
+        if (!g.attr_set) {
+            CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          TC_SMEM_BYTES));
+            g.attr_set = true;
+        }
+    }
+    if (g.timing) {
+        if (!g.ev0) {
+            CSG_CUDA(cudaEventCreate(&g.ev0));
+            CSG_CUDA(cudaEventCreate(&g.ev1));
+        }
+        CSG_CUDA(cudaEventRecord(g.ev0, stream));
+    }
+    if (variant == CSG_VARIANT_TENSOR) {
+        const int grid = std::max(1, std::min(g.ntiles, g.sm_count));
+        tensor_action_kernel<<<grid, TC_THREADS, TC_SMEM_BYTES, stream>>>(
+            rel_bits, N, stride, kmax, reinterpret_cast<unsigned long long*>(counts), g.d_tiles, g.ntiles);
+    } else {
+        const long long nb = (N + BS_T - 1) / BS_T;
+        const long long ntiles = nb * (nb + 1) / 2;
+        const int grid = (int)std::max<long long>(1, std::min<long long>(ntiles, (long long)g.sm_count * 2));
+        bitset_action_kernel<<<grid, BS_THREADS, 0, stream>>>(reinterpret_cast<const uint32_t*>(rel_bits), N,
+                                                               stride * 2, kmax,
+                                                               reinterpret_cast<unsigned long long*>(counts), nb,
+                                                               ntiles);
+    }
+    CSG_CUDA(cudaGetLastError());
+    ++g.launches;
+    if (g.timing) {
+        CSG_CUDA(cudaEventRecord(g.ev1, stream));
+        g.ev_valid = true;
+    }
+    finish_action_kernel<<<1, FIN_THREADS, 0, stream>>>(counts, N, dim, eps, kmax, S);
+    CSG_CUDA(cudaGetLastError());
+    ++g.launches;
+    return CSG_OK;
+}
+
+}  // namespace csg
+
+using namespace csg;
+
+extern "C" {
+
+int64_t csg_row_stride_words(int64_t N) { return N < 1 ? 0 : 4 * ((N + 255) / 256); }
+
+int csg_action(const uint64_t* rel_bits, int64_t N, int dim, double eps, int kmax, int64_t* counts, double* S,
+               cudaStream_t stream) {
+    std::lock_guard<std::mutex> lock(g.mu);
+    int rc = validate(rel_bits, N, dim, eps, kmax, counts, S);
+    if (rc) return rc;
+    if ((reinterpret_cast<uintptr_t>(rel_bits) & 15) || (reinterpret_cast<uintptr_t>(counts) & 7) ||
+        (reinterpret_cast<uintptr_t>(S) & 7))
+        return CSG_E_ALIGN;
+    return action_device(rel_bits, N, dim, eps, kmax, reinterpret_cast<long long*>(counts), S, stream);
+}
+
+int csg_action_host(const uint64_t* rel_bits_host, int64_t N, int dim, double eps, int kmax, int64_t* counts_host,
+                    double* S_host) {
+    std::lock_guard<std::mutex> lock(g.mu);
+    int rc = validate(rel_bits_host, N, dim, eps, kmax, counts_host, S_host);
+    if (rc) return rc;
+    rc = ensure_device();
+    if (rc) return rc;
+    if (!g.host_stream) CSG_CUDA(cudaStreamCreateWithFlags(&g.host_stream, cudaStreamNonBlocking));
+    const size_t bits_bytes = (size_t)N * (size_t)csg_row_stride_words(N) * sizeof(uint64_t);
+    const size_t counts_bytes = (size_t)(kmax + 1) * sizeof(long long);
+    if (g.d_bits_bytes < bits_bytes) {
+        if (g.d_bits) CSG_CUDA(cudaFree(g.d_bits));
+        g.d_bits = nullptr;
+        g.d_bits_bytes = 0;
+        CSG_CUDA(cudaMalloc(&g.d_bits, bits_bytes));
+        g.d_bits_bytes = bits_bytes;
+    }
+    if (g.d_counts_bytes < counts_bytes) {
+        if (g.d_counts) CSG_CUDA(cudaFree(g.d_counts));
+        g.d_counts = nullptr;
+        g.d_counts_bytes = 0;
+        CSG_CUDA(cudaMalloc(&g.d_counts, counts_bytes));
+        g.d_counts_bytes = counts_bytes;
+    }
+    if (!g.d_S) CSG_CUDA(cudaMalloc(&g.d_S, sizeof(double)));
+    CSG_CUDA(cudaMemcpyAsync(g.d_bits, rel_bits_host, bits_bytes, cudaMemcpyHostToDevice, g.host_stream));
+    rc = action_device(g.d_bits, N, dim, eps, kmax, g.d_counts, g.d_S, g.host_stream);
+    if (rc) return rc;
+    CSG_CUDA(cudaMemcpyAsync(counts_host, g.d_counts, counts_bytes, cudaMemcpyDeviceToHost, g.host_stream));
+    CSG_CUDA(cudaMemcpyAsync(S_host, g.d_S, sizeof(double), cudaMemcpyDeviceToHost, g.host_stream));
+    CSG_CUDA(cudaStreamSynchronize(g.host_stream));
+    return CSG_OK;
+}
+
+int csg_interval_sizes(const uint64_t* rel_bits, int64_t N, const int64_t* pairs_ij, int64_t npairs, int32_t* n_out,
+                       cudaStream_t stream) {
+    std::lock_guard<std::mutex> lock(g.mu);
+    if (!rel_bits || (npairs > 0 && (!pairs_ij || !n_out))) return CSG_E_NULL;
+    if (N < 1 || N > CSG_MAX_N || npairs < 0) return CSG_E_SIZE;
+    if (reinterpret_cast<uintptr_t>(rel_bits) & 15) return CSG_E_ALIGN;
+    int rc = ensure_device();
+    if (rc) return rc;
+    if (npairs == 0) return CSG_OK;
+    const int warps_per_block = 8;
+    const long long blocks = (npairs + warps_per_block - 1) / warps_per_block;
+    pair_interval_kernel<<<(unsigned)blocks, warps_per_block * 32, 0, stream>>>(
+        reinterpret_cast<const uint32_t*>(rel_bits), N, csg_row_stride_words(N) * 2,
+        reinterpret_cast<const long long*>(pairs_ij), npairs, n_out);
+    CSG_CUDA(cudaGetLastError());
+    ++g.launches;
+    return CSG_OK;
+}
+
+int csg_set_variant(int variant) {
+    std::lock_guard<std::mutex> lock(g.mu);
+    if (variant != CSG_VARIANT_AUTO && variant != CSG_VARIANT_BITSET && variant != CSG_VARIANT_TENSOR)
+        return CSG_E_VARIANT;
+    g.variant = variant;
+    return CSG_OK;
+}
+
+int csg_effective_variant(int64_t N) {
+    std::lock_guard<std::mutex> lock(g.mu);
+    return effective_variant(N);
+}
+
+int csg_set_kernel_timing(int enable) {
+    std::lock_guard<std::mutex> lock(g.mu);
+    g.timing = enable != 0;
+    if (!g.timing) g.ev_valid = false;
+    return CSG_OK;
+}
+
+int csg_last_kernel_ms(float* ms) {
+    std::lock_guard<std::mutex> lock(g.mu);
+    if (!ms) return CSG_E_NULL;
+    if (!g.ev_valid) {
+        snprintf(g.cuda_msg, sizeof(g.cuda_msg), "csg_last_kernel_ms: no timed csg_action call yet");
+        return CSG_E_CUDA;
+    }
+    CSG_CUDA(cudaEventSynchronize(g.ev1));
+    CSG_CUDA(cudaEventElapsedTime(ms, g.ev0, g.ev1));
+    return CSG_OK;
+}
+
+int64_t csg_launch_count(void) {
+    std::lock_guard<std::mutex> lock(g.mu);
+    return g.launches;
+}
+
+const char* csg_strerror(int code) {
+    switch (code) {
+        case CSG_OK: return "success";
+        case CSG_E_NULL: return "null pointer";
+        case CSG_E_SIZE: return "N or npairs out of range";
+        case CSG_E_ALIGN: return "misaligned buffer (rel_bits needs 16 bytes, counts and S 8 bytes)";
+        case CSG_E_DIM: return "dim must be 2 or 4";
+        case CSG_E_EPS: return "eps must be in (0, 1]";
+        case CSG_E_KMAX: return "kmax out of range (local action needs kmax >= 2 in 2D, >= 3 in 4D)";
+        case CSG_E_UNSUPPORTED: return "smeared action is defined for dim 2 only";
+        case CSG_E_CUDA: return g.cuda_msg;
+        case CSG_E_VARIANT: return "unknown variant";
+        default: return "unknown error code";
+    }
+}
+
+int csg_shutdown(void) {
+    std::lock_guard<std::mutex> lock(g.mu);
+    if (g.d_tiles) cudaFree(g.d_tiles);
+    if (g.d_bits) cudaFree(g.d_bits);
+    if (g.d_counts) cudaFree(g.d_counts);
+    if (g.d_S) cudaFree(g.d_S);
+    if (g.ev0) cudaEventDestroy(g.ev0);
+    if (g.ev1) cudaEventDestroy(g.ev1);
+    if (g.host_stream) cudaStreamDestroy(g.host_stream);
+    g.d_tiles = nullptr;
+    g.d_bits = nullptr;
+    g.d_counts = nullptr;
+    g.d_S = nullptr;
+    g.ev0 = g.ev1 = nullptr;
+    g.host_stream = nullptr;
+    g.tiles_N = -1;
+    g.d_bits_bytes = g.d_counts_bytes = 0;
+    g.ev_valid = false;
+    cudaGetLastError();
+    return CSG_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,237 @@
+"""Parity of the CUDA path (through the C ABI) with the oracle, element by element, on the same seeded
+inputs.  Counts are int64 and must match bit for bit; the local action is an exact integer times a constant
+and must match exactly; the smeared action within 1e-12 of its term scale."""
+import math
+
+import numpy as np
+import pytest
+
+import csg_inputs
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def csg():
+    import paper_1709_03013_b200 as m
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    if m._build.needs_build():
+        m.build()
+    m.load()
+    yield m
+    m.csg_set_variant(m.VARIANT_AUTO)
+
+
+VARIANTS = [1, 2]
+
+
+def run_action(csg, bits, N, dim, eps, kmax, variant):
+    csg.csg_set_variant(variant)
+    counts, S = csg.csg_action(csg.to_device(bits), N, dim, eps, kmax)
+    torch.cuda.synchronize()
+    return counts.cpu().numpy(), float(S.item())
+
+
+def reference_counts(bits, N, kmax):
+    return oracle.counts_from_bits(bits, N, kmax) if N <= 1200 else oracle.alg5_counts(bits, N, kmax)
+
+
+# --------------------------------------------------------------------------- small and ragged sizes
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("N", [1, 2, 3, 31, 63, 64, 65, 127, 128, 129, 255, 256, 257, 383, 385, 511, 513, 777, 1025])
+def test_random_posets_full_histogram(csg, variant, N):
+    for transitive in (True, False):
+        _, bits = csg_inputs.random_poset_bits(N, min(0.5, 8.0 / max(N, 1) + 0.02), seed=N, transitive=transitive)
+        kmax = max(N - 2, 3)
+        want = oracle.counts_from_bits(bits, N, kmax)
+        got, S = run_action(csg, bits, N, 2, 1.0, kmax, variant)
+        assert (got == want).all(), (N, transitive, np.nonzero(got != want)[0][:10])
+        assert S == oracle.action_local(2, N, want)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("dim,N,seed", [(2, 300, 1), (4, 300, 2), (2, 1500, 3), (4, 1500, 4), (4, 2600, 5), (2, 3000, 6)])
+def test_sprinkled_local_action(csg, variant, dim, N, seed):
+    _, bits = csg_inputs.make_causet(dim, N, seed)
+    want = reference_counts(bits, N, 3)
+    got, S = run_action(csg, bits, N, dim, 1.0, 3, variant)
+    assert (got == want).all(), (got, want)
+    assert S == oracle.action_local(dim, N, want)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("N,eps", [(700, 0.1), (1500, 2.0 ** -6), (2100, 0.5)])
+def test_smeared_action_full_histogram(csg, variant, N, eps):
+    _, bits = csg_inputs.make_causet(2, N, 40 + N)
+    want = reference_counts(bits, N, N - 2)
+    got, S = run_action(csg, bits, N, 2, eps, N - 2, variant)
+    assert (got == want).all()
+    s_want, scale = oracle.action_smeared_2d(N, want, eps)
+    assert abs(S - s_want) <= 1e-12 * scale, (S, s_want, scale)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_kmax_truncation_and_dense_chain(csg, variant):
+    """Total order of 600 elements: N_k = N-1-k (largest possible interval sizes); kmax cuts, never clamps."""
+    N = 600
+    bits = csg_inputs.pack_dense(np.triu(np.ones((N, N)), 1))
+    got, S = run_action(csg, bits, N, 2, 1.0, N - 2, variant)
+    assert (got == N - 1 - np.arange(N - 1)).all() and S == 2.0 * N
+    got, _ = run_action(csg, bits, N, 4, 1.0, 10, variant)
+    assert (got == N - 1 - np.arange(11)).all()
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_empty_relation_and_dirty_diagonal(csg, variant):
+    N = 500
+    got, S = run_action(csg, csg_inputs.pack_dense(np.zeros((N, N))), N, 4, 1.0, 3, variant)
+    assert got.sum() == 0 and S == (4.0 / math.sqrt(6.0)) * N
+    up, bits = csg_inputs.random_poset_bits(N, 0.05, seed=3)
+    want = oracle.counts_from_bits(bits, N, N - 2)
+    dirty = bits.copy()
+    for r in range(N):
+        dirty[r, r // 64] |= np.uint64(1) << np.uint64(r % 64)
+    got, _ = run_action(csg, dirty, N, 2, 1.0, N - 2, variant)
+    assert (got == want).all()
+
+
+def test_repeat_calls_are_deterministic_and_overwrite(csg):
+    _, bits = csg_inputs.make_causet(2, 2500, 9)
+    d = csg.to_device(bits)
+    csg.csg_set_variant(csg.VARIANT_TENSOR)
+    counts = torch.full((2499,), 77, dtype=torch.int64, device="cuda")
+    S = torch.zeros(1, dtype=torch.float64, device="cuda")
+    outs = []
+    for _ in range(3):
+        csg.csg_action(d, 2500, 2, 0.1, 2498, counts, S)
+        torch.cuda.synchronize()
+        outs.append((counts.cpu().numpy().copy(), S.item()))
+    assert all((o[0] == outs[0][0]).all() and o[1] == outs[0][1] for o in outs)
+    assert (outs[0][0] == oracle.alg5_counts(bits, 2500, 2498)).all()
+
+
+def test_host_entry_point(csg):
+    _, bits = csg_inputs.make_causet(4, 2300, 10)
+    csg.csg_set_variant(csg.VARIANT_AUTO)
+    counts, S = csg.csg_action_host(bits, 2300, 4, 1.0, 3)
+    want = oracle.alg5_counts(bits, 2300, 3)
+    assert (counts == want).all() and S == oracle.action_local(4, 2300, want)
+    pinned = torch.from_numpy(bits.view(np.int64)).pin_memory()
+    counts2, S2 = csg.csg_action_host(pinned, 2300, 4, 1.0, 3)
+    assert (counts2 == want).all() and S2 == S
+
+
+def test_interval_sizes_hook(csg):
+    N = 3000
+    _, bits = csg_inputs.make_causet(4, N, 11)
+    rng = np.random.default_rng(0)
+    pairs = rng.integers(0, N, size=(4000, 2))
+    pairs = np.concatenate([pairs, [[0, N - 1], [5, 5], [9, 3], [N - 2, N - 1], [0, 1], [63, 64], [64, 127]]])
+    got = csg.csg_interval_sizes(csg.to_device(bits), N, torch.from_numpy(pairs.astype(np.int64)).cuda())
+    torch.cuda.synchronize()
+    got = got.cpu().numpy()
+    for (i, j), n in zip(pairs, got):
+        assert n == oracle.pair_interval(bits, N, i, j), (i, j)
+
+
+def test_error_codes_on_device(csg):
+    d = torch.zeros(64, dtype=torch.int64, device="cuda")
+    with pytest.raises(csg.CsgError) as e:
+        csg._check(csg.load().csg_action(d.data_ptr() + 8, 8, 2, 1.0, 3, d.data_ptr(), d.data_ptr(), None))
+    assert e.value.code == -3
+    with pytest.raises(csg.CsgError) as e:
+        csg._check(csg.load().csg_action(None, 8, 2, 1.0, 3, d.data_ptr(), d.data_ptr(), None))
+    assert e.value.code == -1
+
+
+# --------------------------------------------------------------------------- BASELINE.json configs
+def degree_invariants(bits, N):
+    """#relations and sum_k in_k*out_k from row popcounts (O(N^2/64), no N^3 code): for a transitive set the
+    second equals the number of 3-chains = sum_k k N_k (pin P4)."""
+    W = bits.shape[1]
+    indeg = np.zeros(N, np.int64)
+    outdeg = np.zeros(N, np.int64)
+    cols = np.arange(W)
+    for r0 in range(0, N, 2048):
+        blk = bits[r0:r0 + 2048]
+        pc = np.bitwise_count(blk).astype(np.int64)
+        rows = np.arange(r0, r0 + blk.shape[0])
+        wi = rows // 64
+        below = (pc * (cols[None, :] < wi[:, None])).sum(1)
+        own = blk[np.arange(blk.shape[0]), wi]
+        lowmask = (np.uint64(1) << (rows % 64).astype(np.uint64)) - np.uint64(1)
+        below += np.bitwise_count(own & lowmask).astype(np.int64)
+        indeg[rows] = below
+        outdeg[rows] = pc.sum(1) - below
+    return int(outdeg.sum()), int((indeg * outdeg).sum())
+
+
+def check_config(csg, cfg, full_reference):
+    N, dim = cfg["N"], cfg["dim"]
+    _, bits = csg_inputs.make_causet(dim, N, cfg["seed"])
+    d = csg.to_device(bits)
+    csg.csg_set_variant(csg.VARIANT_AUTO)
+    # (1) the configuration as benchmarked
+    counts, S = csg.csg_action(d, N, dim, cfg["eps"], cfg["kmax"])
+    torch.cuda.synchronize()
+    counts = counts.cpu().numpy()
+    # (2) full histogram through the same launch configuration: properties that hold at any size
+    full, _ = csg.csg_action(d, N, 2, 1.0, N - 2)
+    torch.cuda.synchronize()
+    full = full.cpu().numpy()
+    assert (full[:cfg["kmax"] + 1] == counts).all()
+    nrel, chains = degree_invariants(bits, N)
+    assert full.sum() == nrel                                         # I1
+    assert int((np.arange(N - 1, dtype=object) * full.astype(object)).sum()) == chains   # I2 = I3
+    # (3) sampled outputs the oracle computes one by one
+    rng = np.random.default_rng(cfg["seed"])
+    pairs = np.sort(rng.integers(0, N, size=(300, 2)), axis=1).astype(np.int64)
+    got = csg.csg_interval_sizes(d, N, torch.from_numpy(pairs).cuda()).cpu().numpy()
+    for (i, j), n in zip(pairs[:60], got[:60]):
+        assert n == oracle.pair_interval(bits, N, i, j)
+    # (4) exact reference histogram where Algorithm 5 finishes in reasonable time
+    if full_reference:
+        want = oracle.alg5_counts(bits, N, cfg["kmax"])
+        assert (counts == want).all(), (counts, want)
+        if cfg["eps"] == 1.0:
+            assert float(S.item()) == oracle.action_local(dim, N, want)
+    if cfg["eps"] < 1.0:
+        s_want, scale = oracle.action_smeared_2d(N, full, cfg["eps"])   # oracle arithmetic on the counts
+        assert abs(float(S.item()) - s_want) <= 1e-12 * scale
+    return counts, float(S.item())
+
+
+def test_config0_plain_oracle(csg):
+    cfg = csg_inputs.CONFIGS[0]
+    _, bits = csg_inputs.make_causet(cfg["dim"], cfg["N"], cfg["seed"])
+    want = oracle.counts_from_bits(bits, cfg["N"], cfg["kmax"])
+    for variant in VARIANTS:
+        got, S = run_action(csg, bits, cfg["N"], cfg["dim"], 1.0, cfg["kmax"], variant)
+        assert (got == want).all() and S == oracle.action_local(2, cfg["N"], want)
+
+
+def test_config1(csg):
+    check_config(csg, csg_inputs.CONFIGS[1], full_reference=True)
+    cfg = csg_inputs.CONFIGS[1]
+    _, bits = csg_inputs.make_causet(cfg["dim"], cfg["N"], cfg["seed"])
+    want = oracle.alg5_counts(bits, cfg["N"], 3)
+    got, _ = run_action(csg, bits, cfg["N"], 2, 1.0, 3, 1)            # bitset variant too
+    assert (got == want).all()
+
+
+@pytest.mark.slow
+def test_config2(csg):
+    check_config(csg, csg_inputs.CONFIGS[2], full_reference=True)
+
+
+@pytest.mark.slow
+def test_config3_headline(csg):
+    check_config(csg, csg_inputs.CONFIGS[3], full_reference=True)
+
+
+@pytest.mark.slow
+def test_config4_smeared(csg):
+    check_config(csg, csg_inputs.CONFIGS[4], full_reference=False)
