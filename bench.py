@@ -1,0 +1,364 @@
+#!/usr/bin/env python
+"""bench.py -- Benincasa-Dowker action throughput on B200 (contract: see DESIGN.md "Measurement").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 0..4] [--variant 0|1|2]
+
+One "step" = one whole pass of the hot path (csg_action: relation test, interval sizes, histogram, action) over
+one synthetic causal set.  Default workload = BASELINE.json configs[3]: 4D Minkowski diamond, N = 131072
+(2 GiB bitset, larger than the 126 MB L2, so no flush is needed between steps).  metric = ordered-triple tests
+per second = C(N,3) / time.  N > 1 ranks (torchrun): every rank owns an independent causal set of the same
+ensemble (seed + 1000*rank); no data-path collective; value = all ranks' triples / max-over-ranks time.
+
+Prints ONE JSON line on rank 0.  `--impl reference` times the oracle (Algorithm 5 restated, oracle/alg5_packed.c)
+on the host cores on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "ordered_triple_tests_per_s"
+UNIT = "triple-tests/s"
+
+
+def comb3(n):
+    return n * (n - 1) * (n - 2) // 6
+
+
+def workload_name(cfg):
+    return "%dD Minkowski diamond N=%d %s (BASELINE.json configs[%d])" % (
+        cfg["dim"], cfg["N"], "local action" if cfg["eps"] == 1.0 else "smeared eps=%g" % cfg["eps"], cfg["index"])
+
+
+def read_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        p = json.load(open(path))
+        return dict(bf16=float(p["bf16_tflops"]), bf16_sustained=float(p.get("bf16_tflops_sustained", p["bf16_tflops"])),
+                    hbm=float(p["hbm_gbs"]), source="measured (MEASURED_PEAKS.json)")
+    return dict(bf16=1590.0, bf16_sustained=1400.0, hbm=6650.0, source="fallback (B200_PROFILING.md)")
+
+
+def read_traffic(kernel):
+    """dram bytes per launch of the dominant kernel from the committed ncu --set full summary, or None."""
+    path = os.path.join(ROOT, "profiles", "dram_traffic.json")
+    if not os.path.exists(path):
+        return None
+    return json.load(open(path)).get(kernel)
+
+
+# ------------------------------------------------------------------------------------------- clocks sampler
+class ClockSampler:
+    """nvidia-smi sampling of SM clock and throttle reasons while the timed region runs."""
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.gpu_index = gpu_index
+        self.proc = None
+        self.tmp = None
+
+    def start(self):
+        try:
+            self.tmp = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.gpu_index), "--query-gpu=" + self.FIELDS, "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=self.tmp, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        self.tmp.flush()
+        self.tmp.seek(0)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.tmp.read().splitlines():
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1])); pw.append(float(parts[2]))
+            except ValueError:
+                continue
+            for name, val in zip(names, parts[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        self.tmp.close()
+        os.unlink(self.tmp.name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(mx), "power_w_max": max(pw), "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------- oracle legs
+def oracle_sample(bits, N, kmax, target_s, nblocks=16):
+    """Time Algorithm 5 (oracle/alg5_packed.c, all host threads) on `nblocks` row blocks spread evenly over
+    the causal set, sized from a calibration block so that the whole sample takes about target_s seconds.
+    Returns (triple tests covered, seconds, rows, threads)."""
+    import oracle
+    oracle.build()
+    t0 = time.perf_counter()
+    # calibration: one row per host thread from each of 4 places
+    tests = 0
+    for b in range(4):
+        r0 = min(N - 1, (2 * b + 1) * N // 8)
+        _, t = oracle.alg5_counts_rows(bits, N, kmax, r0, min(N, r0 + oracle.alg5_threads()))
+        tests += t
+    dt = max(time.perf_counter() - t0, 1e-4)
+    rate = tests / dt
+    total_rows = 0
+    want_tests = rate * target_s
+    # rows per block so that the blocks together stand for ~want_tests (mean row stands for ~N^2/6 tests)
+    per_row = max(1.0, N * N / 6.0)
+    rows_per_block = int(max(1, min(N // nblocks, want_tests / per_row / nblocks)))
+    t0 = time.perf_counter()
+    tests = 0
+    for b in range(nblocks):
+        r0 = (2 * b + 1) * N // (2 * nblocks)
+        r1 = min(N, r0 + rows_per_block)
+        _, t = oracle.alg5_counts_rows(bits, N, kmax, r0, r1)
+        tests += t
+        total_rows += r1 - r0
+    dt = time.perf_counter() - t0
+    return tests, dt, total_rows, oracle.alg5_threads()
+
+
+def plain_oracle_sample(bits, N, kmax, n_sub=3072):
+    """The plain single-thread triple loop (oracle/csg_oracle.c) on the sub-causal-set made of the first n_sub
+    elements of the workload (an order-ideal of the same sprinkling)."""
+    import numpy as np
+    import oracle
+    n = min(N, n_sub)
+    sub = np.ascontiguousarray(bits[:n])
+    B = oracle.expand(sub, n)
+    t0 = time.perf_counter()
+    oracle.counts_plain(B, min(kmax, max(n - 2, 0)))
+    dt = time.perf_counter() - t0
+    return comb3(n), dt, n
+
+
+def run_reference(args, cfg, rank, world):
+    if rank != 0:
+        return 0
+    import csg_inputs
+    csg_inputs.build()
+    N, dim, kmax = cfg["N"], cfg["dim"], cfg["kmax"]
+    _, bits = csg_inputs.make_causet(dim, N, cfg["seed"])
+    per_step_s = 4.0
+    for _ in range(args.warmup):
+        oracle_sample(bits, N, kmax, 0.5, nblocks=4)
+    tests_total, secs_total, rows, threads = 0, 0.0, 0, 1
+    for _ in range(args.steps):
+        tests, dt, r, threads = oracle_sample(bits, N, kmax, per_step_s)
+        tests_total += tests; secs_total += dt; rows += r
+    value = tests_total / secs_total
+    sample = ("Algorithm 5 (oracle/alg5_packed.c) on %d rows per step in 16 evenly spaced row blocks of the same "
+              "causal set; tests = sum over visited pairs of (j-i-1)" % (rows // max(args.steps, 1)))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * secs_total / max(args.steps, 1), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "u64 bit ops (host)", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "N": N, "dim": dim, "eps": cfg["eps"], "kmax": kmax,
+                   "seed": cfg["seed"], "note": "each step is a bounded sample of the workload"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------------------- our arm
+def run_ours(args, cfg, rank, local_rank, world):
+    import numpy as np
+    import torch
+    import csg_inputs
+    import paper_1709_03013_b200 as csg
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; libcsg has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    if csg._build.needs_build():
+        if local_rank == 0:
+            csg.build()
+        if dist is not None:
+            dist.barrier()
+    csg.load()
+    csg_inputs.build()
+    csg.csg_set_variant(args.variant)
+
+    N, dim, eps, kmax = cfg["N"], cfg["dim"], cfg["eps"], cfg["kmax"]
+    seed = cfg["seed"] + 1000 * rank
+    t0 = time.perf_counter()
+    _, bits = csg_inputs.make_causet(dim, N, seed)
+    gen_s = time.perf_counter() - t0
+    host = torch.from_numpy(bits.view(np.int64)).pin_memory()
+    d_bits = host.to("cuda", non_blocking=False)
+    counts = torch.empty(kmax + 1, dtype=torch.int64, device="cuda")
+    S = torch.empty(1, dtype=torch.float64, device="cuda")
+    variant = csg.csg_effective_variant(N)
+    kernel_name = "tensor_action_kernel" if variant == csg.VARIANT_TENSOR else "bitset_action_kernel"
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step():
+        csg.csg_action(d_bits, N, dim, eps, kmax, counts, S)
+
+    # ---- device-resident leg
+    csg.csg_set_kernel_timing(True)
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    launches0 = csg.csg_launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record()
+    for _ in range(args.steps):
+        step()
+    ev1.record()
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    launches = csg.csg_launch_count() - launches0
+    ms_total = ev0.elapsed_time(ev1)
+    kernel_ms = csg.csg_kernel_ms_history(min(args.steps, 64))
+    csg.csg_set_kernel_timing(False)
+    result_counts = counts.cpu().numpy().copy()
+    result_S = float(S.item())
+
+    # ---- end-to-end leg: HOST buffers through csg_action_host (H2D of the bitset + D2H of counts, S inside)
+    e2e_steps = max(1, min(args.steps, 3))
+    csg.csg_action_host(host, N, dim, eps, kmax)   # warm-up (allocates the library's device buffers)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        c_host, S_host = csg.csg_action_host(host, N, dim, eps, kmax)
+    e2e_s = time.perf_counter() - t0
+    assert (c_host == result_counts).all() and S_host == result_S, "e2e and device legs disagree"
+
+    t = torch.tensor([ms_total, 1e3 * e2e_s], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total, e2e_ms = float(t[0]), float(t[1])
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    triples = comb3(N)
+    value = world * triples * args.steps / (ms_total * 1e-3)
+    e2e_value = world * triples * e2e_steps / (e2e_ms * 1e-3)
+    k_ms = sum(kernel_ms) / len(kernel_ms)
+    peaks = read_peaks()
+    if variant == csg.VARIANT_TENSOR:
+        # dense binary contraction on tcgen05 kind::i8: 1 triple test = 1 MAC = 2 int8 ops.
+        # peak = measured bf16 dense peak x 2 (nominal int8:bf16 ratio of B200, B200_PROFILING.md table).
+        achieved = 2.0 * triples / (k_ms * 1e-3) / 1e12
+        roofline = {"bound": "tensor", "kernel": kernel_name, "achieved": achieved, "peak": 2.0 * peaks["bf16"],
+                    "unit": "TOP/s (int8)", "frac": achieved / (2.0 * peaks["bf16"]),
+                    "peak_sustained": 2.0 * peaks["bf16_sustained"],
+                    "frac_of_sustained": achieved / (2.0 * peaks["bf16_sustained"]),
+                    "peak_source": "2 x bf16 " + peaks["source"], "kernel_ms": k_ms,
+                    "traffic": read_traffic(kernel_name)}
+    else:
+        # LOP3+POPC+IADD per 32 triple tests; POPC pipe 16 lanes/clk/SM x 148 SMs x 1.965 GHz
+        peak = 16 * 148 * 1.965e9 * 32 / 1e12
+        achieved = triples / (k_ms * 1e-3) / 1e12
+        roofline = {"bound": "alu", "kernel": kernel_name, "achieved": achieved, "peak": peak,
+                    "unit": "T bit-tests/s", "frac": achieved / peak, "peak_source": "derived: POPC 16/clk/SM",
+                    "kernel_ms": k_ms, "traffic": read_traffic(kernel_name)}
+    roofline["hbm_gbs_algorithmic"] = (N * csg.csg_row_stride_words(N) * 8) / (k_ms * 1e-3) / 1e9
+
+    cpu_baseline = None
+    extra = {}
+    if world == 1 and not args.no_cpu_baseline:
+        tests, dt, rows, threads = oracle_sample(bits, N, min(kmax, 3) if eps == 1.0 else kmax, 12.0)
+        cpu_baseline = {"value": tests / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
+                        "sample": "Algorithm 5 restated (oracle/alg5_packed.c, OpenMP) on %d rows in 16 evenly spaced "
+                                  "row blocks of the same causal set, %.1f s; tests = sum over visited pairs of (j-i-1)"
+                                  % (rows, dt)}
+        ptests, pdt, pn = plain_oracle_sample(bits, N, kmax)
+        extra["cpu_baseline_plain"] = {"value": ptests / pdt, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                       "sample": "plain triple loop (oracle/csg_oracle.c) on the first %d elements "
+                                                 "of the same causal set, %.2f s" % (pn, pdt)}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u8 x u8 -> s32 (tcgen05 kind::i8)" if variant == csg.VARIANT_TENSOR else "u32 and/popc",
+        "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "N": N, "dim": dim, "eps": eps, "kmax": kmax, "seed": cfg["seed"],
+                   "variant": {1: "bitset", 2: "tensor"}[variant], "bitset_bytes": N * csg.csg_row_stride_words(N) * 8,
+                   "l2": "input (%.0f MiB) %s L2 (126 MB)" % (N * csg.csg_row_stride_words(N) * 8 / 2**20,
+                                                            "larger than" if N * csg.csg_row_stride_words(N) * 8 > 126e6
+                                                            else "fits in"),
+                   "parallelism": "1 causal set per GPU, no collectives", "host_generation_s": gen_s},
+        "action_time_s": ms_total / args.steps * 1e-3,
+        "kernel_ms_per_step": kernel_ms,
+        "result": {"counts_head": [int(x) for x in result_counts[:4]], "S": result_S},
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": N * csg.csg_row_stride_words(N) * 8,
+                "d2h_bytes_per_step": (kmax + 1) * 8 + 8, "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps},
+        "gpu_launches": launches,
+        "roofline": roofline,
+        "cpu_baseline": cpu_baseline,
+    }
+    line.update(extra)
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="index into BASELINE.json configs (default 3, the headline)")
+    ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 bitset, 2 tensor")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    import csg_inputs
+    cfg = dict(csg_inputs.CONFIGS[args.config])
+    cfg["index"] = args.config
+    if args.impl == "reference":
+        return run_reference(args, cfg, rank, world)
+    return run_ours(args, cfg, rank, local_rank, world)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -105,6 +105,9 @@ int csg_effective_variant(int64_t N);
  */
 int csg_set_kernel_timing(int enable);
 int csg_last_kernel_ms(float *ms);
+/* Same for the latest n timed calls (1 <= n <= 64), oldest first: ms HOST, n floats.  CSG_E_CUDA if fewer
+ * than n calls were timed since timing was enabled. */
+int csg_kernel_ms_history(float *ms, int n);
 int64_t csg_launch_count(void);
 
 /* Text for a code; for CSG_E_CUDA it includes the text of the last CUDA error the library saw. */

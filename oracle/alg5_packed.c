@@ -57,7 +57,7 @@ void csg_alg5_counts_rows(const uint64_t *bits, int64_t N, int64_t stride_words,
 #pragma omp parallel reduction(+ : tests)
     {
         int64_t *priv = (int64_t *)calloc((size_t)nb, sizeof(int64_t));
-#pragma omp for schedule(dynamic, 8)
+#pragma omp for schedule(dynamic, 1)
         for (int64_t i = row_begin; i < row_end; ++i) {
             const uint64_t *ri = bits + i * stride_words;
             for (int64_t j = i + 1; j < N; ++j) {

@@ -5,7 +5,8 @@ hand-written sm_100a kernels behind the C ABI.  PyTorch is used for device memor
 There is no CPU fallback: if libcsg.so is missing, importing the compute entry points fails loudly.
 
 Functions carry the C names: csg_action, csg_action_host, csg_interval_sizes, csg_row_stride_words,
-csg_set_variant, csg_effective_variant, csg_set_kernel_timing, csg_last_kernel_ms, csg_launch_count,
+csg_set_variant, csg_effective_variant, csg_set_kernel_timing, csg_last_kernel_ms, csg_kernel_ms_history,
+csg_launch_count,
 csg_strerror, csg_shutdown.
 """
 import ctypes
@@ -20,7 +21,8 @@ LIB_PATH = _build.LIB_PATH
 
 EXPORTS = [
     "csg_row_stride_words", "csg_action", "csg_action_host", "csg_interval_sizes", "csg_set_variant",
-    "csg_effective_variant", "csg_set_kernel_timing", "csg_last_kernel_ms", "csg_launch_count",
+    "csg_effective_variant", "csg_set_kernel_timing", "csg_last_kernel_ms", "csg_kernel_ms_history",
+    "csg_launch_count",
     "csg_strerror", "csg_shutdown",
 ]
 
@@ -64,6 +66,8 @@ def load():
     lib.csg_set_kernel_timing.restype = ci
     lib.csg_last_kernel_ms.argtypes = [ctypes.POINTER(ctypes.c_float)]
     lib.csg_last_kernel_ms.restype = ci
+    lib.csg_kernel_ms_history.argtypes = [ctypes.POINTER(ctypes.c_float), ci]
+    lib.csg_kernel_ms_history.restype = ci
     lib.csg_launch_count.argtypes = []
     lib.csg_launch_count.restype = i64
     lib.csg_strerror.argtypes = [ci]
@@ -166,6 +170,12 @@ def csg_last_kernel_ms():
     ms = ctypes.c_float(0.0)
     _check(load().csg_last_kernel_ms(ctypes.byref(ms)))
     return float(ms.value)
+
+
+def csg_kernel_ms_history(n):
+    buf = (ctypes.c_float * int(n))()
+    _check(load().csg_kernel_ms_history(buf, int(n)))
+    return [float(x) for x in buf]
 
 
 def csg_launch_count():

@@ -68,12 +68,15 @@ finish_action_kernel(const long long* __restrict__ counts, long long N, int dim,
 }
 
 // ---------------------------------------------------------------------------------------------- host state
+constexpr int TIMING_RING = 64;
+
 struct State {
     std::mutex mu;
     int variant = CSG_VARIANT_AUTO;
     bool timing = false;
-    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
-    bool ev_valid = false;
+    // ring of event pairs around the interval kernel of the latest TIMING_RING timed calls
+    cudaEvent_t ev0[TIMING_RING] = {}, ev1[TIMING_RING] = {};
+    long long timed_calls = 0;
     long long launches = 0;
     char cuda_msg[256] = "no CUDA error recorded";
     // cached tile schedule of the tensor variant
@@ -176,12 +179,13 @@ static int action_device(const uint64_t* rel_bits, long long N, int dim, double 
             g.attr_set = true;
         }
     }
+    const int slot = (int)(g.timed_calls % TIMING_RING);
     if (g.timing) {
-        if (!g.ev0) {
-            CSG_CUDA(cudaEventCreate(&g.ev0));
-            CSG_CUDA(cudaEventCreate(&g.ev1));
+        if (!g.ev0[slot]) {
+            CSG_CUDA(cudaEventCreate(&g.ev0[slot]));
+            CSG_CUDA(cudaEventCreate(&g.ev1[slot]));
         }
-        CSG_CUDA(cudaEventRecord(g.ev0, stream));
+        CSG_CUDA(cudaEventRecord(g.ev0[slot], stream));
     }
     if (variant == CSG_VARIANT_TENSOR) {
         const int grid = std::max(1, std::min(g.ntiles, g.sm_count));
@@ -199,8 +203,8 @@ static int action_device(const uint64_t* rel_bits, long long N, int dim, double 
     CSG_CUDA(cudaGetLastError());
     ++g.launches;
     if (g.timing) {
-        CSG_CUDA(cudaEventRecord(g.ev1, stream));
-        g.ev_valid = true;
+        CSG_CUDA(cudaEventRecord(g.ev1[slot], stream));
+        ++g.timed_calls;
     }
     finish_action_kernel<<<1, FIN_THREADS, 0, stream>>>(counts, N, dim, eps, kmax, S);
     CSG_CUDA(cudaGetLastError());
@@ -296,20 +300,34 @@ int csg_effective_variant(int64_t N) {
 int csg_set_kernel_timing(int enable) {
     std::lock_guard<std::mutex> lock(g.mu);
     g.timing = enable != 0;
-    if (!g.timing) g.ev_valid = false;
+    if (!g.timing) g.timed_calls = 0;
+    return CSG_OK;
+}
+
+static int kernel_ms_history(float* ms, int n) {
+    if (!ms) return CSG_E_NULL;
+    if (n < 1 || n > TIMING_RING) return CSG_E_SIZE;
+    if (g.timed_calls < n) {
+        snprintf(g.cuda_msg, sizeof(g.cuda_msg), "kernel timing: only %lld timed csg_action calls so far, %d asked",
+                 g.timed_calls, n);
+        return CSG_E_CUDA;
+    }
+    for (int k = 0; k < n; ++k) {
+        const int slot = (int)((g.timed_calls - n + k) % TIMING_RING);
+        CSG_CUDA(cudaEventSynchronize(g.ev1[slot]));
+        CSG_CUDA(cudaEventElapsedTime(&ms[k], g.ev0[slot], g.ev1[slot]));
+    }
     return CSG_OK;
 }
 
 int csg_last_kernel_ms(float* ms) {
     std::lock_guard<std::mutex> lock(g.mu);
-    if (!ms) return CSG_E_NULL;
-    if (!g.ev_valid) {
-        snprintf(g.cuda_msg, sizeof(g.cuda_msg), "csg_last_kernel_ms: no timed csg_action call yet");
-        return CSG_E_CUDA;
-    }
-    CSG_CUDA(cudaEventSynchronize(g.ev1));
-    CSG_CUDA(cudaEventElapsedTime(ms, g.ev0, g.ev1));
-    return CSG_OK;
+    return kernel_ms_history(ms, 1);
+}
+
+int csg_kernel_ms_history(float* ms, int n) {
+    std::lock_guard<std::mutex> lock(g.mu);
+    return kernel_ms_history(ms, n);
 }
 
 int64_t csg_launch_count(void) {
@@ -339,18 +357,20 @@ int csg_shutdown(void) {
     if (g.d_bits) cudaFree(g.d_bits);
     if (g.d_counts) cudaFree(g.d_counts);
     if (g.d_S) cudaFree(g.d_S);
-    if (g.ev0) cudaEventDestroy(g.ev0);
-    if (g.ev1) cudaEventDestroy(g.ev1);
+    for (int k = 0; k < TIMING_RING; ++k) {
+        if (g.ev0[k]) cudaEventDestroy(g.ev0[k]);
+        if (g.ev1[k]) cudaEventDestroy(g.ev1[k]);
+        g.ev0[k] = g.ev1[k] = nullptr;
+    }
     if (g.host_stream) cudaStreamDestroy(g.host_stream);
     g.d_tiles = nullptr;
     g.d_bits = nullptr;
     g.d_counts = nullptr;
     g.d_S = nullptr;
-    g.ev0 = g.ev1 = nullptr;
     g.host_stream = nullptr;
     g.tiles_N = -1;
     g.d_bits_bytes = g.d_counts_bytes = 0;
-    g.ev_valid = false;
+    g.timed_calls = 0;
     cudaGetLastError();
     return CSG_OK;
 }
