@@ -1,12 +1,14 @@
 // libcsg: C-ABI entry points (include/csg.h), argument validation, cached device workspace, tile
 // schedule, finishing kernel.  Every step of the hot path runs in the kernels of this directory; there is
 // no CPU fallback.
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <mutex>
 #include <vector>
 
@@ -86,6 +88,11 @@ struct State {
     std::vector<int2> h_tiles;
     int sm_count = 0;
     bool attr_set = false;
+    // TMA descriptor of the relation matrix seen as N rows of stride*8 bytes (cached per pointer and N)
+    void* encode_tiled = nullptr;
+    CUtensorMap bits_map;
+    const void* map_ptr = nullptr;
+    long long map_N = -1;
     // end-to-end (host buffer) path
     cudaStream_t host_stream = nullptr;
     uint64_t* d_bits = nullptr;
@@ -151,6 +158,42 @@ static int ensure_tiles(long long N, cudaStream_t stream) {
     return CSG_OK;
 }
 
+// 2D byte view of the packed relation matrix for the TMA warp of the tensor variant: dim0 = stride*8 bytes of a
+// row, dim1 = N rows; box = 32 bytes x 128 rows, 32-byte swizzle (conflict-free 16-byte reads by the producers);
+// rows >= N and bytes beyond the row are zero-filled by the hardware.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static int ensure_bits_map(const uint64_t* rel_bits, long long N, long long stride_words) {
+    if (g.map_ptr == rel_bits && g.map_N == N) return CSG_OK;
+    if (!g.encode_tiled) {
+        cudaDriverEntryPointQueryResult qres;
+        CSG_CUDA(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &g.encode_tiled, cudaEnableDefault, &qres));
+        if (qres != cudaDriverEntryPointSuccess || !g.encode_tiled) {
+            snprintf(g.cuda_msg, sizeof(g.cuda_msg), "cuTensorMapEncodeTiled not available from the driver");
+            g.encode_tiled = nullptr;
+            return CSG_E_CUDA;
+        }
+    }
+    const cuuint64_t dims[2] = {(cuuint64_t)stride_words * 8, (cuuint64_t)N};
+    const cuuint64_t strides[1] = {(cuuint64_t)stride_words * 8};
+    const cuuint32_t box[2] = {(cuuint32_t)TC_BITS_ROW_BYTES, (cuuint32_t)TC_BITS_BOX_ROWS};
+    const cuuint32_t estr[2] = {1, 1};
+    CUresult r = reinterpret_cast<EncodeTiledFn>(g.encode_tiled)(
+        &g.bits_map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<uint64_t*>(rel_bits), dims, strides, box, estr,
+        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        snprintf(g.cuda_msg, sizeof(g.cuda_msg), "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+        g.map_ptr = nullptr;
+        return CSG_E_CUDA;
+    }
+    g.map_ptr = rel_bits;
+    g.map_N = N;
+    return CSG_OK;
+}
+
 static int validate(const void* rel_bits, long long N, int dim, double eps, int kmax, const void* counts,
                     const void* S) {
     if (!rel_bits || !counts || !S) return CSG_E_NULL;
@@ -173,9 +216,13 @@ static int action_device(const uint64_t* rel_bits, long long N, int dim, double 
     if (variant == CSG_VARIANT_TENSOR) {
         rc = ensure_tiles(N, stream);
         if (rc) return rc;
+        rc = ensure_bits_map(rel_bits, N, stride);
+        if (rc) return rc;
         if (!g.attr_set) {
-            CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                          TC_SMEM_BYTES));
+            CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM_BYTES));
+            CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM_BYTES));
+            CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM_BYTES));
+            CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM_BYTES));
             g.attr_set = true;
         }
     }
@@ -189,8 +236,19 @@ static int action_device(const uint64_t* rel_bits, long long N, int dim, double 
     }
     if (variant == CSG_VARIANT_TENSOR) {
         const int grid = std::max(1, std::min(g.ntiles, g.sm_count));
-        tensor_action_kernel<<<grid, TC_THREADS, TC_SMEM_BYTES, stream>>>(
-            rel_bits, N, stride, kmax, reinterpret_cast<unsigned long long*>(counts), g.d_tiles, g.ntiles);
+        // operand bit TB: the accumulator holds n_ij << 2TB and n_ij <= N-2, so TB is the largest with
+        // (N-2) << 2TB < 2^31; TB = 7 turns every unpack shift into a left shift (FMA pipe).
+        unsigned long long* c64 = reinterpret_cast<unsigned long long*>(counts);
+        const char* dbg_env = getenv("CSG_DEBUG");
+        const int dbg = dbg_env ? atoi(dbg_env) : 0;
+        if (N - 2 < (1LL << 17))
+            tensor_action_kernel<7><<<grid, TC_THREADS, TC_SMEM_BYTES, stream>>>(g.bits_map, rel_bits, N, stride, kmax, c64, g.d_tiles, g.ntiles, dbg);
+        else if (N - 2 < (1LL << 19))
+            tensor_action_kernel<6><<<grid, TC_THREADS, TC_SMEM_BYTES, stream>>>(g.bits_map, rel_bits, N, stride, kmax, c64, g.d_tiles, g.ntiles, dbg);
+        else if (N - 2 < (1LL << 21))
+            tensor_action_kernel<5><<<grid, TC_THREADS, TC_SMEM_BYTES, stream>>>(g.bits_map, rel_bits, N, stride, kmax, c64, g.d_tiles, g.ntiles, dbg);
+        else
+            tensor_action_kernel<4><<<grid, TC_THREADS, TC_SMEM_BYTES, stream>>>(g.bits_map, rel_bits, N, stride, kmax, c64, g.d_tiles, g.ntiles, dbg);
     } else {
         const long long nb = (N + BS_T - 1) / BS_T;
         const long long ntiles = nb * (nb + 1) / 2;
@@ -369,6 +427,8 @@ int csg_shutdown(void) {
     g.d_S = nullptr;
     g.host_stream = nullptr;
     g.tiles_N = -1;
+    g.map_ptr = nullptr;
+    g.map_N = -1;
     g.d_bits_bytes = g.d_counts_bytes = 0;
     g.timed_calls = 0;
     cudaGetLastError();

@@ -7,11 +7,13 @@
 //
 //   * a CTA owns a 128 x 256 tile of pairs (rows i of block I, rows j of block J) and sweeps K from the
 //     first column of block I to the last column of block J in stages of 128 columns;
-//   * 12 producer warps read the packed bits of their row (16 bytes per row per stage, straight from
-//     global/L2 with a two-stage register prefetch), expand them to 0/1 unsigned bytes and store them into a
-//     4-stage ring of K-major, 128-byte-swizzled operand tiles in shared memory.  The order of the 32 k's
-//     inside a 32-bit word is permuted ((w >> q) & 0x01010101 puts bits q, q+8, q+16, q+24 into one 32-bit
-//     store); both operands use the same permutation and the MMA sums over k, so the result is unchanged;
+//   * one TMA warp streams the packed bits of the 384 rows (32 bytes = 2 stages per row per copy, a
+//     32-byte-swizzled 2D box per 128 rows) into a 4-deep shared-memory ring, so the global reads are whole
+//     sectors issued by one thread instead of 16-byte gathers by every thread;
+//   * 12 producer warps (one row per thread) read their row's 16 bytes per stage from that ring, expand the
+//     bits to bytes (0 or 1 << TB) and store them into a 3-stage ring of K-major, 128-byte-swizzled operand
+//     tiles.  The order of the 32 k's inside a 32-bit word is permuted (bits q, q+8, q+16, q+24 share one
+//     32-bit store); both operands use the same permutation and the MMA sums over k, so the result is unchanged;
 //   * one thread issues tcgen05.mma.cta_group::1.kind::i8 (M=128, N=256, K=32, u8 x u8 -> s32, exact) four
 //     times per stage, accumulating in 256 TMEM columns; tcgen05.commit hands the stage back to the producers;
 //   * the open range i<k<j costs nothing in the steady state: only the first stage of a tile (columns of
@@ -23,6 +25,8 @@
 // Tiles are handed out statically from a list sorted by K-depth, longest first, in boustrophedon order over
 // the persistent CTAs (one per SM), which balances the triangular workload without a global counter.
 #pragma once
+#include <cuda.h>
+
 #include <cstdint>
 
 namespace csg {
@@ -30,16 +34,29 @@ namespace csg {
 constexpr int TC_TM = 128;                 // rows i per tile (UMMA M)
 constexpr int TC_TN = 256;                 // rows j per tile (UMMA N)
 constexpr int TC_KS = 128;                 // k columns per stage = bytes per operand row in smem
-constexpr int TC_STAGES = 4;
+constexpr int TC_STAGES = 3;
 constexpr int TC_A_BYTES = TC_TM * TC_KS;  // 16 KiB
 constexpr int TC_B_BYTES = TC_TN * TC_KS;  // 32 KiB
 constexpr int TC_STAGE_BYTES = TC_A_BYTES + TC_B_BYTES;
+constexpr int TC_ROWS = TC_TM + TC_TN;     // packed-bit rows staged per group
+constexpr int TC_GROUP = 2;                // stages covered by one packed-bit copy
+constexpr int TC_BITS_ROW_BYTES = TC_GROUP * TC_KS / 8;   // 32
+constexpr int TC_BITS_BOX_ROWS = 128;
+constexpr int TC_BITS_BOX_BYTES = TC_BITS_BOX_ROWS * TC_BITS_ROW_BYTES;   // 4 KiB
+constexpr int TC_BITS_BUF_BYTES = TC_ROWS * TC_BITS_ROW_BYTES;            // 12 KiB
+constexpr int TC_BITS_BUFS = 4;
 constexpr int TC_PRODUCER_WARPS = 12;      // 4 for the A rows, 8 for the B rows
 constexpr int TC_PRODUCERS = TC_PRODUCER_WARPS * 32;
-constexpr int TC_THREADS = TC_PRODUCERS + 32;  // + the MMA warp
-constexpr int TC_HIST = 4096;              // privatised low bins per CTA
+constexpr int TC_MMA_WARP = TC_PRODUCER_WARPS;
+constexpr int TC_TMA_WARP = TC_PRODUCER_WARPS + 1;
+constexpr int TC_THREADS = TC_PRODUCERS + 64;  // + the MMA warp + the TMA warp
+constexpr int TC_HIST = 2048;              // privatised low bins per CTA
 constexpr int TC_TMEM_COLS = 256;
-constexpr int TC_SMEM_BYTES = TC_STAGES * TC_STAGE_BYTES + TC_HIST * 4 + 256 + 1024;  // + barriers + align
+constexpr int TC_OFF_BITS = TC_STAGES * TC_STAGE_BYTES;
+constexpr int TC_OFF_HIST = TC_OFF_BITS + TC_BITS_BUFS * TC_BITS_BUF_BYTES;
+constexpr int TC_OFF_BARS = TC_OFF_HIST + TC_HIST * 4;
+constexpr int TC_NUM_BARS = 2 * TC_STAGES + 2 + 2 * TC_BITS_BUFS;
+constexpr int TC_SMEM_BYTES = TC_OFF_BARS + 8 * TC_NUM_BARS + 16 + 1024;  // + TMEM slot + alignment slack
 
 // ---------------------------------------------------------------------------------------------- PTX helpers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
@@ -60,8 +77,53 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
         "bra WAIT_%=;\n\t"
         "DONE_%=:\n\t}" ::"r"(bar), "r"(parity) : "memory");
 }
+// One non-blocking probe of the barrier phase; lets the caller overlap the probe latency with other work.
+__device__ __forceinline__ bool mbar_try(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+// 2D tiled TMA load global -> shared; completes bytes on `bar`.  c0 = byte column, c1 = row.
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+        ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar) : "memory");
+}
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr)
+                 : "memory");
+    return v;
+}
+// Elected arrive that also names two registers of the warp-wide loads it must not overtake.
+__device__ __forceinline__ void mbar_arrive_after(uint32_t bar, uint32_t dep0, uint32_t dep1) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar), "r"(dep0), "r"(dep1) : "memory");
+}
+__device__ __forceinline__ void sts128(uint32_t addr, const uint4& v) {
+    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w)
+                 : "memory");
+}
 __device__ __forceinline__ void fence_proxy_async_smem() {
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+// Same fence, placed AFTER the computation of the 32 registers it names: the fake register dependency stops the
+// compiler from sinking the unpack arithmetic below the fence, so the fence finds the previous stage's stores
+// already drained.
+__device__ __forceinline__ void fence_proxy_async_smem_after(uint4 (&o)[8]) {
+    asm volatile("fence.proxy.async.shared::cta;"
+                 : "+r"(o[0].x), "+r"(o[0].y), "+r"(o[0].z), "+r"(o[0].w), "+r"(o[1].x), "+r"(o[1].y), "+r"(o[1].z),
+                   "+r"(o[1].w), "+r"(o[2].x), "+r"(o[2].y), "+r"(o[2].z), "+r"(o[2].w), "+r"(o[3].x), "+r"(o[3].y),
+                   "+r"(o[3].z), "+r"(o[3].w), "+r"(o[4].x), "+r"(o[4].y), "+r"(o[4].z), "+r"(o[4].w), "+r"(o[5].x),
+                   "+r"(o[5].y), "+r"(o[5].z), "+r"(o[5].w), "+r"(o[6].x), "+r"(o[6].y), "+r"(o[6].z), "+r"(o[6].w),
+                   "+r"(o[7].x), "+r"(o[7].y), "+r"(o[7].z), "+r"(o[7].w)
+                 :
+                 : "memory");
 }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
@@ -105,26 +167,21 @@ __device__ __forceinline__ uint64_t make_kmajor_sw128_desc(uint32_t smem_addr) {
 // Instruction descriptor, kind::i8: D = s32, A = B = u8, both K-major, N = 256, M = 128.
 constexpr uint32_t TC_IDESC = (2u << 4) | ((TC_TN >> 3) << 17) | ((TC_TM >> 4) << 24);
 
-// One row's 128 k-bits (4 words) -> 128 bytes in the swizzled operand row.
-__device__ __forceinline__ void unpack_row_to_smem(uint8_t* tile, int r, const uint4& w) {
-    uint8_t* row = tile + (r >> 3) * 1024 + (r & 7) * 128;
-    const int sw = r & 7;
-    const uint32_t ws[4] = {w.x, w.y, w.z, w.w};
-#pragma unroll
-    for (int m = 0; m < 4; ++m) {
-        const uint32_t x = ws[m];
-        uint4 lo, hi;
-        lo.x = x & 0x01010101u;
-        lo.y = (x >> 1) & 0x01010101u;
-        lo.z = (x >> 2) & 0x01010101u;
-        lo.w = (x >> 3) & 0x01010101u;
-        hi.x = (x >> 4) & 0x01010101u;
-        hi.y = (x >> 5) & 0x01010101u;
-        hi.z = (x >> 6) & 0x01010101u;
-        hi.w = (x >> 7) & 0x01010101u;
-        *reinterpret_cast<uint4*>(row + (((2 * m) ^ sw) << 4)) = lo;
-        *reinterpret_cast<uint4*>(row + (((2 * m + 1) ^ sw) << 4)) = hi;
-    }
+// One 32-bit word of a row (32 k's) -> 32 operand bytes (two 16-byte chunks), each byte 0 or 1 << TB.
+// Class q of the word = bits q, q+8, q+16, q+24; they go to bit TB of the four bytes of one 32-bit lane, so one
+// shift and one AND expand four k's.  Left shifts (q < TB) may be issued as IMAD.SHL on the FMA pipe, which
+// unloads the ALU pipe that carries the ANDs: TB = 7 needs no right shift at all.
+template <int TB>
+__device__ __forceinline__ uint32_t unpack_class(uint32_t x, int q) {
+    constexpr uint32_t M = 0x01010101u << TB;
+    return (q < TB ? (x << (TB - q)) : (x >> (q - TB))) & M;
+}
+template <int TB>
+__device__ __forceinline__ void unpack_word(uint32_t x, uint4& lo, uint4& hi) {
+    lo.x = unpack_class<TB>(x, 0); lo.y = unpack_class<TB>(x, 1);
+    lo.z = unpack_class<TB>(x, 2); lo.w = unpack_class<TB>(x, 3);
+    hi.x = unpack_class<TB>(x, 4); hi.y = unpack_class<TB>(x, 5);
+    hi.z = unpack_class<TB>(x, 6); hi.w = unpack_class<TB>(x, 7);
 }
 
 // keep local bit positions p (0..127) with p > r   (operand U in the stage that holds row i's own column)
@@ -138,34 +195,41 @@ __device__ __forceinline__ uint32_t keep_lt(int lim, int m) {
     return s <= 0 ? 0u : (s >= 32 ? 0xFFFFFFFFu : ((1u << s) - 1u));
 }
 
-// tile list entry: I (128-row block) in the low 16 bits... kept as int2 {I, J} for clarity.
+// TB = bit of the operand byte that carries the relation bit: operands are 0 or 2^TB, every product is 4^TB, and
+// the accumulator holds n_ij << 2TB.  The host picks the largest TB with (N-2) << 2TB < 2^31 (exact in s32).
+template <int TB>
 __global__ void __launch_bounds__(TC_THREADS, 1)
-tensor_action_kernel(const uint64_t* __restrict__ rel, long long N, long long stride_words, int kmax,
-                     unsigned long long* __restrict__ counts, const int2* __restrict__ tiles, int ntiles) {
+tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_t* __restrict__ rel, long long N,
+                     long long stride_words, int kmax, unsigned long long* __restrict__ counts,
+                     const int2* __restrict__ tiles, int ntiles, int dbg) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    uint8_t* stage_base = smem;
-    unsigned int* hist = reinterpret_cast<unsigned int*>(smem + TC_STAGES * TC_STAGE_BYTES);
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + TC_STAGES * TC_STAGE_BYTES + TC_HIST * 4);
-    // bars[0..3] full, bars[4..7] empty, bars[8] tmem_full, bars[9] tmem_empty, then the TMEM base address
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 10);
+    unsigned int* hist = reinterpret_cast<unsigned int*>(smem + TC_OFF_HIST);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + TC_OFF_BARS);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + TC_NUM_BARS);
 
     const int tid = threadIdx.x;
     const int warp = tid >> 5, lane = tid & 31;
-    const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + TC_STAGES);
-    const uint32_t tmem_full = smem_u32(bars + 2 * TC_STAGES), tmem_empty = smem_u32(bars + 2 * TC_STAGES + 1);
+    const uint32_t smem0 = smem_u32(smem);
+    const uint32_t full0 = smem_u32(bars), empty0 = full0 + 8 * TC_STAGES;
+    const uint32_t tmem_full = empty0 + 8 * TC_STAGES, tmem_empty = tmem_full + 8;
+    const uint32_t bits_full0 = tmem_empty + 8, bits_empty0 = bits_full0 + 8 * TC_BITS_BUFS;
 
     for (int b = tid; b < TC_HIST; b += TC_THREADS) hist[b] = 0u;
     if (tid == 0) {
         for (int s = 0; s < TC_STAGES; ++s) {
-            mbar_init(full0 + 8 * s, TC_PRODUCERS);
-            mbar_init(empty0 + 8 * s, 1);
+            mbar_init(full0 + 8 * s, TC_PRODUCER_WARPS);   // one elected arrive per producer warp
+            mbar_init(empty0 + 8 * s, 1);                  // tcgen05.commit
         }
         mbar_init(tmem_full, 1);
         mbar_init(tmem_empty, TC_PRODUCERS);
+        for (int b = 0; b < TC_BITS_BUFS; ++b) {
+            mbar_init(bits_full0 + 8 * b, 1);              // expect_tx arrive of the TMA thread
+            mbar_init(bits_empty0 + 8 * b, TC_PRODUCER_WARPS);
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (warp == TC_PRODUCER_WARPS) {
+    if (warp == TC_MMA_WARP) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)),
                      "n"(TC_TMEM_COLS) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
@@ -185,8 +249,15 @@ tensor_action_kernel(const uint64_t* __restrict__ rel, long long N, long long st
         const int q4 = warp & 3;                      // TMEM lane quarter this warp may read
         const int cgrp = warp >> 2;                   // which third of the 8 column chunks it drains
         const int c_begin = cgrp * 3, c_end = cgrp == 2 ? 8 : c_begin + 3;
-        uint32_t stage = 0, sphase = 0;               // ring position / parity
+        uint32_t stage = 0, sphase = 0;               // operand ring position / parity
+        uint32_t bb = 0, bphase = 0;                  // packed-bit ring position / parity
         uint32_t tphase = 0;                          // parity of tmem_full
+        int pending = -1;                             // ring stage written but not yet published
+        const uint32_t row_smem = smem0 + (isA ? 0 : TC_A_BYTES) + (r >> 3) * 1024 + (r & 7) * 128;
+        const int sw = r & 7;
+        // this thread's row in a packed-bit buffer: 32 bytes per row, 16-byte halves swapped on odd groups of 4 rows
+        const uint32_t bits_row = smem0 + TC_OFF_BITS + tid * TC_BITS_ROW_BYTES;
+        const uint32_t bits_sw = ((tid >> 2) & 1) << 4;
 
         for (int rd = 0; rd < rounds; ++rd) {
             const int t = rd * G + ((rd & 1) ? (G - 1 - cta) : cta);
@@ -195,32 +266,61 @@ tensor_action_kernel(const uint64_t* __restrict__ rel, long long N, long long st
             const int I = tile.x, J = tile.y;
             const long long i0 = (long long)I * TC_TM, j0 = (long long)J * TC_TN;
             const int kb_begin = I, kb_end = 2 * J + 2;   // stages of 128 columns, [begin, end)
-            const long long row = isA ? i0 + r : j0 + r;
-            const bool row_ok = row < N;
-            const uint4* src = reinterpret_cast<const uint4*>(rel + (row_ok ? row : 0) * stride_words);
-            const uint4 zero = make_uint4(0, 0, 0, 0);
 
-            uint4 w0 = row_ok ? __ldg(src + kb_begin) : zero;
-            uint4 w1 = (row_ok && kb_begin + 1 < kb_end) ? __ldg(src + kb_begin + 1) : zero;
-            for (int kb = kb_begin; kb < kb_end; ++kb) {
-                uint4 w2 = (row_ok && kb + 2 < kb_end) ? __ldg(src + kb + 2) : zero;
-                uint4 w = w0;
-                if (isA) {
-                    if (kb == I) {
-                        w.x &= keep_gt(r, 0); w.y &= keep_gt(r, 1); w.z &= keep_gt(r, 2); w.w &= keep_gt(r, 3);
+            // Software pipeline: the fence + arrive that publishes stage s is issued after the ALU work of stage
+            // s+1 (its stores have drained by then); the empty-slot barrier is probed before that ALU work.
+            for (int kb0 = kb_begin; kb0 < kb_end; kb0 += TC_GROUP) {
+                mbar_wait(bits_full0 + 8 * bb, bphase);
+                uint4 cur[TC_GROUP];
+#pragma unroll
+                for (int u = 0; u < TC_GROUP; ++u)
+                    cur[u] = lds128(bits_row + bb * TC_BITS_BUF_BYTES + ((u << 4) ^ bits_sw));
+                __syncwarp();
+                if (lane == 0) mbar_arrive_after(bits_empty0 + 8 * bb, cur[0].x, cur[TC_GROUP - 1].x);
+                if (++bb == TC_BITS_BUFS) { bb = 0; bphase ^= 1; }
+#pragma unroll
+                for (int u = 0; u < TC_GROUP; ++u) {
+                    const int kb = kb0 + u;
+                    if (kb < kb_end) {
+                        uint4 w = cur[u];
+                        if (isA) {
+                            if (kb == I) {
+                                w.x &= keep_gt(r, 0); w.y &= keep_gt(r, 1); w.z &= keep_gt(r, 2); w.w &= keep_gt(r, 3);
+                            }
+                        } else if (kb >= 2 * J) {
+                            const int lim = r - 128 * (kb - 2 * J);
+                            w.x &= keep_lt(lim, 0); w.y &= keep_lt(lim, 1); w.z &= keep_lt(lim, 2); w.w &= keep_lt(lim, 3);
+                        }
+                        const bool slot_free = mbar_try(empty0 + 8 * stage, sphase ^ 1);
+                        uint4 o[8];
+                        if (dbg & 1) {
+#pragma unroll
+                            for (int c = 0; c < 8; ++c) o[c] = w;
+                        } else {
+                            unpack_word<TB>(w.x, o[0], o[1]);
+                            unpack_word<TB>(w.y, o[2], o[3]);
+                            unpack_word<TB>(w.z, o[4], o[5]);
+                            unpack_word<TB>(w.w, o[6], o[7]);
+                        }
+                        if (pending >= 0) {                   // publish the previous stage
+                            fence_proxy_async_smem_after(o);
+                            __syncwarp();
+                            if (lane == 0) mbar_arrive(full0 + 8 * pending);
+                        }
+                        if (!slot_free) mbar_wait(empty0 + 8 * stage, sphase ^ 1);
+                        const uint32_t rowp = row_smem + stage * TC_STAGE_BYTES;
+#pragma unroll
+                        for (int c = 0; c < 8; ++c)
+                            if (!(dbg & 4) || c == 0) sts128(rowp + ((c ^ sw) << 4), o[c]);
+                        pending = (int)stage;
+                        if (++stage == TC_STAGES) { stage = 0; sphase ^= 1; }
                     }
-                } else if (kb >= 2 * J) {
-                    const int lim = r - 128 * (kb - 2 * J);
-                    w.x &= keep_lt(lim, 0); w.y &= keep_lt(lim, 1); w.z &= keep_lt(lim, 2); w.w &= keep_lt(lim, 3);
                 }
-                mbar_wait(empty0 + 8 * stage, sphase ^ 1);
-                uint8_t* tile_smem = stage_base + stage * TC_STAGE_BYTES + (isA ? 0 : TC_A_BYTES);
-                unpack_row_to_smem(tile_smem, r, w);
-                fence_proxy_async_smem();
-                mbar_arrive(full0 + 8 * stage);
-                if (++stage == TC_STAGES) { stage = 0; sphase ^= 1; }
-                w0 = w1; w1 = w2;
             }
+            fence_proxy_async_smem();                          // publish the last stage of the tile
+            __syncwarp();
+            if (lane == 0) mbar_arrive(full0 + 8 * pending);
+            pending = -1;
 
             // ---- epilogue: TMEM -> registers -> mask by R[i][j], i<j -> histogram
             mbar_wait(tmem_full, tphase);
@@ -238,7 +338,7 @@ tensor_action_kernel(const uint64_t* __restrict__ rel, long long N, long long st
                 else if (jc <= i) relw &= 0xFFFFFFFFu << (int)(i - jc + 1);
 #pragma unroll
                 for (int x = 0; x < 32; ++x) {
-                    const int n = (int)v[x];
+                    const int n = (int)(v[x] >> (2 * TB));
                     if (((relw >> x) & 1u) && n <= kmax) {
                         if (n < TC_HIST) atomicAdd(&hist[n], 1u);
                         else atomicAdd(&counts[n], 1ULL);
@@ -248,7 +348,7 @@ tensor_action_kernel(const uint64_t* __restrict__ rel, long long N, long long st
             tc_fence_before();
             mbar_arrive(tmem_empty);
         }
-    } else {
+    } else if (warp == TC_MMA_WARP) {
         // ================================================================== MMA issuer (one warp, lane 0 issues)
         uint32_t stage = 0, sphase = 0, ephase = 0;
         int done_tiles = 0;
@@ -265,8 +365,11 @@ tensor_action_kernel(const uint64_t* __restrict__ rel, long long N, long long st
             for (int kb = kb_begin; kb < kb_end; ++kb) {
                 mbar_wait(full0 + 8 * stage, sphase);
                 tc_fence_after();
-                if (lane == 0) {
-                    const uint32_t a_addr = smem_u32(stage_base + stage * TC_STAGE_BYTES);
+                if (lane == 0 && (dbg & 2)) {
+                    umma_commit(empty0 + 8 * stage);
+                    if (kb == kb_end - 1) umma_commit(tmem_full);
+                } else if (lane == 0) {
+                    const uint32_t a_addr = smem0 + stage * TC_STAGE_BYTES;
                     const uint64_t adesc = make_kmajor_sw128_desc(a_addr);
                     const uint64_t bdesc = make_kmajor_sw128_desc(a_addr + TC_A_BYTES);
 #pragma unroll
@@ -280,6 +383,28 @@ tensor_action_kernel(const uint64_t* __restrict__ rel, long long N, long long st
             }
             ++done_tiles;
         }
+    } else {
+        // ================================================================== TMA warp: packed bits -> shared ring
+        if (lane == 0) {
+            uint32_t bb = 0, bphase = 0;
+            for (int rd = 0; rd < rounds; ++rd) {
+                const int t = rd * G + ((rd & 1) ? (G - 1 - cta) : cta);
+                if (t >= ntiles) continue;
+                const int2 tile = tiles[t];
+                const int i0 = tile.x * TC_TM, j0 = tile.y * TC_TN;
+                const int kb_begin = tile.x, kb_end = 2 * tile.y + 2;
+                for (int kb0 = kb_begin; kb0 < kb_end; kb0 += TC_GROUP) {
+                    mbar_wait(bits_empty0 + 8 * bb, bphase ^ 1);
+                    const uint32_t bar = bits_full0 + 8 * bb;
+                    const uint32_t dst = smem0 + TC_OFF_BITS + bb * TC_BITS_BUF_BYTES;
+                    mbar_expect_tx(bar, TC_BITS_BUF_BYTES);
+                    tma_load_2d(dst, &bits_map, kb0 * 16, i0, bar);
+                    tma_load_2d(dst + TC_BITS_BOX_BYTES, &bits_map, kb0 * 16, j0, bar);
+                    tma_load_2d(dst + 2 * TC_BITS_BOX_BYTES, &bits_map, kb0 * 16, j0 + TC_BITS_BOX_ROWS, bar);
+                    if (++bb == TC_BITS_BUFS) { bb = 0; bphase ^= 1; }
+                }
+            }
+        }
     }
 
     // ---- teardown: flush the privatised histogram, release TMEM
@@ -288,7 +413,7 @@ tensor_action_kernel(const uint64_t* __restrict__ rel, long long N, long long st
     tc_fence_after();
     for (int b = tid; b < TC_HIST && b <= kmax; b += TC_THREADS)
         if (hist[b]) atomicAdd(&counts[b], (unsigned long long)hist[b]);
-    if (warp == TC_PRODUCER_WARPS) {
+    if (warp == TC_MMA_WARP) {
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(TC_TMEM_COLS)
                      : "memory");
     }
