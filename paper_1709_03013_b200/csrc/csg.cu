@@ -134,17 +134,14 @@ static int effective_variant(long long N) {
     return N >= 2048 ? CSG_VARIANT_TENSOR : CSG_VARIANT_BITSET;
 }
 
-// Tiles (I, J) of the tensor variant: I = block of 128 rows i, J = block of 256 rows j; a tile is needed
-// iff it holds some pair i<j.  K-depth in 128-column stages = 2J+2-I.  Sorted longest first.
+// Tiles (I, J) of the tensor variant in 256-row blocks, I <= J; K-depth in 128-column stages = 2(J-I)+2.
+// Sorted longest first.
 static int ensure_tiles(long long N, cudaStream_t stream) {
     if (g.tiles_N == N && g.d_tiles) return CSG_OK;
-    const int nI = (int)((N + TC_TM - 1) / TC_TM), nJ = (int)((N + TC_TN - 1) / TC_TN);
+    const int nB = (int)((N + TC_T - 1) / TC_T);
     g.h_tiles.clear();
-    for (int J = 0; J < nJ; ++J)
-        for (int I = 0; I < nI && I <= 2 * J + 1; ++I) g.h_tiles.push_back(make_int2(I, J));
-    std::stable_sort(g.h_tiles.begin(), g.h_tiles.end(), [](const int2& a, const int2& b) {
-        return (2 * a.y + 2 - a.x) > (2 * b.y + 2 - b.x);
-    });
+    for (int d = nB - 1; d >= 0; --d)
+        for (int I = 0; I + d < nB; ++I) g.h_tiles.push_back(make_int2(I, I + d));
     if (g.d_tiles) {
         CSG_CUDA(cudaStreamSynchronize(stream));
         CSG_CUDA(cudaFree(g.d_tiles));
@@ -235,7 +232,7 @@ static int action_device(const uint64_t* rel_bits, long long N, int dim, double 
         CSG_CUDA(cudaEventRecord(g.ev0[slot], stream));
     }
     if (variant == CSG_VARIANT_TENSOR) {
-        const int grid = std::max(1, std::min(g.ntiles, g.sm_count));
+        const int grid = 2 * std::max(1, std::min(g.ntiles, g.sm_count / 2));   // one CTA pair per SM pair
         // operand bit TB: the accumulator holds n_ij << 2TB and n_ij <= N-2, so TB is the largest with
         // (N-2) << 2TB < 2^31; TB = 7 turns every unpack shift into a left shift (FMA pipe).
         unsigned long long* c64 = reinterpret_cast<unsigned long long*>(counts);

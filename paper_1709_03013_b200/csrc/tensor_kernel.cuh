@@ -1,29 +1,32 @@
-// Tensor-core variant of the interval kernel: a tiled binary "GEMM" on tcgen05 (sm_100a).
+// Tensor-core variant of the interval kernel: a tiled binary "GEMM" on tcgen05 (sm_100a), CTA pairs.
 //
 // What it computes (Sec. 4.1, Fig. 2, Alg. 5 l.7): for every related
 // pair i<j, n_ij = sum_{i<k<j} R[i][k] * R[j][k], bucketed into counts[n_ij].  With U[i][k] = R[i][k]*[k>i]
 // and L[j][k] = R[j][k]*[k<j] this is the matrix product C = U * L^T restricted to the upper triangle and
 // masked by R[i][j] -- a dense contraction over k, so it runs on the 5th-generation tensor cores:
 //
-//   * a CTA owns a 128 x 256 tile of pairs (rows i of block I, rows j of block J) and sweeps K from the
-//     first column of block I to the last column of block J in stages of 128 columns;
-//   * one TMA warp streams the packed bits of the 384 rows (32 bytes = 2 stages per row per copy, a
-//     32-byte-swizzled 2D box per 128 rows) into a 4-deep shared-memory ring, so the global reads are whole
-//     sectors issued by one thread instead of 16-byte gathers by every thread;
-//   * 12 producer warps (one row per thread) read their row's 16 bytes per stage from that ring, expand the
-//     bits to bytes (0 or 1 << TB) and store them into a 3-stage ring of K-major, 128-byte-swizzled operand
-//     tiles.  The order of the 32 k's inside a 32-bit word is permuted (bits q, q+8, q+16, q+24 share one
-//     32-bit store); both operands use the same permutation and the MMA sums over k, so the result is unchanged;
-//   * one thread issues tcgen05.mma.cta_group::1.kind::i8 (M=128, N=256, K=32, u8 x u8 -> s32, exact) four
-//     times per stage, accumulating in 256 TMEM columns; tcgen05.commit hands the stage back to the producers;
-//   * the open range i<k<j costs nothing in the steady state: only the first stage of a tile (columns of
-//     block I) needs the k>i mask and only the last two stages (columns of block J) need the k<j mask;
-//   * fused epilogue: the same 12 warps read the accumulators back with tcgen05.ld, test bit R[i][j] (and
-//     i<j), and bucket n_ij into a privatised shared-memory histogram (low bins) or straight into the global
-//     counts (high bins, smeared action only).  No N x N count matrix ever reaches HBM.
+//   * a cluster of two CTAs (one SM pair) owns a 256 x 256 tile of pairs (rows i of block I, rows j of block J)
+//     and sweeps K from the first column of block I to the last column of block J in stages of 128 columns.
+//     CTA rank p holds rows i0+128p.. of the A operand and rows j0+128p.. of the B operand, so each SM expands
+//     256 rows per stage for a 256 x 256 x 128 product (the single-CTA form needed 384 rows per 128 x 256 x 128),
+//     and each tensor core reads half of B from its own shared memory and half from its peer's;
+//   * per CTA one TMA thread streams the packed bits of its 256 rows (32 bytes = 2 stages per row per copy,
+//     32-byte-swizzled 2D boxes of 128 rows) into a 4-deep shared-memory ring: whole sectors, one issuing thread;
+//   * 16 producer warps (two threads per row) read 8 bytes per stage from that ring, expand the bits to
+//     bytes (0 or 1 << TB) and store them into a ring of K-major, 128-byte-swizzled operand tiles.  The order
+//     of the 32 k's inside a 32-bit word is permuted (bits q, q+8, q+16, q+24 share one 32-bit store); both
+//     operands use the same permutation and the MMA sums over k, so the result is unchanged;
+//   * one thread of the leader CTA issues tcgen05.mma.cta_group::2.kind::i8 (M=256, N=256, K=32, u8 x u8 -> s32,
+//     exact) four times per stage; each CTA's 128 accumulator rows live in 256 columns of its own TMEM;
+//     tcgen05.commit (multicast) hands the stage back to the producers of both CTAs;
+//   * the open range i<k<j costs nothing in the steady state: only the first two stages of a tile (columns of
+//     block I) need the k>i mask and only the last two (columns of block J) need the k<j mask;
+//   * fused epilogue: the producer warps read their CTA's accumulators back with tcgen05.ld, test bit R[i][j]
+//     (and i<j), and bucket n_ij into a privatised shared-memory histogram (low bins) or straight into the
+//     global counts (high bins, smeared action only).  No N x N count matrix ever reaches HBM.
 //
 // Tiles are handed out statically from a list sorted by K-depth, longest first, in boustrophedon order over
-// the persistent CTAs (one per SM), which balances the triangular workload without a global counter.
+// the persistent clusters (one per SM pair), which balances the triangular workload without a global counter.
 #pragma once
 #include <cuda.h>
 
@@ -31,21 +34,22 @@
 
 namespace csg {
 
-constexpr int TC_TM = 128;                 // rows i per tile (UMMA M)
-constexpr int TC_TN = 256;                 // rows j per tile (UMMA N)
+constexpr int TC_T = 256;                  // tile edge in pairs (UMMA M = N = 256 over the CTA pair)
+constexpr int TC_ROWS_A = 128;             // A rows per CTA
+constexpr int TC_ROWS_B = 128;             // B rows per CTA
+constexpr int TC_ROWS = TC_ROWS_A + TC_ROWS_B;
 constexpr int TC_KS = 128;                 // k columns per stage = bytes per operand row in smem
-constexpr int TC_STAGES = 3;
-constexpr int TC_A_BYTES = TC_TM * TC_KS;  // 16 KiB
-constexpr int TC_B_BYTES = TC_TN * TC_KS;  // 32 KiB
+constexpr int TC_STAGES = 4;
+constexpr int TC_A_BYTES = TC_ROWS_A * TC_KS;  // 16 KiB
+constexpr int TC_B_BYTES = TC_ROWS_B * TC_KS;  // 16 KiB
 constexpr int TC_STAGE_BYTES = TC_A_BYTES + TC_B_BYTES;
-constexpr int TC_ROWS = TC_TM + TC_TN;     // packed-bit rows staged per group
 constexpr int TC_GROUP = 2;                // stages covered by one packed-bit copy
 constexpr int TC_BITS_ROW_BYTES = TC_GROUP * TC_KS / 8;   // 32
 constexpr int TC_BITS_BOX_ROWS = 128;
 constexpr int TC_BITS_BOX_BYTES = TC_BITS_BOX_ROWS * TC_BITS_ROW_BYTES;   // 4 KiB
-constexpr int TC_BITS_BUF_BYTES = TC_ROWS * TC_BITS_ROW_BYTES;            // 12 KiB
+constexpr int TC_BITS_BUF_BYTES = TC_ROWS * TC_BITS_ROW_BYTES;            // 8 KiB
 constexpr int TC_BITS_BUFS = 4;
-constexpr int TC_PRODUCER_WARPS = 12;      // 4 for the A rows, 8 for the B rows
+constexpr int TC_PRODUCER_WARPS = 16;      // two threads per row: 8 warps for the A rows, 8 for the B rows
 constexpr int TC_PRODUCERS = TC_PRODUCER_WARPS * 32;
 constexpr int TC_MMA_WARP = TC_PRODUCER_WARPS;
 constexpr int TC_TMA_WARP = TC_PRODUCER_WARPS + 1;
@@ -62,11 +66,31 @@ constexpr int TC_SMEM_BYTES = TC_OFF_BARS + 8 * TC_NUM_BARS + 16 + 1024;  // + T
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
     return static_cast<uint32_t>(__cvta_generic_to_shared(p));
 }
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// shared::cluster address of the same shared-memory offset in CTA `rank` of the cluster
+__device__ __forceinline__ uint32_t map_to_cta(uint32_t addr, uint32_t rank) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+    return r;
+}
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
 }
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+// Arrive on a barrier of any CTA of the cluster (address from map_to_cta).  Default semantics on purpose: the
+// operand bytes reach the tensor cores through the async proxy, ordered by fence.proxy.async before this arrive;
+// a .release.cluster here compiles to MEMBAR.ALL.GPU + an L1 invalidate per stage and tripled the stage time.
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_bar) {
+    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     asm volatile(
@@ -95,10 +119,9 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map
         "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
         ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar) : "memory");
 }
-__device__ __forceinline__ uint4 lds128(uint32_t addr) {
-    uint4 v;
-    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr)
-                 : "memory");
+__device__ __forceinline__ uint2 lds64(uint32_t addr) {
+    uint2 v;
+    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr) : "memory");
     return v;
 }
 // Elected arrive that also names two registers of the warp-wide loads it must not overtake.
@@ -112,35 +135,34 @@ __device__ __forceinline__ void sts128(uint32_t addr, const uint4& v) {
 __device__ __forceinline__ void fence_proxy_async_smem() {
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
-// Same fence, placed AFTER the computation of the 32 registers it names: the fake register dependency stops the
+// Same fence, placed AFTER the computation of the 16 registers it names: the fake register dependency stops the
 // compiler from sinking the unpack arithmetic below the fence, so the fence finds the previous stage's stores
 // already drained.
-__device__ __forceinline__ void fence_proxy_async_smem_after(uint4 (&o)[8]) {
+__device__ __forceinline__ void fence_proxy_async_smem_after(uint4 (&o)[4]) {
     asm volatile("fence.proxy.async.shared::cta;"
                  : "+r"(o[0].x), "+r"(o[0].y), "+r"(o[0].z), "+r"(o[0].w), "+r"(o[1].x), "+r"(o[1].y), "+r"(o[1].z),
                    "+r"(o[1].w), "+r"(o[2].x), "+r"(o[2].y), "+r"(o[2].z), "+r"(o[2].w), "+r"(o[3].x), "+r"(o[3].y),
-                   "+r"(o[3].z), "+r"(o[3].w), "+r"(o[4].x), "+r"(o[4].y), "+r"(o[4].z), "+r"(o[4].w), "+r"(o[5].x),
-                   "+r"(o[5].y), "+r"(o[5].z), "+r"(o[5].w), "+r"(o[6].x), "+r"(o[6].y), "+r"(o[6].z), "+r"(o[6].w),
-                   "+r"(o[7].x), "+r"(o[7].y), "+r"(o[7].z), "+r"(o[7].w)
+                   "+r"(o[3].z), "+r"(o[3].w)
                  :
                  : "memory");
 }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 
-// D[tmem] (+)= A[smem] * B[smem]^T, u8 x u8 -> s32, one CTA.
-__device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
-                                        uint32_t accumulate) {
+// D[tmem] (+)= A[smem] * B[smem]^T, u8 x u8 -> s32, over the CTA pair (issued by the leader CTA only).
+__device__ __forceinline__ void umma_i8_2cta(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                             uint32_t accumulate) {
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
         "setp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d), "l"(adesc), "l"(bdesc),
+        "tcgen05.mma.cta_group::2.kind::i8 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d), "l"(adesc), "l"(bdesc),
         "r"(idesc), "r"(accumulate) : "memory");
 }
-// Arrive on an mbarrier once all tcgen05 ops issued so far by this thread have completed.
-__device__ __forceinline__ void umma_commit(uint32_t bar) {
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar)
-                 : "memory");
+// Arrive on the barrier at this shared-memory offset in BOTH CTAs once all tcgen05 ops issued so far completed.
+__device__ __forceinline__ void umma_commit_2cta(uint32_t bar) {
+    asm volatile(
+        "tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(bar),
+        "h"((uint16_t)3) : "memory");
 }
 // 32 lanes x 32 consecutive 32-bit columns: thread t of the warp gets lane (base+t), columns c..c+31.
 __device__ __forceinline__ void tmem_ld_32x32(uint32_t taddr, uint32_t (&v)[32]) {
@@ -164,8 +186,8 @@ __device__ __forceinline__ uint64_t make_kmajor_sw128_desc(uint32_t smem_addr) {
     const uint32_t hi = (1024u >> 4) | (1u << 14) | (2u << 29);              // SBO, version, SWIZZLE_128B
     return (static_cast<uint64_t>(hi) << 32) | lo;
 }
-// Instruction descriptor, kind::i8: D = s32, A = B = u8, both K-major, N = 256, M = 128.
-constexpr uint32_t TC_IDESC = (2u << 4) | ((TC_TN >> 3) << 17) | ((TC_TM >> 4) << 24);
+// Instruction descriptor, kind::i8: D = s32, A = B = u8, both K-major, N = 256, M = 256 (cta_group::2).
+constexpr uint32_t TC_IDESC = (2u << 4) | ((256u >> 3) << 17) | ((256u >> 4) << 24);
 
 // One 32-bit word of a row (32 k's) -> 32 operand bytes (two 16-byte chunks), each byte 0 or 1 << TB.
 // Class q of the word = bits q, q+8, q+16, q+24; they go to bit TB of the four bytes of one 32-bit lane, so one
@@ -184,12 +206,13 @@ __device__ __forceinline__ void unpack_word(uint32_t x, uint4& lo, uint4& hi) {
     hi.z = unpack_class<TB>(x, 6); hi.w = unpack_class<TB>(x, 7);
 }
 
-// keep local bit positions p (0..127) with p > r   (operand U in the stage that holds row i's own column)
+// Word m (bits 32m..32m+31) of a 128-column stage: keep local bit positions p with p > r (operand U in the
+// stages that hold row i's own column; r may be negative -> keep all, or >= 128 -> keep none).
 __device__ __forceinline__ uint32_t keep_gt(int r, int m) {
     const int s = r - 32 * m + 1;  // number of low bits to clear
     return s <= 0 ? 0xFFFFFFFFu : (s >= 32 ? 0u : (0xFFFFFFFFu << s));
 }
-// keep local bit positions p with p < lim   (operand L in the stages that hold row j's own column)
+// keep local bit positions p with p < lim (operand L in the stages that hold row j's own column)
 __device__ __forceinline__ uint32_t keep_lt(int lim, int m) {
     const int s = lim - 32 * m;    // number of low bits to keep
     return s <= 0 ? 0u : (s >= 32 ? 0xFFFFFFFFu : ((1u << s) - 1u));
@@ -197,138 +220,142 @@ __device__ __forceinline__ uint32_t keep_lt(int lim, int m) {
 
 // TB = bit of the operand byte that carries the relation bit: operands are 0 or 2^TB, every product is 4^TB, and
 // the accumulator holds n_ij << 2TB.  The host picks the largest TB with (N-2) << 2TB < 2^31 (exact in s32).
+// tiles[t] = {I, J}: 256-row blocks, I <= J.  Grid = 2 x (number of SM pairs), cluster (2,1,1).
 template <int TB>
-__global__ void __launch_bounds__(TC_THREADS, 1)
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(TC_THREADS, 1)
 tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_t* __restrict__ rel, long long N,
                      long long stride_words, int kmax, unsigned long long* __restrict__ counts,
                      const int2* __restrict__ tiles, int ntiles, int dbg) {
     extern __shared__ uint8_t smem_raw[];
-    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    // the dynamic shared window starts at the same offset in both CTAs, so this rounding is identical in both
+    const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    uint8_t* smem = smem_raw + (smem0 - smem_u32(smem_raw));
     unsigned int* hist = reinterpret_cast<unsigned int*>(smem + TC_OFF_HIST);
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + TC_OFF_BARS);
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + TC_NUM_BARS);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + TC_OFF_BARS + 8 * TC_NUM_BARS);
 
     const int tid = threadIdx.x;
     const int warp = tid >> 5, lane = tid & 31;
-    const uint32_t smem0 = smem_u32(smem);
-    const uint32_t full0 = smem_u32(bars), empty0 = full0 + 8 * TC_STAGES;
+    const uint32_t rank = cluster_ctarank();          // 0 = leader (issues the MMAs)
+    const uint32_t full0 = smem0 + TC_OFF_BARS, empty0 = full0 + 8 * TC_STAGES;
     const uint32_t tmem_full = empty0 + 8 * TC_STAGES, tmem_empty = tmem_full + 8;
     const uint32_t bits_full0 = tmem_empty + 8, bits_empty0 = bits_full0 + 8 * TC_BITS_BUFS;
 
     for (int b = tid; b < TC_HIST; b += TC_THREADS) hist[b] = 0u;
     if (tid == 0) {
         for (int s = 0; s < TC_STAGES; ++s) {
-            mbar_init(full0 + 8 * s, TC_PRODUCER_WARPS);   // one elected arrive per producer warp
-            mbar_init(empty0 + 8 * s, 1);                  // tcgen05.commit
+            mbar_init(full0 + 8 * s, 2 * TC_PRODUCER_WARPS);   // leader's copy is used: one arrive per producer warp of the pair
+            mbar_init(empty0 + 8 * s, 1);                      // multicast tcgen05.commit
         }
-        mbar_init(tmem_full, 1);
-        mbar_init(tmem_empty, TC_PRODUCERS);
+        mbar_init(tmem_full, 1);                               // multicast tcgen05.commit
+        mbar_init(tmem_empty, 2 * TC_PRODUCER_WARPS);          // leader's copy is used
         for (int b = 0; b < TC_BITS_BUFS; ++b) {
-            mbar_init(bits_full0 + 8 * b, 1);              // expect_tx arrive of the TMA thread
+            mbar_init(bits_full0 + 8 * b, 1);                  // expect_tx arrive of the TMA thread
             mbar_init(bits_empty0 + 8 * b, TC_PRODUCER_WARPS);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == TC_MMA_WARP) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)),
+        asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)),
                      "n"(TC_TMEM_COLS) : "memory");
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
     }
     tc_fence_before();
     __syncthreads();
+    cluster_sync_all();                               // both CTAs' barriers initialised before any remote arrive
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
 
-    const int G = gridDim.x, cta = blockIdx.x;
+    const int G = gridDim.x >> 1, cl = blockIdx.x >> 1;   // persistent clusters
     const int rounds = (ntiles + G - 1) / G;
 
     if (warp < TC_PRODUCER_WARPS) {
         // ================================================================== producers + epilogue
-        const bool isA = warp < 4;
-        const int r = isA ? tid : tid - 128;          // row inside the A (0..127) or B (0..255) tile
+        const int prow = tid >> 1, half = tid & 1;    // row 0..255 of this CTA's staged rows, 64-bit half of the stage
+        const bool isA = prow < TC_ROWS_A;
+        const int r = isA ? prow : prow - TC_ROWS_A;  // row inside this CTA's A or B operand tile
+        const int rt = (int)rank * 128 + r;           // row inside the 256-row block of the cluster tile
         const int q4 = warp & 3;                      // TMEM lane quarter this warp may read
-        const int cgrp = warp >> 2;                   // which third of the 8 column chunks it drains
-        const int c_begin = cgrp * 3, c_end = cgrp == 2 ? 8 : c_begin + 3;
+        const int cq = warp >> 2;                     // which 64 accumulator columns it drains
         uint32_t stage = 0, sphase = 0;               // operand ring position / parity
         uint32_t bb = 0, bphase = 0;                  // packed-bit ring position / parity
         uint32_t tphase = 0;                          // parity of tmem_full
         int pending = -1;                             // ring stage written but not yet published
         const uint32_t row_smem = smem0 + (isA ? 0 : TC_A_BYTES) + (r >> 3) * 1024 + (r & 7) * 128;
         const int sw = r & 7;
-        // this thread's row in a packed-bit buffer: 32 bytes per row, 16-byte halves swapped on odd groups of 4 rows
-        const uint32_t bits_row = smem0 + TC_OFF_BITS + tid * TC_BITS_ROW_BYTES;
-        const uint32_t bits_sw = ((tid >> 2) & 1) << 4;
+        // this thread's 8 bytes per stage in a packed-bit buffer: 32 bytes per row, 16-byte halves swapped on
+        // odd groups of 4 rows (TMA 32-byte swizzle)
+        const uint32_t bits_row = smem0 + TC_OFF_BITS + prow * TC_BITS_ROW_BYTES + half * 8;
+        const uint32_t bits_sw = ((prow >> 2) & 1) << 4;
+        const uint32_t full_leader0 = map_to_cta(full0, 0);
+        const uint32_t tmem_empty_leader = map_to_cta(tmem_empty, 0);
 
         for (int rd = 0; rd < rounds; ++rd) {
-            const int t = rd * G + ((rd & 1) ? (G - 1 - cta) : cta);
+            const int t = rd * G + ((rd & 1) ? (G - 1 - cl) : cl);
             if (t >= ntiles) continue;
             const int2 tile = tiles[t];
             const int I = tile.x, J = tile.y;
-            const long long i0 = (long long)I * TC_TM, j0 = (long long)J * TC_TN;
-            const int kb_begin = I, kb_end = 2 * J + 2;   // stages of 128 columns, [begin, end)
+            const long long i0 = (long long)I * TC_T, j0 = (long long)J * TC_T;
+            const int kb_begin = 2 * I, kb_end = 2 * J + 2;   // stages of 128 columns, [begin, end): always even count
 
             // Software pipeline: the fence + arrive that publishes stage s is issued after the ALU work of stage
             // s+1 (its stores have drained by then); the empty-slot barrier is probed before that ALU work.
             for (int kb0 = kb_begin; kb0 < kb_end; kb0 += TC_GROUP) {
                 mbar_wait(bits_full0 + 8 * bb, bphase);
-                uint4 cur[TC_GROUP];
+                uint2 cur[TC_GROUP];
 #pragma unroll
                 for (int u = 0; u < TC_GROUP; ++u)
-                    cur[u] = lds128(bits_row + bb * TC_BITS_BUF_BYTES + ((u << 4) ^ bits_sw));
+                    cur[u] = lds64(bits_row + bb * TC_BITS_BUF_BYTES + ((u << 4) ^ bits_sw));
                 __syncwarp();
                 if (lane == 0) mbar_arrive_after(bits_empty0 + 8 * bb, cur[0].x, cur[TC_GROUP - 1].x);
                 if (++bb == TC_BITS_BUFS) { bb = 0; bphase ^= 1; }
 #pragma unroll
                 for (int u = 0; u < TC_GROUP; ++u) {
                     const int kb = kb0 + u;
-                    if (kb < kb_end) {
-                        uint4 w = cur[u];
-                        if (isA) {
-                            if (kb == I) {
-                                w.x &= keep_gt(r, 0); w.y &= keep_gt(r, 1); w.z &= keep_gt(r, 2); w.w &= keep_gt(r, 3);
-                            }
-                        } else if (kb >= 2 * J) {
-                            const int lim = r - 128 * (kb - 2 * J);
-                            w.x &= keep_lt(lim, 0); w.y &= keep_lt(lim, 1); w.z &= keep_lt(lim, 2); w.w &= keep_lt(lim, 3);
+                    uint2 w = cur[u];
+                    if (isA) {
+                        if (kb < kb_begin + 2) {              // columns of block I: keep k > i
+                            const int rl = rt - 128 * (kb - kb_begin);
+                            w.x &= keep_gt(rl, 2 * half); w.y &= keep_gt(rl, 2 * half + 1);
                         }
-                        const bool slot_free = mbar_try(empty0 + 8 * stage, sphase ^ 1);
-                        uint4 o[8];
-                        if (dbg & 1) {
-#pragma unroll
-                            for (int c = 0; c < 8; ++c) o[c] = w;
-                        } else {
-                            unpack_word<TB>(w.x, o[0], o[1]);
-                            unpack_word<TB>(w.y, o[2], o[3]);
-                            unpack_word<TB>(w.z, o[4], o[5]);
-                            unpack_word<TB>(w.w, o[6], o[7]);
-                        }
-                        if (pending >= 0) {                   // publish the previous stage
-                            fence_proxy_async_smem_after(o);
-                            __syncwarp();
-                            if (lane == 0) mbar_arrive(full0 + 8 * pending);
-                        }
-                        if (!slot_free) mbar_wait(empty0 + 8 * stage, sphase ^ 1);
-                        const uint32_t rowp = row_smem + stage * TC_STAGE_BYTES;
-#pragma unroll
-                        for (int c = 0; c < 8; ++c)
-                            if (!(dbg & 4) || c == 0) sts128(rowp + ((c ^ sw) << 4), o[c]);
-                        pending = (int)stage;
-                        if (++stage == TC_STAGES) { stage = 0; sphase ^= 1; }
+                    } else if (kb >= kb_end - 2) {            // columns of block J: keep k < j
+                        const int lim = rt - 128 * (kb - (kb_end - 2));
+                        w.x &= keep_lt(lim, 2 * half); w.y &= keep_lt(lim, 2 * half + 1);
                     }
+                    const bool slot_free = mbar_try(empty0 + 8 * stage, sphase ^ 1);
+                    uint4 o[4];
+                    if (dbg & 1) {
+                        o[0] = o[1] = o[2] = o[3] = make_uint4(w.x, w.y, w.x, w.y);
+                    } else {
+                        unpack_word<TB>(w.x, o[0], o[1]);
+                        unpack_word<TB>(w.y, o[2], o[3]);
+                    }
+                    if (pending >= 0) {                       // publish the previous stage to the leader's MMA thread
+                        fence_proxy_async_smem_after(o);
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive_cluster(full_leader0 + 8 * pending);
+                    }
+                    if (!slot_free) mbar_wait(empty0 + 8 * stage, sphase ^ 1);
+                    const uint32_t rowp = row_smem + stage * TC_STAGE_BYTES;
+#pragma unroll
+                    for (int c = 0; c < 4; ++c)
+                        if (!(dbg & 4) || c == 0) sts128(rowp + (((4 * half + c) ^ sw) << 4), o[c]);
+                    pending = (int)stage;
+                    if (++stage == TC_STAGES) { stage = 0; sphase ^= 1; }
                 }
             }
             fence_proxy_async_smem();                          // publish the last stage of the tile
             __syncwarp();
-            if (lane == 0) mbar_arrive(full0 + 8 * pending);
+            if (lane == 0) mbar_arrive_cluster(full_leader0 + 8 * pending);
             pending = -1;
 
             // ---- epilogue: TMEM -> registers -> mask by R[i][j], i<j -> histogram
             mbar_wait(tmem_full, tphase);
             tphase ^= 1;
             tc_fence_after();
-            const long long i = i0 + 32 * q4 + lane;
+            const long long i = i0 + 128 * (int)rank + 32 * q4 + lane;
             const uint32_t* relrow32 = reinterpret_cast<const uint32_t*>(rel + (i < N ? i : 0) * stride_words);
-            for (int c = c_begin; c < c_end; ++c) {
+#pragma unroll 1
+            for (int c = 2 * cq; c < 2 * cq + 2; ++c) {
                 uint32_t v[32];
                 tmem_ld_32x32(tmem_base + ((uint32_t)(32 * q4) << 16) + (uint32_t)(32 * c), v);
                 const long long jc = j0 + 32 * c;
@@ -346,75 +373,78 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 }
             }
             tc_fence_before();
-            mbar_arrive(tmem_empty);
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(tmem_empty_leader);
         }
     } else if (warp == TC_MMA_WARP) {
-        // ================================================================== MMA issuer (one warp, lane 0 issues)
-        uint32_t stage = 0, sphase = 0, ephase = 0;
-        int done_tiles = 0;
-        for (int rd = 0; rd < rounds; ++rd) {
-            const int t = rd * G + ((rd & 1) ? (G - 1 - cta) : cta);
-            if (t >= ntiles) continue;
-            const int2 tile = tiles[t];
-            const int kb_begin = tile.x, kb_end = 2 * tile.y + 2;
-            if (done_tiles > 0) {                       // accumulator must have been drained
-                mbar_wait(tmem_empty, ephase);
-                ephase ^= 1;
-            }
-            tc_fence_after();
-            for (int kb = kb_begin; kb < kb_end; ++kb) {
-                mbar_wait(full0 + 8 * stage, sphase);
-                tc_fence_after();
-                if (lane == 0 && (dbg & 2)) {
-                    umma_commit(empty0 + 8 * stage);
-                    if (kb == kb_end - 1) umma_commit(tmem_full);
-                } else if (lane == 0) {
-                    const uint32_t a_addr = smem0 + stage * TC_STAGE_BYTES;
-                    const uint64_t adesc = make_kmajor_sw128_desc(a_addr);
-                    const uint64_t bdesc = make_kmajor_sw128_desc(a_addr + TC_A_BYTES);
-#pragma unroll
-                    for (int kk = 0; kk < TC_KS / 32; ++kk)   // K = 32 bytes per instruction: +2 in 16-byte units
-                        umma_i8(tmem_base, adesc + 2 * kk, bdesc + 2 * kk, TC_IDESC, (kb > kb_begin || kk > 0) ? 1u : 0u);
-                    umma_commit(empty0 + 8 * stage);
-                    if (kb == kb_end - 1) umma_commit(tmem_full);
+        // ================================================================== MMA issuer (leader CTA, lane 0 issues)
+        if (rank == 0) {
+            uint32_t stage = 0, sphase = 0, ephase = 0;
+            int done_tiles = 0;
+            for (int rd = 0; rd < rounds; ++rd) {
+                const int t = rd * G + ((rd & 1) ? (G - 1 - cl) : cl);
+                if (t >= ntiles) continue;
+                const int2 tile = tiles[t];
+                const int kb_begin = 2 * tile.x, kb_end = 2 * tile.y + 2;
+                if (done_tiles > 0) {                       // both CTAs' accumulators must have been drained
+                    mbar_wait(tmem_empty, ephase);
+                    ephase ^= 1;
                 }
-                __syncwarp();
-                if (++stage == TC_STAGES) { stage = 0; sphase ^= 1; }
+                tc_fence_after();
+                for (int kb = kb_begin; kb < kb_end; ++kb) {
+                    mbar_wait(full0 + 8 * stage, sphase);
+                    tc_fence_after();
+                    if (lane == 0) {
+                        if (!(dbg & 2)) {
+                            const uint32_t a_addr = smem0 + stage * TC_STAGE_BYTES;
+                            const uint64_t adesc = make_kmajor_sw128_desc(a_addr);
+                            const uint64_t bdesc = make_kmajor_sw128_desc(a_addr + TC_A_BYTES);
+#pragma unroll
+                            for (int kk = 0; kk < TC_KS / 32; ++kk)   // K = 32 bytes per instruction: +2 in 16-byte units
+                                umma_i8_2cta(tmem_base, adesc + 2 * kk, bdesc + 2 * kk, TC_IDESC,
+                                             (kb > kb_begin || kk > 0) ? 1u : 0u);
+                        }
+                        umma_commit_2cta(empty0 + 8 * stage);
+                        if (kb == kb_end - 1) umma_commit_2cta(tmem_full);
+                    }
+                    __syncwarp();
+                    if (++stage == TC_STAGES) { stage = 0; sphase ^= 1; }
+                }
+                ++done_tiles;
             }
-            ++done_tiles;
         }
     } else {
         // ================================================================== TMA warp: packed bits -> shared ring
         if (lane == 0) {
             uint32_t bb = 0, bphase = 0;
             for (int rd = 0; rd < rounds; ++rd) {
-                const int t = rd * G + ((rd & 1) ? (G - 1 - cta) : cta);
+                const int t = rd * G + ((rd & 1) ? (G - 1 - cl) : cl);
                 if (t >= ntiles) continue;
                 const int2 tile = tiles[t];
-                const int i0 = tile.x * TC_TM, j0 = tile.y * TC_TN;
-                const int kb_begin = tile.x, kb_end = 2 * tile.y + 2;
+                const int ia = tile.x * TC_T + 128 * (int)rank, jb = tile.y * TC_T + 128 * (int)rank;
+                const int kb_begin = 2 * tile.x, kb_end = 2 * tile.y + 2;
                 for (int kb0 = kb_begin; kb0 < kb_end; kb0 += TC_GROUP) {
                     mbar_wait(bits_empty0 + 8 * bb, bphase ^ 1);
                     const uint32_t bar = bits_full0 + 8 * bb;
                     const uint32_t dst = smem0 + TC_OFF_BITS + bb * TC_BITS_BUF_BYTES;
                     mbar_expect_tx(bar, TC_BITS_BUF_BYTES);
-                    tma_load_2d(dst, &bits_map, kb0 * 16, i0, bar);
-                    tma_load_2d(dst + TC_BITS_BOX_BYTES, &bits_map, kb0 * 16, j0, bar);
-                    tma_load_2d(dst + 2 * TC_BITS_BOX_BYTES, &bits_map, kb0 * 16, j0 + TC_BITS_BOX_ROWS, bar);
+                    tma_load_2d(dst, &bits_map, kb0 * 16, ia, bar);
+                    tma_load_2d(dst + TC_BITS_BOX_BYTES, &bits_map, kb0 * 16, jb, bar);
                     if (++bb == TC_BITS_BUFS) { bb = 0; bphase ^= 1; }
                 }
             }
         }
     }
 
-    // ---- teardown: flush the privatised histogram, release TMEM
+    // ---- teardown: flush the privatised histogram, release TMEM once neither CTA can touch the other any more
     tc_fence_before();
     __syncthreads();
-    tc_fence_after();
     for (int b = tid; b < TC_HIST && b <= kmax; b += TC_THREADS)
         if (hist[b]) atomicAdd(&counts[b], (unsigned long long)hist[b]);
+    cluster_sync_all();
+    tc_fence_after();
     if (warp == TC_MMA_WARP) {
-        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(TC_TMEM_COLS)
+        asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(TC_TMEM_COLS)
                      : "memory");
     }
 }
