@@ -12,8 +12,9 @@
 //     and each tensor core reads half of B from its own shared memory and half from its peer's;
 //   * per CTA one TMA thread streams the packed bits of its 256 rows (32 bytes = 2 stages per row per copy,
 //     32-byte-swizzled 2D boxes of 128 rows) into a 4-deep shared-memory ring: whole sectors, one issuing thread;
-//   * 16 producer warps (two threads per row) read 8 bytes per stage from that ring, expand the bits to
-//     bytes (0 or 1 << TB) and store them into a ring of K-major, 128-byte-swizzled operand tiles.  The order
+//   * 16 producer warps in two sets of 8 (one row per thread; set p takes stage p of every 2-stage copy) read 16
+//     bytes per stage from that ring, expand the bits to bytes (0 or 1 << TB) and store them into a 4-stage
+//     ring of K-major, 128-byte-swizzled operand tiles.  The order
 //     of the 32 k's inside a 32-bit word is permuted (bits q, q+8, q+16, q+24 share one 32-bit store); both
 //     operands use the same permutation and the MMA sums over k, so the result is unchanged;
 //   * one thread of the leader CTA issues tcgen05.mma.cta_group::2.kind::i8 (M=256, N=256, K=32, u8 x u8 -> s32,
@@ -49,7 +50,7 @@ constexpr int TC_BITS_BOX_ROWS = 128;
 constexpr int TC_BITS_BOX_BYTES = TC_BITS_BOX_ROWS * TC_BITS_ROW_BYTES;   // 4 KiB
 constexpr int TC_BITS_BUF_BYTES = TC_ROWS * TC_BITS_ROW_BYTES;            // 8 KiB
 constexpr int TC_BITS_BUFS = 4;
-constexpr int TC_PRODUCER_WARPS = 16;      // two threads per row: 8 warps for the A rows, 8 for the B rows
+constexpr int TC_PRODUCER_WARPS = 16;      // two sets of 8 warps; in a set: 4 warps for the A rows, 4 for the B rows
 constexpr int TC_PRODUCERS = TC_PRODUCER_WARPS * 32;
 constexpr int TC_MMA_WARP = TC_PRODUCER_WARPS;
 constexpr int TC_TMA_WARP = TC_PRODUCER_WARPS + 1;
@@ -119,9 +120,10 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map
         "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
         ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar) : "memory");
 }
-__device__ __forceinline__ uint2 lds64(uint32_t addr) {
-    uint2 v;
-    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr) : "memory");
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr)
+                 : "memory");
     return v;
 }
 // Elected arrive that also names two registers of the warp-wide loads it must not overtake.
@@ -135,14 +137,16 @@ __device__ __forceinline__ void sts128(uint32_t addr, const uint4& v) {
 __device__ __forceinline__ void fence_proxy_async_smem() {
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
-// Same fence, placed AFTER the computation of the 16 registers it names: the fake register dependency stops the
+// Same fence, placed AFTER the computation of the 32 registers it names: the fake register dependency stops the
 // compiler from sinking the unpack arithmetic below the fence, so the fence finds the previous stage's stores
 // already drained.
-__device__ __forceinline__ void fence_proxy_async_smem_after(uint4 (&o)[4]) {
+__device__ __forceinline__ void fence_proxy_async_smem_after(uint4 (&o)[8]) {
     asm volatile("fence.proxy.async.shared::cta;"
                  : "+r"(o[0].x), "+r"(o[0].y), "+r"(o[0].z), "+r"(o[0].w), "+r"(o[1].x), "+r"(o[1].y), "+r"(o[1].z),
                    "+r"(o[1].w), "+r"(o[2].x), "+r"(o[2].y), "+r"(o[2].z), "+r"(o[2].w), "+r"(o[3].x), "+r"(o[3].y),
-                   "+r"(o[3].z), "+r"(o[3].w)
+                   "+r"(o[3].z), "+r"(o[3].w), "+r"(o[4].x), "+r"(o[4].y), "+r"(o[4].z), "+r"(o[4].w), "+r"(o[5].x),
+                   "+r"(o[5].y), "+r"(o[5].z), "+r"(o[5].w), "+r"(o[6].x), "+r"(o[6].y), "+r"(o[6].z), "+r"(o[6].w),
+                   "+r"(o[7].x), "+r"(o[7].y), "+r"(o[7].z), "+r"(o[7].w)
                  :
                  : "memory");
 }
@@ -243,7 +247,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
     for (int b = tid; b < TC_HIST; b += TC_THREADS) hist[b] = 0u;
     if (tid == 0) {
         for (int s = 0; s < TC_STAGES; ++s) {
-            mbar_init(full0 + 8 * s, 2 * TC_PRODUCER_WARPS);   // leader's copy is used: one arrive per producer warp of the pair
+            mbar_init(full0 + 8 * s, TC_PRODUCER_WARPS);       // leader's copy is used: 8 warps of one producer set x 2 CTAs
             mbar_init(empty0 + 8 * s, 1);                      // multicast tcgen05.commit
         }
         mbar_init(tmem_full, 1);                               // multicast tcgen05.commit
@@ -270,22 +274,24 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
 
     if (warp < TC_PRODUCER_WARPS) {
         // ================================================================== producers + epilogue
-        const int prow = tid >> 1, half = tid & 1;    // row 0..255 of this CTA's staged rows, 64-bit half of the stage
+        // Two producer sets of 8 warps; set p expands stage p of every 2-stage group (one row per thread), so a
+        // warp has two stage times for the serial chain wait -> expand -> fence -> arrive -> store of its stage.
+        const int pset = warp >> 3;                   // 0 or 1: which stage of each group this thread expands
+        const int prow = tid & 255;                   // row 0..255 of this CTA's staged rows
         const bool isA = prow < TC_ROWS_A;
         const int r = isA ? prow : prow - TC_ROWS_A;  // row inside this CTA's A or B operand tile
         const int rt = (int)rank * 128 + r;           // row inside the 256-row block of the cluster tile
         const int q4 = warp & 3;                      // TMEM lane quarter this warp may read
         const int cq = warp >> 2;                     // which 64 accumulator columns it drains
-        uint32_t stage = 0, sphase = 0;               // operand ring position / parity
+        uint32_t gc = 0;                              // running group count: operand slot = pset + 2*(gc&1)
         uint32_t bb = 0, bphase = 0;                  // packed-bit ring position / parity
         uint32_t tphase = 0;                          // parity of tmem_full
         int pending = -1;                             // ring stage written but not yet published
         const uint32_t row_smem = smem0 + (isA ? 0 : TC_A_BYTES) + (r >> 3) * 1024 + (r & 7) * 128;
         const int sw = r & 7;
-        // this thread's 8 bytes per stage in a packed-bit buffer: 32 bytes per row, 16-byte halves swapped on
+        // this thread's 16 bytes per group in a packed-bit buffer: 32 bytes per row, 16-byte halves swapped on
         // odd groups of 4 rows (TMA 32-byte swizzle)
-        const uint32_t bits_row = smem0 + TC_OFF_BITS + prow * TC_BITS_ROW_BYTES + half * 8;
-        const uint32_t bits_sw = ((prow >> 2) & 1) << 4;
+        const uint32_t bits_row = smem0 + TC_OFF_BITS + prow * TC_BITS_ROW_BYTES + (((uint32_t)pset << 4) ^ (((prow >> 2) & 1) << 4));
         const uint32_t full_leader0 = map_to_cta(full0, 0);
         const uint32_t tmem_empty_leader = map_to_cta(tmem_empty, 0);
 
@@ -297,51 +303,47 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
             const long long i0 = (long long)I * TC_T, j0 = (long long)J * TC_T;
             const int kb_begin = 2 * I, kb_end = 2 * J + 2;   // stages of 128 columns, [begin, end): always even count
 
-            // Software pipeline: the fence + arrive that publishes stage s is issued after the ALU work of stage
-            // s+1 (its stores have drained by then); the empty-slot barrier is probed before that ALU work.
-            for (int kb0 = kb_begin; kb0 < kb_end; kb0 += TC_GROUP) {
+            // Software pipeline: the fence + arrive that publishes a stage is issued after the ALU work of this
+            // set's next stage (its stores have drained by then); the empty-slot barrier is probed before that work.
+            for (int kb0 = kb_begin; kb0 < kb_end; kb0 += TC_GROUP, ++gc) {
+                const uint32_t stage = pset + 2 * (gc & 1), sphase = (gc >> 1) & 1;
+                const int kb = kb0 + pset;
                 mbar_wait(bits_full0 + 8 * bb, bphase);
-                uint2 cur[TC_GROUP];
-#pragma unroll
-                for (int u = 0; u < TC_GROUP; ++u)
-                    cur[u] = lds64(bits_row + bb * TC_BITS_BUF_BYTES + ((u << 4) ^ bits_sw));
+                uint4 w = lds128(bits_row + bb * TC_BITS_BUF_BYTES);
                 __syncwarp();
-                if (lane == 0) mbar_arrive_after(bits_empty0 + 8 * bb, cur[0].x, cur[TC_GROUP - 1].x);
+                if (lane == 0) mbar_arrive_after(bits_empty0 + 8 * bb, w.x, w.w);
                 if (++bb == TC_BITS_BUFS) { bb = 0; bphase ^= 1; }
-#pragma unroll
-                for (int u = 0; u < TC_GROUP; ++u) {
-                    const int kb = kb0 + u;
-                    uint2 w = cur[u];
-                    if (isA) {
-                        if (kb < kb_begin + 2) {              // columns of block I: keep k > i
-                            const int rl = rt - 128 * (kb - kb_begin);
-                            w.x &= keep_gt(rl, 2 * half); w.y &= keep_gt(rl, 2 * half + 1);
-                        }
-                    } else if (kb >= kb_end - 2) {            // columns of block J: keep k < j
-                        const int lim = rt - 128 * (kb - (kb_end - 2));
-                        w.x &= keep_lt(lim, 2 * half); w.y &= keep_lt(lim, 2 * half + 1);
+                if (isA) {
+                    if (kb < kb_begin + 2) {                  // columns of block I: keep k > i
+                        const int rl = rt - 128 * (kb - kb_begin);
+                        w.x &= keep_gt(rl, 0); w.y &= keep_gt(rl, 1); w.z &= keep_gt(rl, 2); w.w &= keep_gt(rl, 3);
                     }
-                    const bool slot_free = mbar_try(empty0 + 8 * stage, sphase ^ 1);
-                    uint4 o[4];
-                    if (dbg & 1) {
-                        o[0] = o[1] = o[2] = o[3] = make_uint4(w.x, w.y, w.x, w.y);
-                    } else {
-                        unpack_word<TB>(w.x, o[0], o[1]);
-                        unpack_word<TB>(w.y, o[2], o[3]);
-                    }
-                    if (pending >= 0) {                       // publish the previous stage to the leader's MMA thread
-                        fence_proxy_async_smem_after(o);
-                        __syncwarp();
-                        if (lane == 0) mbar_arrive_cluster(full_leader0 + 8 * pending);
-                    }
-                    if (!slot_free) mbar_wait(empty0 + 8 * stage, sphase ^ 1);
-                    const uint32_t rowp = row_smem + stage * TC_STAGE_BYTES;
-#pragma unroll
-                    for (int c = 0; c < 4; ++c)
-                        if (!(dbg & 4) || c == 0) sts128(rowp + (((4 * half + c) ^ sw) << 4), o[c]);
-                    pending = (int)stage;
-                    if (++stage == TC_STAGES) { stage = 0; sphase ^= 1; }
+                } else if (kb >= kb_end - 2) {                // columns of block J: keep k < j
+                    const int lim = rt - 128 * (kb - (kb_end - 2));
+                    w.x &= keep_lt(lim, 0); w.y &= keep_lt(lim, 1); w.z &= keep_lt(lim, 2); w.w &= keep_lt(lim, 3);
                 }
+                const bool slot_free = mbar_try(empty0 + 8 * stage, sphase ^ 1);
+                uint4 o[8];
+                if (dbg & 1) {
+#pragma unroll
+                    for (int c = 0; c < 8; ++c) o[c] = w;
+                } else {
+                    unpack_word<TB>(w.x, o[0], o[1]);
+                    unpack_word<TB>(w.y, o[2], o[3]);
+                    unpack_word<TB>(w.z, o[4], o[5]);
+                    unpack_word<TB>(w.w, o[6], o[7]);
+                }
+                if (pending >= 0) {                           // publish this set's previous stage to the leader's MMA thread
+                    fence_proxy_async_smem_after(o);
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive_cluster(full_leader0 + 8 * pending);
+                }
+                if (!slot_free) mbar_wait(empty0 + 8 * stage, sphase ^ 1);
+                const uint32_t rowp = row_smem + stage * TC_STAGE_BYTES;
+#pragma unroll
+                for (int c = 0; c < 8; ++c)
+                    if (!(dbg & 4) || c == 0) sts128(rowp + ((c ^ sw) << 4), o[c]);
+                pending = (int)stage;
             }
             fence_proxy_async_smem();                          // publish the last stage of the tile
             __syncwarp();
