@@ -220,7 +220,8 @@ def run_ours(args, cfg, rank, local_rank, world):
     counts = torch.empty(kmax + 1, dtype=torch.int64, device="cuda")
     S = torch.empty(1, dtype=torch.float64, device="cuda")
     variant = csg.csg_effective_variant(N)
-    kernel_name = "tensor_action_kernel" if variant == csg.VARIANT_TENSOR else "bitset_action_kernel"
+    kernel_name = {csg.VARIANT_BITSET: "bitset_action_kernel", csg.VARIANT_TENSOR: "tensor_action_kernel<KIND_I8>",
+                   csg.VARIANT_TENSOR_FP4: "tensor_action_kernel<KIND_FP4>"}[variant]
 
     def barrier():
         if dist is not None:
@@ -279,15 +280,17 @@ def run_ours(args, cfg, rank, local_rank, world):
     e2e_value = world * triples * e2e_steps / (e2e_ms * 1e-3)
     k_ms = sum(kernel_ms) / len(kernel_ms)
     peaks = read_peaks()
-    if variant == csg.VARIANT_TENSOR:
-        # dense binary contraction on tcgen05 kind::i8: 1 triple test = 1 MAC = 2 int8 ops.
-        # peak = measured bf16 dense peak x 2 (nominal int8:bf16 ratio of B200, B200_PROFILING.md table).
+    if variant in (csg.VARIANT_TENSOR, csg.VARIANT_TENSOR_FP4):
+        # dense binary contraction on tcgen05: 1 triple test = 1 MAC = 2 ops.  peak = measured bf16 dense peak x the
+        # nominal ratio of the operand type on B200 (B200_PROFILING.md table: int8/fp8 2x, fp4 4x bf16).
+        ratio = 4.0 if variant == csg.VARIANT_TENSOR_FP4 else 2.0
         achieved = 2.0 * triples / (k_ms * 1e-3) / 1e12
-        roofline = {"bound": "tensor", "kernel": kernel_name, "achieved": achieved, "peak": 2.0 * peaks["bf16"],
-                    "unit": "TOP/s (int8)", "frac": achieved / (2.0 * peaks["bf16"]),
-                    "peak_sustained": 2.0 * peaks["bf16_sustained"],
-                    "frac_of_sustained": achieved / (2.0 * peaks["bf16_sustained"]),
-                    "peak_source": "2 x bf16 " + peaks["source"], "kernel_ms": k_ms,
+        roofline = {"bound": "tensor", "kernel": kernel_name, "achieved": achieved, "peak": ratio * peaks["bf16"],
+                    "unit": "TOP/s (%s)" % ("fp4 e2m1, kind::mxf4" if ratio == 4.0 else "int8, kind::i8"),
+                    "frac": achieved / (ratio * peaks["bf16"]),
+                    "peak_sustained": ratio * peaks["bf16_sustained"],
+                    "frac_of_sustained": achieved / (ratio * peaks["bf16_sustained"]),
+                    "peak_source": "%g x bf16 " % ratio + peaks["source"], "kernel_ms": k_ms,
                     "traffic": read_traffic(kernel_name)}
     else:
         # LOP3+POPC+IADD per 32 triple tests; POPC pipe 16 lanes/clk/SM x 148 SMs x 1.965 GHz
@@ -314,10 +317,12 @@ def run_ours(args, cfg, rank, local_rank, world):
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "u8 x u8 -> s32 (tcgen05 kind::i8)" if variant == csg.VARIANT_TENSOR else "u32 and/popc",
+        "dtype": {csg.VARIANT_TENSOR: "u8 x u8 -> s32 (tcgen05 kind::i8)",
+                  csg.VARIANT_TENSOR_FP4: "e2m1 x e2m1 -> f32, exact integers (tcgen05 kind::mxf4, unit scales)",
+                  csg.VARIANT_BITSET: "u32 and/popc"}[variant],
         "data": "synthetic",
         "config": {"workload": workload_name(cfg), "N": N, "dim": dim, "eps": eps, "kmax": kmax, "seed": cfg["seed"],
-                   "variant": {1: "bitset", 2: "tensor"}[variant], "bitset_bytes": N * csg.csg_row_stride_words(N) * 8,
+                   "variant": {1: "bitset", 2: "tensor_i8", 3: "tensor_fp4"}[variant], "bitset_bytes": N * csg.csg_row_stride_words(N) * 8,
                    "l2": "input (%.0f MiB) %s L2 (126 MB)" % (N * csg.csg_row_stride_words(N) * 8 / 2**20,
                                                             "larger than" if N * csg.csg_row_stride_words(N) * 8 > 126e6
                                                             else "fits in"),
@@ -346,7 +351,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, help="index into BASELINE.json configs (default 3, the headline)")
-    ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 bitset, 2 tensor")
+    ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 bitset, 2 tensor int8, 3 tensor fp4")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))

@@ -49,9 +49,11 @@ enum {
 #define CSG_MAX_KMAX (1 << 22)
 
 enum {
-    CSG_VARIANT_AUTO = 0,   /* tensor variant when N >= 2048, else bitset */
+    CSG_VARIANT_AUTO = 0,   /* fp4 tensor variant when N >= 2048, else bitset */
     CSG_VARIANT_BITSET = 1, /* LOP3 AND + POPC over packed 32-bit words, register micro-tiles */
-    CSG_VARIANT_TENSOR = 2  /* bits unpacked to 0/1 u8 in shared memory, tcgen05.mma kind::i8 into TMEM */
+    CSG_VARIANT_TENSOR = 2, /* bits unpacked to u8 in shared memory, tcgen05.mma kind::i8, s32 accumulators in TMEM */
+    CSG_VARIANT_TENSOR_FP4 = 3 /* bits unpacked to e2m1 nibbles, tcgen05.mma kind::mxf4 with unit block scales, f32
+                                  accumulators (exact: every partial sum is an integer below 2^24) */
 };
 
 /* Row stride of the relation matrix in 64-bit words: 4*ceil(N/256) (rows 256-bit aligned). */
@@ -94,7 +96,7 @@ int csg_interval_sizes(const uint64_t *rel_bits, int64_t N, const int64_t *pairs
 
 /* Choose the kernel variant for later csg_action calls (CSG_VARIANT_*); returns CSG_E_VARIANT if unknown. */
 int csg_set_variant(int variant);
-/* The variant csg_action would run for this N under the current setting (CSG_VARIANT_BITSET or _TENSOR). */
+/* The variant csg_action would run for this N under the current setting (CSG_VARIANT_BITSET, _TENSOR or _TENSOR_FP4). */
 int csg_effective_variant(int64_t N);
 
 /*

@@ -16,7 +16,7 @@ import numpy as np
 
 from . import _build
 
-VARIANT_AUTO, VARIANT_BITSET, VARIANT_TENSOR = 0, 1, 2
+VARIANT_AUTO, VARIANT_BITSET, VARIANT_TENSOR, VARIANT_TENSOR_FP4 = 0, 1, 2, 3
 LIB_PATH = _build.LIB_PATH
 
 EXPORTS = [

@@ -90,9 +90,9 @@ struct State {
     bool attr_set = false;
     // TMA descriptor of the relation matrix seen as N rows of stride*8 bytes (cached per pointer and N)
     void* encode_tiled = nullptr;
-    CUtensorMap bits_map;
-    const void* map_ptr = nullptr;
-    long long map_N = -1;
+    CUtensorMap bits_map[2];            // [KIND_I8], [KIND_FP4]
+    const void* map_ptr[2] = {nullptr, nullptr};
+    long long map_N[2] = {-1, -1};
     // end-to-end (host buffer) path
     cudaStream_t host_stream = nullptr;
     uint64_t* d_bits = nullptr;
@@ -131,7 +131,7 @@ static int ensure_device() {
 
 static int effective_variant(long long N) {
     if (g.variant != CSG_VARIANT_AUTO) return g.variant;
-    return N >= 2048 ? CSG_VARIANT_TENSOR : CSG_VARIANT_BITSET;
+    return N >= 2048 ? CSG_VARIANT_TENSOR_FP4 : CSG_VARIANT_BITSET;
 }
 
 // Tiles (I, J) of the tensor variant in 256-row blocks, I <= J; K-depth in 128-column stages = 2(J-I)+2.
@@ -155,15 +155,15 @@ static int ensure_tiles(long long N, cudaStream_t stream) {
     return CSG_OK;
 }
 
-// 2D byte view of the packed relation matrix for the TMA warp of the tensor variant: dim0 = stride*8 bytes of a
-// row, dim1 = N rows; box = 32 bytes x 128 rows, 32-byte swizzle (conflict-free 16-byte reads by the producers);
-// rows >= N and bytes beyond the row are zero-filled by the hardware.
+// 2D byte view of the packed relation matrix for the TMA warp of the tensor variants: dim0 = stride*8 bytes of a
+// row, dim1 = N rows; box = 32 (int8) or 64 (fp4) bytes x 128 rows with the matching 32/64-byte swizzle
+// (conflict-free 16-byte reads by the producers); rows >= N and bytes beyond the row are zero-filled by the hardware.
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-static int ensure_bits_map(const uint64_t* rel_bits, long long N, long long stride_words) {
-    if (g.map_ptr == rel_bits && g.map_N == N) return CSG_OK;
+static int ensure_bits_map(int kind, const uint64_t* rel_bits, long long N, long long stride_words) {
+    if (g.map_ptr[kind] == rel_bits && g.map_N[kind] == N) return CSG_OK;
     if (!g.encode_tiled) {
         cudaDriverEntryPointQueryResult qres;
         CSG_CUDA(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &g.encode_tiled, cudaEnableDefault, &qres));
@@ -173,21 +173,22 @@ static int ensure_bits_map(const uint64_t* rel_bits, long long N, long long stri
             return CSG_E_CUDA;
         }
     }
+    const int row_bytes = kind == KIND_FP4 ? TcTraits<KIND_FP4>::BITS_ROW_BYTES : TcTraits<KIND_I8>::BITS_ROW_BYTES;
     const cuuint64_t dims[2] = {(cuuint64_t)stride_words * 8, (cuuint64_t)N};
     const cuuint64_t strides[1] = {(cuuint64_t)stride_words * 8};
-    const cuuint32_t box[2] = {(cuuint32_t)TC_BITS_ROW_BYTES, (cuuint32_t)TC_BITS_BOX_ROWS};
+    const cuuint32_t box[2] = {(cuuint32_t)row_bytes, (cuuint32_t)TC_BITS_BOX_ROWS};
     const cuuint32_t estr[2] = {1, 1};
     CUresult r = reinterpret_cast<EncodeTiledFn>(g.encode_tiled)(
-        &g.bits_map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<uint64_t*>(rel_bits), dims, strides, box, estr,
-        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        &g.bits_map[kind], CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<uint64_t*>(rel_bits), dims, strides, box, estr,
+        CU_TENSOR_MAP_INTERLEAVE_NONE, kind == KIND_FP4 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_32B,
+        CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
         snprintf(g.cuda_msg, sizeof(g.cuda_msg), "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
-        g.map_ptr = nullptr;
+        g.map_ptr[kind] = nullptr;
         return CSG_E_CUDA;
     }
-    g.map_ptr = rel_bits;
-    g.map_N = N;
+    g.map_ptr[kind] = rel_bits;
+    g.map_N[kind] = N;
     return CSG_OK;
 }
 
@@ -210,16 +211,20 @@ static int action_device(const uint64_t* rel_bits, long long N, int dim, double 
     const long long stride = csg_row_stride_words(N);
     CSG_CUDA(cudaMemsetAsync(counts, 0, (size_t)(kmax + 1) * sizeof(long long), stream));
     const int variant = effective_variant(N);
-    if (variant == CSG_VARIANT_TENSOR) {
+    const bool tensor = variant == CSG_VARIANT_TENSOR || variant == CSG_VARIANT_TENSOR_FP4;
+    const int kind = variant == CSG_VARIANT_TENSOR_FP4 ? KIND_FP4 : KIND_I8;
+    if (tensor) {
         rc = ensure_tiles(N, stream);
         if (rc) return rc;
-        rc = ensure_bits_map(rel_bits, N, stride);
+        rc = ensure_bits_map(kind, rel_bits, N, stride);
         if (rc) return rc;
         if (!g.attr_set) {
-            CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM_BYTES));
-            CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM_BYTES));
-            CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM_BYTES));
-            CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM_BYTES));
+            const int s8 = TcTraits<KIND_I8>::SMEM_BYTES, s4 = TcTraits<KIND_FP4>::SMEM_BYTES;
+            CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_I8, 7>, cudaFuncAttributeMaxDynamicSharedMemorySize, s8));
+            CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_I8, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, s8));
+            CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_I8, 5>, cudaFuncAttributeMaxDynamicSharedMemorySize, s8));
+            CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_I8, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, s8));
+            CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_FP4, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, s4));
             g.attr_set = true;
         }
     }
@@ -231,21 +236,24 @@ static int action_device(const uint64_t* rel_bits, long long N, int dim, double 
         }
         CSG_CUDA(cudaEventRecord(g.ev0[slot], stream));
     }
-    if (variant == CSG_VARIANT_TENSOR) {
+    if (tensor) {
         const int grid = 2 * std::max(1, std::min(g.ntiles, g.sm_count / 2));   // one CTA pair per SM pair
-        // operand bit TB: the accumulator holds n_ij << 2TB and n_ij <= N-2, so TB is the largest with
-        // (N-2) << 2TB < 2^31; TB = 7 turns every unpack shift into a left shift (FMA pipe).
         unsigned long long* c64 = reinterpret_cast<unsigned long long*>(counts);
         const char* dbg_env = getenv("CSG_DEBUG");
         const int dbg = dbg_env ? atoi(dbg_env) : 0;
-        if (N - 2 < (1LL << 17))
-            tensor_action_kernel<7><<<grid, TC_THREADS, TC_SMEM_BYTES, stream>>>(g.bits_map, rel_bits, N, stride, kmax, c64, g.d_tiles, g.ntiles, dbg);
+        const int s8 = TcTraits<KIND_I8>::SMEM_BYTES, s4 = TcTraits<KIND_FP4>::SMEM_BYTES;
+        // int8: operand bit TB: the accumulator holds n_ij << 2TB and n_ij <= N-2, so TB is the largest with
+        // (N-2) << 2TB < 2^31; TB = 7 turns every unpack shift into a left shift (FMA pipe).
+        if (kind == KIND_FP4)
+            tensor_action_kernel<KIND_FP4, 0><<<grid, TC_THREADS, s4, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, g.d_tiles, g.ntiles, dbg);
+        else if (N - 2 < (1LL << 17))
+            tensor_action_kernel<KIND_I8, 7><<<grid, TC_THREADS, s8, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, g.d_tiles, g.ntiles, dbg);
         else if (N - 2 < (1LL << 19))
-            tensor_action_kernel<6><<<grid, TC_THREADS, TC_SMEM_BYTES, stream>>>(g.bits_map, rel_bits, N, stride, kmax, c64, g.d_tiles, g.ntiles, dbg);
+            tensor_action_kernel<KIND_I8, 6><<<grid, TC_THREADS, s8, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, g.d_tiles, g.ntiles, dbg);
         else if (N - 2 < (1LL << 21))
-            tensor_action_kernel<5><<<grid, TC_THREADS, TC_SMEM_BYTES, stream>>>(g.bits_map, rel_bits, N, stride, kmax, c64, g.d_tiles, g.ntiles, dbg);
+            tensor_action_kernel<KIND_I8, 5><<<grid, TC_THREADS, s8, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, g.d_tiles, g.ntiles, dbg);
         else
-            tensor_action_kernel<4><<<grid, TC_THREADS, TC_SMEM_BYTES, stream>>>(g.bits_map, rel_bits, N, stride, kmax, c64, g.d_tiles, g.ntiles, dbg);
+            tensor_action_kernel<KIND_I8, 4><<<grid, TC_THREADS, s8, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, g.d_tiles, g.ntiles, dbg);
     } else {
         const long long nb = (N + BS_T - 1) / BS_T;
         const long long ntiles = nb * (nb + 1) / 2;
@@ -341,7 +349,7 @@ int csg_interval_sizes(const uint64_t* rel_bits, int64_t N, const int64_t* pairs
 
 int csg_set_variant(int variant) {
     std::lock_guard<std::mutex> lock(g.mu);
-    if (variant != CSG_VARIANT_AUTO && variant != CSG_VARIANT_BITSET && variant != CSG_VARIANT_TENSOR)
+    if (variant < CSG_VARIANT_AUTO || variant > CSG_VARIANT_TENSOR_FP4)
         return CSG_E_VARIANT;
     g.variant = variant;
     return CSG_OK;
@@ -424,8 +432,8 @@ int csg_shutdown(void) {
     g.d_S = nullptr;
     g.host_stream = nullptr;
     g.tiles_N = -1;
-    g.map_ptr = nullptr;
-    g.map_N = -1;
+    g.map_ptr[0] = g.map_ptr[1] = nullptr;
+    g.map_N[0] = g.map_N[1] = -1;
     g.d_bits_bytes = g.d_counts_bytes = 0;
     g.timed_calls = 0;
     cudaGetLastError();

@@ -39,16 +39,13 @@ constexpr int TC_T = 256;                  // tile edge in pairs (UMMA M = N = 2
 constexpr int TC_ROWS_A = 128;             // A rows per CTA
 constexpr int TC_ROWS_B = 128;             // B rows per CTA
 constexpr int TC_ROWS = TC_ROWS_A + TC_ROWS_B;
-constexpr int TC_KS = 128;                 // k columns per stage = bytes per operand row in smem
+constexpr int TC_ROW_BYTES = 128;          // bytes per operand row per stage in smem (one 128-byte swizzle row)
 constexpr int TC_STAGES = 4;
-constexpr int TC_A_BYTES = TC_ROWS_A * TC_KS;  // 16 KiB
-constexpr int TC_B_BYTES = TC_ROWS_B * TC_KS;  // 16 KiB
+constexpr int TC_A_BYTES = TC_ROWS_A * TC_ROW_BYTES;  // 16 KiB
+constexpr int TC_B_BYTES = TC_ROWS_B * TC_ROW_BYTES;  // 16 KiB
 constexpr int TC_STAGE_BYTES = TC_A_BYTES + TC_B_BYTES;
 constexpr int TC_GROUP = 2;                // stages covered by one packed-bit copy
-constexpr int TC_BITS_ROW_BYTES = TC_GROUP * TC_KS / 8;   // 32
 constexpr int TC_BITS_BOX_ROWS = 128;
-constexpr int TC_BITS_BOX_BYTES = TC_BITS_BOX_ROWS * TC_BITS_ROW_BYTES;   // 4 KiB
-constexpr int TC_BITS_BUF_BYTES = TC_ROWS * TC_BITS_ROW_BYTES;            // 8 KiB
 constexpr int TC_BITS_BUFS = 4;
 constexpr int TC_PRODUCER_WARPS = 16;      // two sets of 8 warps; in a set: 4 warps for the A rows, 4 for the B rows
 constexpr int TC_PRODUCERS = TC_PRODUCER_WARPS * 32;
@@ -56,12 +53,28 @@ constexpr int TC_MMA_WARP = TC_PRODUCER_WARPS;
 constexpr int TC_TMA_WARP = TC_PRODUCER_WARPS + 1;
 constexpr int TC_THREADS = TC_PRODUCERS + 64;  // + the MMA warp + the TMA warp
 constexpr int TC_HIST = 2048;              // privatised low bins per CTA
-constexpr int TC_TMEM_COLS = 256;
-constexpr int TC_OFF_BITS = TC_STAGES * TC_STAGE_BYTES;
-constexpr int TC_OFF_HIST = TC_OFF_BITS + TC_BITS_BUFS * TC_BITS_BUF_BYTES;
-constexpr int TC_OFF_BARS = TC_OFF_HIST + TC_HIST * 4;
 constexpr int TC_NUM_BARS = 2 * TC_STAGES + 2 + 2 * TC_BITS_BUFS;
-constexpr int TC_SMEM_BYTES = TC_OFF_BARS + 8 * TC_NUM_BARS + 16 + 1024;  // + TMEM slot + alignment slack
+constexpr int TC_OFF_BITS = TC_STAGES * TC_STAGE_BYTES;
+
+// The two operand encodings of the kernel.
+//   KIND_I8 : one relation bit -> one u8 (0 or 1 << TB); tcgen05.mma kind::i8, K = 32 per instruction, s32
+//             accumulators; a stage row of 128 bytes covers 128 columns.
+//   KIND_FP4: one relation bit -> one e2m1 nibble (0 or 2.0 = 0b0100), two per byte; tcgen05.mma kind::mxf4 with
+//             all block scales 1.0 (UE8M0 0x7F), K = 64 per instruction, f32 accumulators holding 4 n_ij (exact
+//             below 2^24); a stage row of 128 bytes covers 256 columns, at twice the int8 MAC rate.
+constexpr int KIND_I8 = 0, KIND_FP4 = 1;
+template <int KIND>
+struct TcTraits {
+    static constexpr int STAGE_COLS = KIND == KIND_FP4 ? 256 : 128;           // k columns per stage
+    static constexpr int WORDS = STAGE_COLS / 32;                             // packed 32-bit words per row per stage
+    static constexpr int BITS_ROW_BYTES = TC_GROUP * STAGE_COLS / 8;          // 32 or 64 bytes per row per copy
+    static constexpr int BITS_BOX_BYTES = TC_BITS_BOX_ROWS * BITS_ROW_BYTES;
+    static constexpr int BITS_BUF_BYTES = TC_ROWS * BITS_ROW_BYTES;           // 8 or 16 KiB
+    static constexpr int OFF_HIST = TC_OFF_BITS + TC_BITS_BUFS * BITS_BUF_BYTES;
+    static constexpr int OFF_BARS = OFF_HIST + TC_HIST * 4;
+    static constexpr int SMEM_BYTES = OFF_BARS + 8 * TC_NUM_BARS + 16 + 1024;  // + TMEM slot + alignment slack
+    static constexpr int TMEM_COLS = KIND == KIND_FP4 ? 512 : 256;            // fp4: + 256 columns of scale factors
+};
 
 // ---------------------------------------------------------------------------------------------- PTX helpers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
@@ -193,10 +206,33 @@ __device__ __forceinline__ uint64_t make_kmajor_sw128_desc(uint32_t smem_addr) {
 // Instruction descriptor, kind::i8: D = s32, A = B = u8, both K-major, N = 256, M = 256 (cta_group::2).
 constexpr uint32_t TC_IDESC = (2u << 4) | ((256u >> 3) << 17) | ((256u >> 4) << 24);
 
-// One 32-bit word of a row (32 k's) -> 32 operand bytes (two 16-byte chunks), each byte 0 or 1 << TB.
+// D[tmem] (+)= A[smem] * B[smem]^T, e2m1 x e2m1 -> f32 with UE8M0 block scales (one per 32 k) read from TMEM,
+// over the CTA pair (issued by the leader CTA only).  K = 64 per instruction.
+__device__ __forceinline__ void umma_mxf4_2cta(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                               uint32_t accumulate, uint32_t tmem_sfa, uint32_t tmem_sfb) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::mxf4.block_scale.block32 [%0], %1, %2, %3, [%5], [%6], p;\n\t}" ::"r"(tmem_d),
+        "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate), "r"(tmem_sfa), "r"(tmem_sfb) : "memory");
+}
+// Instruction descriptor, kind::mxf4 block scaled: A = B = e2m1 (1), scales UE8M0 (1), K-major, N = 256, M = 256,
+// scale-factor ids 0, K = 64.
+constexpr uint32_t TC_IDESC_FP4 = (1u << 7) | (1u << 10) | ((256u >> 3) << 17) | (1u << 23) | ((256u >> 4) << 24);
+// 32 lanes x 32 columns store of one value (fills the scale-factor region of TMEM).
+__device__ __forceinline__ void tmem_fill_32x32(uint32_t taddr, uint32_t v) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+        "{%1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, "
+        "%1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1};" ::"r"(taddr), "r"(v) : "memory");
+}
+
+// ---------------------------------------------------------------------------------------------- bit expansion
+// KIND_I8.  One 32-bit word of a row (32 k's) -> 32 operand bytes (two 16-byte chunks), each 0 or 1 << TB.
 // Class q of the word = bits q, q+8, q+16, q+24; they go to bit TB of the four bytes of one 32-bit lane, so one
 // shift and one AND expand four k's.  Left shifts (q < TB) may be issued as IMAD.SHL on the FMA pipe, which
-// unloads the ALU pipe that carries the ANDs: TB = 7 needs no right shift at all.
+// unloads the ALU pipe that carries the ANDs: TB = 7 needs no right shift at all.  The order of the k's inside
+// the word is permuted; both operands use the same permutation and the MMA sums over k.
 template <int TB>
 __device__ __forceinline__ uint32_t unpack_class(uint32_t x, int q) {
     constexpr uint32_t M = 0x01010101u << TB;
@@ -209,9 +245,19 @@ __device__ __forceinline__ void unpack_word(uint32_t x, uint4& lo, uint4& hi) {
     hi.x = unpack_class<TB>(x, 4); hi.y = unpack_class<TB>(x, 5);
     hi.z = unpack_class<TB>(x, 6); hi.w = unpack_class<TB>(x, 7);
 }
+// KIND_FP4.  One 32-bit word (32 k's) -> 32 e2m1 nibbles (one 16-byte chunk), each 0 or 0b0100 (= 2.0).
+// Class q = bits q, q+4, ..., q+28 goes to bit 2 of the eight nibbles of one 32-bit lane.
+__device__ __forceinline__ uint4 unpack_word_fp4(uint32_t x) {
+    uint4 o;
+    o.x = (x << 2) & 0x44444444u;
+    o.y = (x << 1) & 0x44444444u;
+    o.z = x & 0x44444444u;
+    o.w = (x >> 1) & 0x44444444u;
+    return o;
+}
 
-// Word m (bits 32m..32m+31) of a 128-column stage: keep local bit positions p with p > r (operand U in the
-// stages that hold row i's own column; r may be negative -> keep all, or >= 128 -> keep none).
+// Word m (bits 32m..32m+31) of a stage: keep local bit positions p with p > r (operand U in the stages that
+// hold row i's own column; r may be negative -> keep all, or beyond the stage -> keep none).
 __device__ __forceinline__ uint32_t keep_gt(int r, int m) {
     const int s = r - 32 * m + 1;  // number of low bits to clear
     return s <= 0 ? 0xFFFFFFFFu : (s >= 32 ? 0u : (0xFFFFFFFFu << s));
@@ -222,25 +268,40 @@ __device__ __forceinline__ uint32_t keep_lt(int lim, int m) {
     return s <= 0 ? 0u : (s >= 32 ? 0xFFFFFFFFu : ((1u << s) - 1u));
 }
 
-// TB = bit of the operand byte that carries the relation bit: operands are 0 or 2^TB, every product is 4^TB, and
-// the accumulator holds n_ij << 2TB.  The host picks the largest TB with (N-2) << 2TB < 2^31 (exact in s32).
+// K range of tile (I, J) in stages of COLS columns: from the stage holding column 256 I to the one holding
+// column 256 J + 255, widened by one fully masked stage when the count would be odd (the two producer sets
+// own the even and the odd ring slots).
+template <int COLS>
+__device__ __forceinline__ void tile_k_range(int I, int J, int& kb_begin, int& kb_end) {
+    kb_begin = (256 * I) / COLS;
+    kb_end = (256 * J + 255) / COLS + 1;
+    if ((kb_end - kb_begin) & 1) {
+        if (kb_begin > 0) --kb_begin; else ++kb_end;
+    }
+}
+
+// KIND_I8: TB = bit of the operand byte that carries the relation bit: operands are 0 or 2^TB, every product is
+// 4^TB, the accumulator holds n_ij << 2TB; the host picks the largest TB with (N-2) << 2TB < 2^31 (exact in s32).
+// KIND_FP4: TB unused (pass 0); the f32 accumulator holds 4 n_ij, exact for n_ij < 2^22.
 // tiles[t] = {I, J}: 256-row blocks, I <= J.  Grid = 2 x (number of SM pairs), cluster (2,1,1).
-template <int TB>
+template <int KIND, int TB>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(TC_THREADS, 1)
 tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_t* __restrict__ rel, long long N,
                      long long stride_words, int kmax, unsigned long long* __restrict__ counts,
                      const int2* __restrict__ tiles, int ntiles, int dbg) {
+    using T = TcTraits<KIND>;
+    constexpr int COLS = T::STAGE_COLS, WORDS = T::WORDS;
     extern __shared__ uint8_t smem_raw[];
     // the dynamic shared window starts at the same offset in both CTAs, so this rounding is identical in both
     const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* smem = smem_raw + (smem0 - smem_u32(smem_raw));
-    unsigned int* hist = reinterpret_cast<unsigned int*>(smem + TC_OFF_HIST);
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + TC_OFF_BARS + 8 * TC_NUM_BARS);
+    unsigned int* hist = reinterpret_cast<unsigned int*>(smem + T::OFF_HIST);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + T::OFF_BARS + 8 * TC_NUM_BARS);
 
     const int tid = threadIdx.x;
     const int warp = tid >> 5, lane = tid & 31;
     const uint32_t rank = cluster_ctarank();          // 0 = leader (issues the MMAs)
-    const uint32_t full0 = smem0 + TC_OFF_BARS, empty0 = full0 + 8 * TC_STAGES;
+    const uint32_t full0 = smem0 + T::OFF_BARS, empty0 = full0 + 8 * TC_STAGES;
     const uint32_t tmem_full = empty0 + 8 * TC_STAGES, tmem_empty = tmem_full + 8;
     const uint32_t bits_full0 = tmem_empty + 8, bits_empty0 = bits_full0 + 8 * TC_BITS_BUFS;
 
@@ -260,14 +321,23 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
     }
     if (warp == TC_MMA_WARP) {
         asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)),
-                     "n"(TC_TMEM_COLS) : "memory");
+                     "n"(T::TMEM_COLS) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
     }
     tc_fence_before();
     __syncthreads();
-    cluster_sync_all();                               // both CTAs' barriers initialised before any remote arrive
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
+    if (KIND == KIND_FP4 && warp < 4) {
+        // every block scale = 1.0: fill TMEM columns 256..511 of all 128 lanes with UE8M0 0x7F bytes
+        for (int c = 0; c < 8; ++c)
+            tmem_fill_32x32(tmem_base + ((uint32_t)(32 * warp) << 16) + 256u + 32u * c, 0x7F7F7F7Fu);
+        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+        tc_fence_before();
+    }
+    __syncthreads();
+    cluster_sync_all();                               // both CTAs' barriers and scale factors are ready
+    tc_fence_after();
 
     const int G = gridDim.x >> 1, cl = blockIdx.x >> 1;   // persistent clusters
     const int rounds = (ntiles + G - 1) / G;
@@ -289,9 +359,13 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
         int pending = -1;                             // ring stage written but not yet published
         const uint32_t row_smem = smem0 + (isA ? 0 : TC_A_BYTES) + (r >> 3) * 1024 + (r & 7) * 128;
         const int sw = r & 7;
-        // this thread's 16 bytes per group in a packed-bit buffer: 32 bytes per row, 16-byte halves swapped on
-        // odd groups of 4 rows (TMA 32-byte swizzle)
-        const uint32_t bits_row = smem0 + TC_OFF_BITS + prow * TC_BITS_ROW_BYTES + (((uint32_t)pset << 4) ^ (((prow >> 2) & 1) << 4));
+        // This thread's bytes of stage `pset` in a packed-bit buffer.  I8: 32-byte rows, TMA 32-byte swizzle
+        // (16-byte halves swapped on odd groups of 4 rows).  FP4: 64-byte rows, TMA 64-byte swizzle (16-byte
+        // chunk index ^ (row/2 mod 4)); the thread reads chunks 2*pset and 2*pset+1.
+        const uint32_t bits_row = smem0 + TC_OFF_BITS + prow * T::BITS_ROW_BYTES;
+        const uint32_t bits_c0 = KIND == KIND_FP4 ? (((2u * pset) ^ ((prow >> 1) & 3)) << 4)
+                                                  : (((uint32_t)pset ^ ((prow >> 2) & 1)) << 4);
+        const uint32_t bits_c1 = ((2u * pset + 1) ^ ((prow >> 1) & 3)) << 4;   // FP4 only
         const uint32_t full_leader0 = map_to_cta(full0, 0);
         const uint32_t tmem_empty_leader = map_to_cta(tmem_empty, 0);
 
@@ -301,7 +375,10 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
             const int2 tile = tiles[t];
             const int I = tile.x, J = tile.y;
             const long long i0 = (long long)I * TC_T, j0 = (long long)J * TC_T;
-            const int kb_begin = 2 * I, kb_end = 2 * J + 2;   // stages of 128 columns, [begin, end): always even count
+            int kb_begin, kb_end;                     // stages of COLS columns, [begin, end): even count
+            tile_k_range<COLS>(I, J, kb_begin, kb_end);
+            const int kbA = (256 * I + 255) / COLS;   // stages kb <= kbA can hold columns k <= i
+            const int kbB = (256 * J) / COLS;         // stages kb >= kbB can hold columns k >= j
 
             // Software pipeline: the fence + arrive that publishes a stage is issued after the ALU work of this
             // set's next stage (its stores have drained by then); the empty-slot barrier is probed before that work.
@@ -309,29 +386,37 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 const uint32_t stage = pset + 2 * (gc & 1), sphase = (gc >> 1) & 1;
                 const int kb = kb0 + pset;
                 mbar_wait(bits_full0 + 8 * bb, bphase);
-                uint4 w = lds128(bits_row + bb * TC_BITS_BUF_BYTES);
+                uint32_t w[WORDS];
+                {
+                    const uint4 v0 = lds128(bits_row + bb * T::BITS_BUF_BYTES + bits_c0);
+                    w[0] = v0.x; w[1] = v0.y; w[2] = v0.z; w[3] = v0.w;
+                    if (KIND == KIND_FP4) {
+                        const uint4 v1 = lds128(bits_row + bb * T::BITS_BUF_BYTES + bits_c1);
+                        w[WORDS - 4] = v1.x; w[WORDS - 3] = v1.y; w[WORDS - 2] = v1.z; w[WORDS - 1] = v1.w;
+                    }
+                }
                 __syncwarp();
-                if (lane == 0) mbar_arrive_after(bits_empty0 + 8 * bb, w.x, w.w);
+                if (lane == 0) mbar_arrive_after(bits_empty0 + 8 * bb, w[0], w[WORDS - 1]);
                 if (++bb == TC_BITS_BUFS) { bb = 0; bphase ^= 1; }
                 if (isA) {
-                    if (kb < kb_begin + 2) {                  // columns of block I: keep k > i
-                        const int rl = rt - 128 * (kb - kb_begin);
-                        w.x &= keep_gt(rl, 0); w.y &= keep_gt(rl, 1); w.z &= keep_gt(rl, 2); w.w &= keep_gt(rl, 3);
+                    if (kb <= kbA) {                          // keep k > i
+                        const int rl = 256 * I + rt - COLS * kb;
+#pragma unroll
+                        for (int m = 0; m < WORDS; ++m) w[m] &= keep_gt(rl, m);
                     }
-                } else if (kb >= kb_end - 2) {                // columns of block J: keep k < j
-                    const int lim = rt - 128 * (kb - (kb_end - 2));
-                    w.x &= keep_lt(lim, 0); w.y &= keep_lt(lim, 1); w.z &= keep_lt(lim, 2); w.w &= keep_lt(lim, 3);
+                } else if (kb >= kbB) {                       // keep k < j
+                    const int lim = 256 * J + rt - COLS * kb;
+#pragma unroll
+                    for (int m = 0; m < WORDS; ++m) w[m] &= keep_lt(lim, m);
                 }
                 const bool slot_free = mbar_try(empty0 + 8 * stage, sphase ^ 1);
                 uint4 o[8];
-                if (dbg & 1) {
+                if (KIND == KIND_FP4) {
 #pragma unroll
-                    for (int c = 0; c < 8; ++c) o[c] = w;
+                    for (int m = 0; m < 8; ++m) o[m] = unpack_word_fp4(w[m % WORDS]);
                 } else {
-                    unpack_word<TB>(w.x, o[0], o[1]);
-                    unpack_word<TB>(w.y, o[2], o[3]);
-                    unpack_word<TB>(w.z, o[4], o[5]);
-                    unpack_word<TB>(w.w, o[6], o[7]);
+#pragma unroll
+                    for (int m = 0; m < 4; ++m) unpack_word<TB>(w[m], o[2 * m], o[2 * m + 1]);
                 }
                 if (pending >= 0) {                           // publish this set's previous stage to the leader's MMA thread
                     fence_proxy_async_smem_after(o);
@@ -341,8 +426,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 if (!slot_free) mbar_wait(empty0 + 8 * stage, sphase ^ 1);
                 const uint32_t rowp = row_smem + stage * TC_STAGE_BYTES;
 #pragma unroll
-                for (int c = 0; c < 8; ++c)
-                    if (!(dbg & 4) || c == 0) sts128(rowp + ((c ^ sw) << 4), o[c]);
+                for (int c = 0; c < 8; ++c) sts128(rowp + ((c ^ sw) << 4), o[c]);
                 pending = (int)stage;
             }
             fence_proxy_async_smem();                          // publish the last stage of the tile
@@ -367,7 +451,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 else if (jc <= i) relw &= 0xFFFFFFFFu << (int)(i - jc + 1);
 #pragma unroll
                 for (int x = 0; x < 32; ++x) {
-                    const int n = (int)(v[x] >> (2 * TB));
+                    const int n = KIND == KIND_FP4 ? (int)(__uint_as_float(v[x]) * 0.25f) : (int)(v[x] >> (2 * TB));
                     if (((relw >> x) & 1u) && n <= kmax) {
                         if (n < TC_HIST) atomicAdd(&hist[n], 1u);
                         else atomicAdd(&counts[n], 1ULL);
@@ -387,7 +471,8 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 const int t = rd * G + ((rd & 1) ? (G - 1 - cl) : cl);
                 if (t >= ntiles) continue;
                 const int2 tile = tiles[t];
-                const int kb_begin = 2 * tile.x, kb_end = 2 * tile.y + 2;
+                int kb_begin, kb_end;
+                tile_k_range<COLS>(tile.x, tile.y, kb_begin, kb_end);
                 if (done_tiles > 0) {                       // both CTAs' accumulators must have been drained
                     mbar_wait(tmem_empty, ephase);
                     ephase ^= 1;
@@ -397,14 +482,17 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                     mbar_wait(full0 + 8 * stage, sphase);
                     tc_fence_after();
                     if (lane == 0) {
-                        if (!(dbg & 2)) {
-                            const uint32_t a_addr = smem0 + stage * TC_STAGE_BYTES;
-                            const uint64_t adesc = make_kmajor_sw128_desc(a_addr);
-                            const uint64_t bdesc = make_kmajor_sw128_desc(a_addr + TC_A_BYTES);
+                        const uint32_t a_addr = smem0 + stage * TC_STAGE_BYTES;
+                        const uint64_t adesc = make_kmajor_sw128_desc(a_addr);
+                        const uint64_t bdesc = make_kmajor_sw128_desc(a_addr + TC_A_BYTES);
 #pragma unroll
-                            for (int kk = 0; kk < TC_KS / 32; ++kk)   // K = 32 bytes per instruction: +2 in 16-byte units
-                                umma_i8_2cta(tmem_base, adesc + 2 * kk, bdesc + 2 * kk, TC_IDESC,
-                                             (kb > kb_begin || kk > 0) ? 1u : 0u);
+                        for (int kk = 0; kk < TC_ROW_BYTES / 32; ++kk) {   // 32 bytes of K per instruction: +2 in 16-byte units
+                            const uint32_t acc = (kb > kb_begin || kk > 0) ? 1u : 0u;
+                            if (KIND == KIND_FP4)
+                                umma_mxf4_2cta(tmem_base, adesc + 2 * kk, bdesc + 2 * kk, TC_IDESC_FP4, acc,
+                                               tmem_base + 256u, tmem_base + 384u);
+                            else
+                                umma_i8_2cta(tmem_base, adesc + 2 * kk, bdesc + 2 * kk, TC_IDESC, acc);
                         }
                         umma_commit_2cta(empty0 + 8 * stage);
                         if (kb == kb_end - 1) umma_commit_2cta(tmem_full);
@@ -424,14 +512,15 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 if (t >= ntiles) continue;
                 const int2 tile = tiles[t];
                 const int ia = tile.x * TC_T + 128 * (int)rank, jb = tile.y * TC_T + 128 * (int)rank;
-                const int kb_begin = 2 * tile.x, kb_end = 2 * tile.y + 2;
+                int kb_begin, kb_end;
+                tile_k_range<COLS>(tile.x, tile.y, kb_begin, kb_end);
                 for (int kb0 = kb_begin; kb0 < kb_end; kb0 += TC_GROUP) {
                     mbar_wait(bits_empty0 + 8 * bb, bphase ^ 1);
                     const uint32_t bar = bits_full0 + 8 * bb;
-                    const uint32_t dst = smem0 + TC_OFF_BITS + bb * TC_BITS_BUF_BYTES;
-                    mbar_expect_tx(bar, TC_BITS_BUF_BYTES);
-                    tma_load_2d(dst, &bits_map, kb0 * 16, ia, bar);
-                    tma_load_2d(dst + TC_BITS_BOX_BYTES, &bits_map, kb0 * 16, jb, bar);
+                    const uint32_t dst = smem0 + TC_OFF_BITS + bb * T::BITS_BUF_BYTES;
+                    mbar_expect_tx(bar, T::BITS_BUF_BYTES);
+                    tma_load_2d(dst, &bits_map, kb0 * (COLS / 8), ia, bar);
+                    tma_load_2d(dst + T::BITS_BOX_BYTES, &bits_map, kb0 * (COLS / 8), jb, bar);
                     if (++bb == TC_BITS_BUFS) { bb = 0; bphase ^= 1; }
                 }
             }
@@ -446,7 +535,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
     cluster_sync_all();
     tc_fence_after();
     if (warp == TC_MMA_WARP) {
-        asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(TC_TMEM_COLS)
+        asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(T::TMEM_COLS)
                      : "memory");
     }
 }

@@ -25,7 +25,7 @@ def csg():
     m.csg_set_variant(m.VARIANT_AUTO)
 
 
-VARIANTS = [1, 2]
+VARIANTS = [1, 2, 3]
 
 
 def run_action(csg, bits, N, dim, eps, kmax, variant):
