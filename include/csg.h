@@ -42,7 +42,8 @@ enum {
     CSG_E_KMAX = -6,        /* kmax < 0, kmax > CSG_MAX_KMAX, or too small for the local action */
     CSG_E_UNSUPPORTED = -7, /* smeared action in 4D (not defined by the paper) */
     CSG_E_CUDA = -8,        /* a CUDA call failed; csg_strerror(CSG_E_CUDA) carries its text */
-    CSG_E_VARIANT = -9      /* unknown variant id */
+    CSG_E_VARIANT = -9,     /* unknown variant id */
+    CSG_E_SHARD = -10       /* nshards < 1 or shard outside [0, nshards) */
 };
 
 #define CSG_MAX_N (1 << 22)
@@ -78,6 +79,32 @@ int64_t csg_row_stride_words(int64_t N);
  */
 int csg_action(const uint64_t *rel_bits, int64_t N, int dim, double eps, int kmax, int64_t *counts,
                double *S, cudaStream_t stream);
+
+/*
+ * The same path in two halves, for one causal set whose pair tiles are split over several GPUs (the paper
+ * splits the pair loop evenly over computers when the matrix fits on each, and reduces the
+ * private histograms at the end).  Every GPU holds the whole relation matrix.
+ *
+ * csg_action_partial: steps a1-a3 over the tiles of shard `shard` of `nshards` (csg_tile_schedule):
+ *   counts DEVICE, kmax+1 int64, overwritten with this shard's abundances.  The abundances of all shards
+ *   add up to those of csg_action (the caller sums them, e.g. ncclAllReduce).  0 <= shard < nshards.
+ * csg_action_finish: steps a4/a5 on summed abundances: counts DEVICE (read only), S DEVICE, 1 double;
+ *   N, dim, eps, kmax as in csg_action.  csg_action == partial(shard 0 of 1) followed by finish.
+ * Both enqueue on `stream` and do not synchronise.
+ */
+int csg_action_partial(const uint64_t *rel_bits, int64_t N, int kmax, int shard, int nshards, int64_t *counts,
+                       cudaStream_t stream);
+int csg_action_finish(const int64_t *counts, int64_t N, int dim, double eps, int kmax, double *S,
+                      cudaStream_t stream);
+
+/*
+ * Host logic, no device needed: the pair tiles (I, J), I <= J, in 256-row blocks, that shard `shard` of
+ * `nshards` visits, in launch order (deepest K-range first; for matrices larger than L2 grouped in patches of
+ * 8 x 9 blocks so that concurrently running tiles share rows in L2).  tiles_ij HOST, 2*capacity int32
+ * (I0, J0, I1, J1, ...), may be NULL; returns the number of tiles of the shard (or a negative CSG_E_* code);
+ * at most `capacity` tiles are written.  The shards of one N partition the upper triangle exactly.
+ */
+int64_t csg_tile_schedule(int64_t N, int shard, int nshards, int32_t *tiles_ij, int64_t capacity);
 
 /*
  * Same computation with HOST buffers (the end-to-end call): copies rel_bits to the device (pinned or

@@ -6,7 +6,7 @@ There is no CPU fallback: if libcsg.so is missing, importing the compute entry p
 
 Functions carry the C names: csg_action, csg_action_host, csg_interval_sizes, csg_row_stride_words,
 csg_set_variant, csg_effective_variant, csg_set_kernel_timing, csg_last_kernel_ms, csg_kernel_ms_history,
-csg_launch_count,
+csg_launch_count, csg_action_partial, csg_action_finish, csg_tile_schedule,
 csg_strerror, csg_shutdown.
 """
 import ctypes
@@ -22,7 +22,7 @@ LIB_PATH = _build.LIB_PATH
 EXPORTS = [
     "csg_row_stride_words", "csg_action", "csg_action_host", "csg_interval_sizes", "csg_set_variant",
     "csg_effective_variant", "csg_set_kernel_timing", "csg_last_kernel_ms", "csg_kernel_ms_history",
-    "csg_launch_count",
+    "csg_launch_count", "csg_action_partial", "csg_action_finish", "csg_tile_schedule",
     "csg_strerror", "csg_shutdown",
 ]
 
@@ -56,6 +56,12 @@ def load():
     lib.csg_action.restype = ci
     lib.csg_action_host.argtypes = [vp, i64, ci, dbl, ci, vp, vp]
     lib.csg_action_host.restype = ci
+    lib.csg_action_partial.argtypes = [vp, i64, ci, ci, ci, vp, vp]
+    lib.csg_action_partial.restype = ci
+    lib.csg_action_finish.argtypes = [vp, i64, ci, dbl, ci, vp, vp]
+    lib.csg_action_finish.restype = ci
+    lib.csg_tile_schedule.argtypes = [i64, ci, ci, vp, i64]
+    lib.csg_tile_schedule.restype = i64
     lib.csg_interval_sizes.argtypes = [vp, i64, vp, i64, vp, vp]
     lib.csg_interval_sizes.restype = ci
     lib.csg_set_variant.argtypes = [ci]
@@ -122,6 +128,46 @@ def csg_action(rel_bits, N, dim, eps, kmax, counts=None, S=None, stream=None):
     _check(lib.csg_action(rel_bits.data_ptr(), int(N), int(dim), float(eps), int(kmax), counts.data_ptr(),
                           S.data_ptr(), _stream_handle(stream)))
     return counts, S
+
+
+def csg_action_partial(rel_bits, N, kmax, shard, nshards, counts=None, stream=None):
+    """int csg_action_partial(rel_bits, N, kmax, shard, nshards, counts, stream): abundances of one shard of the
+    pair tiles (device tensors; nothing is synchronised).  Returns counts."""
+    import torch
+    lib = load()
+    assert rel_bits.is_cuda and rel_bits.element_size() == 8 and rel_bits.is_contiguous()
+    assert rel_bits.numel() >= int(N) * csg_row_stride_words(N)
+    if counts is None:
+        counts = torch.empty(max(int(kmax), 0) + 1, dtype=torch.int64, device=rel_bits.device)
+    _check(lib.csg_action_partial(rel_bits.data_ptr(), int(N), int(kmax), int(shard), int(nshards), counts.data_ptr(),
+                                  _stream_handle(stream)))
+    return counts
+
+
+def csg_action_finish(counts, N, dim, eps, kmax, S=None, stream=None):
+    """int csg_action_finish(counts, N, dim, eps, kmax, S, stream): summed abundances -> action.  Returns S."""
+    import torch
+    lib = load()
+    assert counts.is_cuda and counts.dtype == torch.int64 and counts.numel() >= int(kmax) + 1
+    if S is None:
+        S = torch.empty(1, dtype=torch.float64, device=counts.device)
+    _check(lib.csg_action_finish(counts.data_ptr(), int(N), int(dim), float(eps), int(kmax), S.data_ptr(),
+                                 _stream_handle(stream)))
+    return S
+
+
+def csg_tile_schedule(N, shard=0, nshards=1):
+    """int64 csg_tile_schedule(N, shard, nshards, tiles_ij, capacity): host logic, needs no device.
+    Returns an (ntiles, 2) int32 numpy array of (I, J) block pairs in launch order."""
+    lib = load()
+    n = int(lib.csg_tile_schedule(int(N), int(shard), int(nshards), None, 0))
+    if n < 0:
+        _check(n)
+    out = np.empty((n, 2), dtype=np.int32)
+    if n:
+        got = int(lib.csg_tile_schedule(int(N), int(shard), int(nshards), out.ctypes.data, n))
+        assert got == n
+    return out
 
 
 def csg_action_host(rel_bits, N, dim, eps, kmax):

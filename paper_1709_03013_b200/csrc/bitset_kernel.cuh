@@ -46,7 +46,8 @@ __device__ __forceinline__ void bitset_tile_from_index(long long t, long long nb
 
 __global__ void __launch_bounds__(BS_THREADS, 2)
 bitset_action_kernel(const uint32_t* __restrict__ rel, long long N, long long stride32, int kmax,
-                     unsigned long long* __restrict__ counts, long long nb, long long ntiles) {
+                     unsigned long long* __restrict__ counts, long long nb, long long ntiles, int shard,
+                     int nshards) {
     __shared__ __align__(16) uint32_t sA[BS_T * BS_LD];
     __shared__ __align__(16) uint32_t sB[BS_T * BS_LD];
     __shared__ unsigned int hist[BS_HIST];
@@ -56,7 +57,8 @@ bitset_action_kernel(const uint32_t* __restrict__ rel, long long N, long long st
     for (int b = tid; b < BS_HIST; b += BS_THREADS) hist[b] = 0u;
     __syncthreads();
 
-    for (long long t = blockIdx.x; t < ntiles; t += gridDim.x) {
+    // this launch owns the tiles t = shard (mod nshards) of the depth-sorted enumeration
+    for (long long t = shard + (long long)blockIdx.x * nshards; t < ntiles; t += (long long)gridDim.x * nshards) {
         long long I, J;
         bitset_tile_from_index(t, nb, I, J);
         const long long i0 = I * BS_T, j0 = J * BS_T;

@@ -83,6 +83,7 @@ struct State {
     char cuda_msg[256] = "no CUDA error recorded";
     // cached tile schedule of the tensor variant
     long long tiles_N = -1;
+    int tiles_shard = 0, tiles_nshards = 1;
     int2* d_tiles = nullptr;
     int ntiles = 0;
     std::vector<int2> h_tiles;
@@ -134,14 +135,62 @@ static int effective_variant(long long N) {
     return N >= 2048 ? CSG_VARIANT_TENSOR_FP4 : CSG_VARIANT_BITSET;
 }
 
-// Tiles (I, J) of the tensor variant in 256-row blocks, I <= J; K-depth in 128-column stages = 2(J-I)+2.
-// Sorted longest first.
-static int ensure_tiles(long long N, cudaStream_t stream) {
-    if (g.tiles_N == N && g.d_tiles) return CSG_OK;
+// Tile schedule of the tensor variant (pure host logic; exported as csg_tile_schedule).  Tiles (I, J) in
+// 256-row blocks, I <= J; the K-depth of a tile is J-I+1 blocks, so the upper triangle is a triangular workload.
+//   * matrix within L2 (<= TILE_L2_BYTES): tiles sorted by depth, longest first; shard s takes every nshards-th.
+//   * larger: tiles grouped in patches of PATCH_H x PATCH_W blocks (about one tile per persistent cluster), patches
+//     sorted by their deepest tile, tiles inside a patch by depth.  The clusters of one round then stream the same
+//     PATCH_H + PATCH_W row blocks at about the same K, so each row segment comes from HBM once per patch and from
+//     L2 for the other tiles of the patch; whole patches are dealt to the shards, least-loaded shard first.
+// Longest first keeps the tail short; the kernel deals consecutive tiles boustrophedon to its persistent clusters.
+constexpr long long TILE_L2_BYTES = 48LL << 20;
+constexpr int PATCH_H = 8, PATCH_W = 9;
+
+static void build_tile_schedule(long long N, int shard, int nshards, std::vector<int2>& out) {
+    out.clear();
     const int nB = (int)((N + TC_T - 1) / TC_T);
-    g.h_tiles.clear();
-    for (int d = nB - 1; d >= 0; --d)
-        for (int I = 0; I + d < nB; ++I) g.h_tiles.push_back(make_int2(I, I + d));
+    const long long bytes = N * (long long)(4 * ((N + 255) / 256)) * 8;
+    if (bytes <= TILE_L2_BYTES) {
+        long long t = 0;
+        for (int d = nB - 1; d >= 0; --d)
+            for (int I = 0; I + d < nB; ++I, ++t)
+                if (t % nshards == shard) out.push_back(make_int2(I, I + d));
+        return;
+    }
+    struct Patch { int depth, p, q; };
+    std::vector<Patch> patches;
+    const int nP = (nB + PATCH_H - 1) / PATCH_H, nQ = (nB + PATCH_W - 1) / PATCH_W;
+    for (int p = 0; p < nP; ++p)
+        for (int q = 0; q < nQ; ++q) {
+            const int Ilo = p * PATCH_H, Jhi = std::min(nB, (q + 1) * PATCH_W) - 1;
+            if (Jhi >= Ilo) patches.push_back({Jhi - Ilo, p, q});
+        }
+    std::stable_sort(patches.begin(), patches.end(), [](const Patch& a, const Patch& b) { return a.depth > b.depth; });
+    // patches go, deepest first, to the shard with the least work so far (work = sum of K-depths; every rank
+    // computes the same assignment)
+    std::vector<long long> load(nshards, 0);
+    std::vector<int2> in_patch;
+    for (size_t k = 0; k < patches.size(); ++k) {
+        const Patch& pt = patches[k];
+        in_patch.clear();
+        long long work = 0;
+        for (int I = pt.p * PATCH_H; I < std::min(nB, (pt.p + 1) * PATCH_H); ++I)
+            for (int J = std::max(I, pt.q * PATCH_W); J < std::min(nB, (pt.q + 1) * PATCH_W); ++J) {
+                in_patch.push_back(make_int2(I, J));
+                work += J - I + 1;
+            }
+        const int owner = (int)(std::min_element(load.begin(), load.end()) - load.begin());
+        load[owner] += work;
+        if (owner != shard) continue;
+        std::stable_sort(in_patch.begin(), in_patch.end(),
+                         [](const int2& a, const int2& b) { return a.y - a.x > b.y - b.x; });
+        out.insert(out.end(), in_patch.begin(), in_patch.end());
+    }
+}
+
+static int ensure_tiles(long long N, int shard, int nshards, cudaStream_t stream) {
+    if (g.tiles_N == N && g.tiles_shard == shard && g.tiles_nshards == nshards && g.d_tiles) return CSG_OK;
+    build_tile_schedule(N, shard, nshards, g.h_tiles);
     if (g.d_tiles) {
         CSG_CUDA(cudaStreamSynchronize(stream));
         CSG_CUDA(cudaFree(g.d_tiles));
@@ -152,6 +201,8 @@ static int ensure_tiles(long long N, cudaStream_t stream) {
     CSG_CUDA(cudaMemcpyAsync(g.d_tiles, g.h_tiles.data(), g.h_tiles.size() * sizeof(int2), cudaMemcpyHostToDevice,
                              stream));
     g.tiles_N = N;
+    g.tiles_shard = shard;
+    g.tiles_nshards = nshards;
     return CSG_OK;
 }
 
@@ -204,8 +255,9 @@ static int validate(const void* rel_bits, long long N, int dim, double eps, int 
     return CSG_OK;
 }
 
-static int action_device(const uint64_t* rel_bits, long long N, int dim, double eps, int kmax, long long* counts,
-                         double* S, cudaStream_t stream) {
+// Interval kernel over the tiles of one shard: counts (kmax+1 int64, overwritten) <- this shard's abundances.
+static int interval_device(const uint64_t* rel_bits, long long N, int kmax, int shard, int nshards,
+                           long long* counts, cudaStream_t stream) {
     int rc = ensure_device();
     if (rc) return rc;
     const long long stride = csg_row_stride_words(N);
@@ -214,7 +266,7 @@ static int action_device(const uint64_t* rel_bits, long long N, int dim, double 
     const bool tensor = variant == CSG_VARIANT_TENSOR || variant == CSG_VARIANT_TENSOR_FP4;
     const int kind = variant == CSG_VARIANT_TENSOR_FP4 ? KIND_FP4 : KIND_I8;
     if (tensor) {
-        rc = ensure_tiles(N, stream);
+        rc = ensure_tiles(N, shard, nshards, stream);
         if (rc) return rc;
         rc = ensure_bits_map(kind, rel_bits, N, stride);
         if (rc) return rc;
@@ -257,11 +309,12 @@ static int action_device(const uint64_t* rel_bits, long long N, int dim, double 
     } else {
         const long long nb = (N + BS_T - 1) / BS_T;
         const long long ntiles = nb * (nb + 1) / 2;
-        const int grid = (int)std::max<long long>(1, std::min<long long>(ntiles, (long long)g.sm_count * 2));
+        const long long mine = (ntiles - shard + nshards - 1) / nshards;   // tiles t = shard (mod nshards)
+        const int grid = (int)std::max<long long>(1, std::min<long long>(mine, (long long)g.sm_count * 2));
         bitset_action_kernel<<<grid, BS_THREADS, 0, stream>>>(reinterpret_cast<const uint32_t*>(rel_bits), N,
                                                                stride * 2, kmax,
                                                                reinterpret_cast<unsigned long long*>(counts), nb,
-                                                               ntiles);
+                                                               ntiles, shard, nshards);
     }
     CSG_CUDA(cudaGetLastError());
     ++g.launches;
@@ -269,10 +322,24 @@ static int action_device(const uint64_t* rel_bits, long long N, int dim, double 
         CSG_CUDA(cudaEventRecord(g.ev1[slot], stream));
         ++g.timed_calls;
     }
+    return CSG_OK;
+}
+
+static int finish_device(const long long* counts, long long N, int dim, double eps, int kmax, double* S,
+                         cudaStream_t stream) {
+    int rc = ensure_device();
+    if (rc) return rc;
     finish_action_kernel<<<1, FIN_THREADS, 0, stream>>>(counts, N, dim, eps, kmax, S);
     CSG_CUDA(cudaGetLastError());
     ++g.launches;
     return CSG_OK;
+}
+
+static int action_device(const uint64_t* rel_bits, long long N, int dim, double eps, int kmax, long long* counts,
+                         double* S, cudaStream_t stream) {
+    int rc = interval_device(rel_bits, N, kmax, 0, 1, counts, stream);
+    if (rc) return rc;
+    return finish_device(counts, N, dim, eps, kmax, S, stream);
 }
 
 }  // namespace csg
@@ -292,6 +359,39 @@ int csg_action(const uint64_t* rel_bits, int64_t N, int dim, double eps, int kma
         (reinterpret_cast<uintptr_t>(S) & 7))
         return CSG_E_ALIGN;
     return action_device(rel_bits, N, dim, eps, kmax, reinterpret_cast<long long*>(counts), S, stream);
+}
+
+int csg_action_partial(const uint64_t* rel_bits, int64_t N, int kmax, int shard, int nshards, int64_t* counts,
+                       cudaStream_t stream) {
+    std::lock_guard<std::mutex> lock(g.mu);
+    if (!rel_bits || !counts) return CSG_E_NULL;
+    if (N < 1 || N > CSG_MAX_N) return CSG_E_SIZE;
+    if (kmax < 0 || kmax > CSG_MAX_KMAX) return CSG_E_KMAX;
+    if (nshards < 1 || shard < 0 || shard >= nshards) return CSG_E_SHARD;
+    if ((reinterpret_cast<uintptr_t>(rel_bits) & 15) || (reinterpret_cast<uintptr_t>(counts) & 7)) return CSG_E_ALIGN;
+    return interval_device(rel_bits, N, kmax, shard, nshards, reinterpret_cast<long long*>(counts), stream);
+}
+
+int csg_action_finish(const int64_t* counts, int64_t N, int dim, double eps, int kmax, double* S,
+                      cudaStream_t stream) {
+    std::lock_guard<std::mutex> lock(g.mu);
+    int rc = validate(counts, N, dim, eps, kmax, counts, S);
+    if (rc) return rc;
+    if ((reinterpret_cast<uintptr_t>(counts) & 7) || (reinterpret_cast<uintptr_t>(S) & 7)) return CSG_E_ALIGN;
+    return finish_device(reinterpret_cast<const long long*>(counts), N, dim, eps, kmax, S, stream);
+}
+
+int64_t csg_tile_schedule(int64_t N, int shard, int nshards, int32_t* tiles_ij, int64_t capacity) {
+    if (N < 1 || N > CSG_MAX_N) return CSG_E_SIZE;
+    if (nshards < 1 || shard < 0 || shard >= nshards) return CSG_E_SHARD;
+    std::vector<int2> tiles;
+    build_tile_schedule(N, shard, nshards, tiles);
+    if (tiles_ij)
+        for (int64_t t = 0; t < (int64_t)tiles.size() && t < capacity; ++t) {
+            tiles_ij[2 * t] = tiles[t].x;
+            tiles_ij[2 * t + 1] = tiles[t].y;
+        }
+    return (int64_t)tiles.size();
 }
 
 int csg_action_host(const uint64_t* rel_bits_host, int64_t N, int dim, double eps, int kmax, int64_t* counts_host,
@@ -410,6 +510,7 @@ const char* csg_strerror(int code) {
         case CSG_E_UNSUPPORTED: return "smeared action is defined for dim 2 only";
         case CSG_E_CUDA: return g.cuda_msg;
         case CSG_E_VARIANT: return "unknown variant";
+        case CSG_E_SHARD: return "shard must satisfy 0 <= shard < nshards";
         default: return "unknown error code";
     }
 }

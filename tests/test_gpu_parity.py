@@ -124,6 +124,29 @@ def test_host_entry_point(csg):
     assert (counts2 == want).all() and S2 == S
 
 
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("dim,N,eps,nshards", [(4, 2600, 1.0, 2), (2, 1900, 0.25, 3), (2, 300, 1.0, 8)])
+def test_tile_shards_sum_to_the_whole(csg, variant, dim, N, eps, nshards):
+    """csg_action_partial over every shard, summed (what the all-reduce does), then csg_action_finish ==
+    csg_action == oracle."""
+    _, bits = csg_inputs.make_causet(dim, N, 70 + N)
+    kmax = N - 2
+    want = reference_counts(bits, N, kmax)
+    d = csg.to_device(bits)
+    csg.csg_set_variant(variant)
+    total = torch.zeros(kmax + 1, dtype=torch.int64, device="cuda")
+    for s in range(nshards):
+        total += csg.csg_action_partial(d, N, kmax, s, nshards)
+    S = csg.csg_action_finish(total, N, dim, eps, kmax)
+    whole, S_whole = csg.csg_action(d, N, dim, eps, kmax)
+    torch.cuda.synchronize()
+    assert (total.cpu().numpy() == want).all()
+    assert (whole.cpu().numpy() == want).all()
+    assert float(S.item()) == float(S_whole.item())
+    if eps == 1.0:
+        assert float(S.item()) == oracle.action_local(dim, N, want)
+
+
 def test_interval_sizes_hook(csg):
     N = 3000
     _, bits = csg_inputs.make_causet(4, N, 11)
@@ -186,6 +209,10 @@ def check_config(csg, cfg, full_reference):
     nrel, chains = degree_invariants(bits, N)
     assert full.sum() == nrel                                         # I1
     assert int((np.arange(N - 1, dtype=object) * full.astype(object)).sum()) == chains   # I2 = I3
+    # (2b) the tile shards of the multi-GPU path (patch schedule at these sizes) add up to the same histogram
+    parts = sum(csg.csg_action_partial(d, N, cfg["kmax"], s, 3) for s in range(3))
+    torch.cuda.synchronize()
+    assert (parts.cpu().numpy() == counts).all()
     # (3) sampled outputs the oracle computes one by one
     rng = np.random.default_rng(cfg["seed"])
     pairs = np.sort(rng.integers(0, N, size=(300, 2)), axis=1).astype(np.int64)

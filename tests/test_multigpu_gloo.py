@@ -1,0 +1,121 @@
+"""The N>1 path on CPU: two processes, gloo.  Host logic only (tile shards, the all-reduce of the private
+histograms, ensemble seeds, max-over-ranks timing); the per-shard abundances that the GPU kernel would
+produce are computed here by the oracle's definition restricted to the shard's tiles."""
+import os
+import socket
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+torch = pytest.importorskip("torch")
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    return port
+
+
+def _shard_counts_by_definition(B, tiles, kmax):
+    """counts of the related pairs (i, j) of the listed 256 x 256 tiles, n_ij = sum_{i<k<j} B[i][k] B[j][k]
+    (PAPER.md:395), through the strictly-upper-triangular integer matrix square."""
+    N = B.shape[0]
+    U = np.triu(B.astype(np.int64), 1)
+    C = U @ U
+    counts = np.zeros(kmax + 1, np.int64)
+    for I, J in tiles:
+        i0, j0 = 256 * int(I), 256 * int(J)
+        for i in range(i0, min(N, i0 + 256)):
+            js = np.arange(max(j0, i + 1), min(N, j0 + 256))
+            js = js[U[i, js] == 1]
+            n = C[i, js]
+            counts += np.bincount(n[n <= kmax], minlength=kmax + 1)[:kmax + 1]
+    return counts
+
+
+def _worker(rank, world, port, N, q):
+    sys.path.insert(0, ROOT)
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    import torch.distributed as dist
+    import csg_inputs
+    import oracle
+    import paper_1709_03013_b200 as csg
+    from paper_1709_03013_b200 import multigpu
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        # --- tiles mode: same causal set on every rank, tiles split, histograms summed
+        _, bits = csg_inputs.make_causet(2, N, 4242)
+        B = oracle.expand(bits, N)
+        kmax = N - 2
+        tiles = csg.csg_tile_schedule(N, rank, world)
+        part = torch.from_numpy(_shard_counts_by_definition(B, tiles, kmax))
+        total = multigpu.allreduce_counts(part.clone())
+        want = oracle.counts_from_bits(bits, N, kmax)
+        ok_tiles = bool((total.numpy() == want).all()) and int(part.sum()) < int(want.sum())
+        # --- ensemble mode: different causal set per rank, timings reduced with max
+        seed = multigpu.ensemble_seed(csg_inputs.CONFIGS[0]["seed"], rank)
+        _, mine = csg_inputs.make_causet(2, 256, seed)
+        h = torch.tensor([int(np.bitwise_xor.reduce(mine.ravel()) >> np.uint64(1))], dtype=torch.int64)
+        hs = [torch.zeros_like(h) for _ in range(world)]
+        dist.all_gather(hs, h)
+        ms = multigpu.max_over_ranks([10.0 + rank, 5.0 - rank])
+        q.put((rank, ok_tiles, len(tiles), [int(x) for x in hs], ms))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.timeout(300)
+def test_two_ranks_gloo_tiles_and_ensemble():
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    world, N, port = 2, 1500, _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, world, port, N, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=240) for _ in range(world))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    nB = (N + 255) // 256
+    assert sum(r[2] for r in res) == nB * (nB + 1) // 2
+    for rank, ok_tiles, _, hashes, ms in res:
+        assert ok_tiles, "summed shard histograms differ from the oracle"
+        assert len(set(hashes)) == world, "ensemble ranks must own different causal sets"
+        assert ms == [11.0, 5.0]
+
+
+@pytest.mark.parametrize("N", [1, 255, 257, 5000, 16384, 40000, 131072, 262144])
+@pytest.mark.parametrize("nshards", [1, 2, 3, 8])
+def test_tile_shards_partition_the_upper_triangle(N, nshards):
+    import paper_1709_03013_b200 as csg
+    nB = (N + 255) // 256
+    seen = np.zeros((nB, nB), np.int32)
+    sizes = []
+    for s in range(nshards):
+        t = csg.csg_tile_schedule(N, s, nshards)
+        assert (t[:, 0] <= t[:, 1]).all() and (t >= 0).all() and (t < nB).all()
+        np.add.at(seen, (t[:, 0], t[:, 1]), 1)
+        sizes.append(int((t[:, 1] - t[:, 0] + 1).sum()))          # K-depth in blocks = the shard's work
+    assert (seen == np.triu(np.ones((nB, nB), np.int32))).all()
+    if nB >= 64:                                                    # shards carry the same work to within 3 %
+        assert max(sizes) <= 1.03 * (sum(sizes) / nshards)
+    # longest first: the tail of every schedule is shallow
+    t = csg.csg_tile_schedule(N, 0, nshards)
+    if len(t) > 200:
+        d = t[:, 1] - t[:, 0]
+        assert d[-20:].max() <= 20 and d[:20].min() >= d.max() - 20
+
+
+def test_multigpu_rate_helpers():
+    from paper_1709_03013_b200 import multigpu
+    assert multigpu.ensemble_seed(7, 3) == 3007
+    assert multigpu.whole_job_rate(2 * 10.0, 5, 1000.0) == 100.0
+    c = torch.arange(4, dtype=torch.int64)
+    assert multigpu.allreduce_counts(c) is c                         # no process group: identity
+    assert multigpu.max_over_ranks([1.5, 2.5]) == [1.5, 2.5]
