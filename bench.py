@@ -193,6 +193,7 @@ def run_ours(args, cfg, rank, local_rank, world):
     import torch
     import csg_inputs
     import paper_1709_03013_b200 as csg
+    from paper_1709_03013_b200 import multigpu
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; libcsg has no CPU fallback")
@@ -211,7 +212,8 @@ def run_ours(args, cfg, rank, local_rank, world):
     csg.csg_set_variant(args.variant)
 
     N, dim, eps, kmax = cfg["N"], cfg["dim"], cfg["eps"], cfg["kmax"]
-    seed = cfg["seed"] + 1000 * rank
+    tiles_mode = args.shard == "tiles" and world > 1
+    seed = cfg["seed"] if tiles_mode else multigpu.ensemble_seed(cfg["seed"], rank)
     t0 = time.perf_counter()
     _, bits = csg_inputs.make_causet(dim, N, seed)
     gen_s = time.perf_counter() - t0
@@ -229,7 +231,10 @@ def run_ours(args, cfg, rank, local_rank, world):
         torch.cuda.synchronize()
 
     def step():
-        csg.csg_action(d_bits, N, dim, eps, kmax, counts, S)
+        if tiles_mode:      # one causal set, tiles split over the ranks, one all-reduce of the abundances
+            multigpu.csg_action_sharded(d_bits, N, dim, eps, kmax, counts, S)
+        else:               # one causal set per rank
+            csg.csg_action(d_bits, N, dim, eps, kmax, counts, S)
 
     # ---- device-resident leg
     csg.csg_set_kernel_timing(True)
@@ -265,10 +270,7 @@ def run_ours(args, cfg, rank, local_rank, world):
     e2e_s = time.perf_counter() - t0
     assert (c_host == result_counts).all() and S_host == result_S, "e2e and device legs disagree"
 
-    t = torch.tensor([ms_total, 1e3 * e2e_s], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_total, e2e_ms = float(t[0]), float(t[1])
+    ms_total, e2e_ms = multigpu.max_over_ranks([ms_total, 1e3 * e2e_s], device="cuda")
 
     if rank != 0:
         if dist is not None:
@@ -276,15 +278,17 @@ def run_ours(args, cfg, rank, local_rank, world):
         return 0
 
     triples = comb3(N)
-    value = world * triples * args.steps / (ms_total * 1e-3)
-    e2e_value = world * triples * e2e_steps / (e2e_ms * 1e-3)
+    sets = 1 if tiles_mode else world           # causal sets the whole job finishes per step
+    value = multigpu.whole_job_rate(sets * triples, args.steps, ms_total)
+    e2e_value = multigpu.whole_job_rate(world * triples, e2e_steps, e2e_ms)   # the host-buffer call is per rank
     k_ms = sum(kernel_ms) / len(kernel_ms)
+    kernel_triples = triples / world if tiles_mode else triples     # what one launch of rank 0 covers
     peaks = read_peaks()
     if variant in (csg.VARIANT_TENSOR, csg.VARIANT_TENSOR_FP4):
         # dense binary contraction on tcgen05: 1 triple test = 1 MAC = 2 ops.  peak = measured bf16 dense peak x the
         # nominal ratio of the operand type on B200 (B200_PROFILING.md table: int8/fp8 2x, fp4 4x bf16).
         ratio = 4.0 if variant == csg.VARIANT_TENSOR_FP4 else 2.0
-        achieved = 2.0 * triples / (k_ms * 1e-3) / 1e12
+        achieved = 2.0 * kernel_triples / (k_ms * 1e-3) / 1e12
         roofline = {"bound": "tensor", "kernel": kernel_name, "achieved": achieved, "peak": ratio * peaks["bf16"],
                     "unit": "TOP/s (%s)" % ("fp4 e2m1, kind::mxf4" if ratio == 4.0 else "int8, kind::i8"),
                     "frac": achieved / (ratio * peaks["bf16"]),
@@ -295,7 +299,7 @@ def run_ours(args, cfg, rank, local_rank, world):
     else:
         # LOP3+POPC+IADD per 32 triple tests; POPC pipe 16 lanes/clk/SM x 148 SMs x 1.965 GHz
         peak = 16 * 148 * 1.965e9 * 32 / 1e12
-        achieved = triples / (k_ms * 1e-3) / 1e12
+        achieved = kernel_triples / (k_ms * 1e-3) / 1e12
         roofline = {"bound": "alu", "kernel": kernel_name, "achieved": achieved, "peak": peak,
                     "unit": "T bit-tests/s", "frac": achieved / peak, "peak_source": "derived: POPC 16/clk/SM",
                     "kernel_ms": k_ms, "traffic": read_traffic(kernel_name)}
@@ -316,7 +320,7 @@ def run_ours(args, cfg, rank, local_rank, world):
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "strong" if tiles_mode else "weak", "vs_baseline": None,
         "dtype": {csg.VARIANT_TENSOR: "u8 x u8 -> s32 (tcgen05 kind::i8)",
                   csg.VARIANT_TENSOR_FP4: "e2m1 x e2m1 -> f32, exact integers (tcgen05 kind::mxf4, unit scales)",
                   csg.VARIANT_BITSET: "u32 and/popc"}[variant],
@@ -326,7 +330,8 @@ def run_ours(args, cfg, rank, local_rank, world):
                    "l2": "input (%.0f MiB) %s L2 (126 MB)" % (N * csg.csg_row_stride_words(N) * 8 / 2**20,
                                                             "larger than" if N * csg.csg_row_stride_words(N) * 8 > 126e6
                                                             else "fits in"),
-                   "parallelism": "1 causal set per GPU, no collectives", "host_generation_s": gen_s},
+                   "parallelism": ("1 causal set, tiles sharded over %d GPUs, one int64 all-reduce" % world) if tiles_mode
+                   else "1 causal set per GPU, no collectives", "host_generation_s": gen_s},
         "action_time_s": ms_total / args.steps * 1e-3,
         "kernel_ms_per_step": kernel_ms,
         "result": {"counts_head": [int(x) for x in result_counts[:4]], "S": result_S},
@@ -353,6 +358,8 @@ def main():
     ap.add_argument("--config", type=int, default=3, help="index into BASELINE.json configs (default 3, the headline)")
     ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 bitset, 2 tensor int8, 3 tensor fp4")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--shard", default="ensemble", choices=["ensemble", "tiles"],
+                    help="N>1 GPUs: one causal set per rank (weak scaling, default) or one set with its tiles split")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
