@@ -12,6 +12,9 @@ from .generate import (  # noqa: F401
     sprinkle,
     relations_from_coords,
     make_causet,
+    sprinkle_de_sitter,
+    relations_de_sitter,
+    make_de_sitter,
     pack_dense,
     bits_hash,
     random_poset_bits,

@@ -11,10 +11,14 @@
  *   - 4D: rejection sampling of (t,x,y,z), t in [0,1), x,y,z in [-1/2,1/2), accept iff
  *     x^2+y^2+z^2 < min(t,1-t)^2 (Alexandrov interval of height 1); related iff dt>0 and
  *     dt*dt > dx*dx+dy*dy+dz*dz (strict, doubles, no sqrt); sorted by (t, draw index).
+ *   - (1+1) de Sitter slab, the paper's own workload: eta = atan(tan(eta0) (2a-1)) with a
+ *     uniform (inverse CDF of rho(eta|eta0) = sec^2 eta / tan eta0 ... normalised on [-eta0, eta0]), theta =
+ *     2 pi b; related iff pi - |pi - |dtheta|| < |deta|; sorted by (eta, draw index).
  *   - Output: symmetric packed matrix, zero diagonal, zero padding, LSB-first 64-bit words,
  *     row stride = 4*ceil(N/256) words (rows 256-bit aligned as PAPER.md:169).
  * Compile without -ffast-math / FMA contraction (-ffp-contract=off) so comparisons are reproducible.
  */
+#include <math.h>
 #include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
@@ -93,6 +97,28 @@ int csg_gen_coords_4d(uint64_t seed, int64_t N, double *coords)
     return 0;
 }
 
+/* coords: N x 2 doubles (eta, theta), written in sorted (conformal time) order. */
+int csg_gen_coords_ds2(uint64_t seed, int64_t N, double eta0, double *coords)
+{
+    sort_item *it = (sort_item *)malloc((size_t)(N > 0 ? N : 1) * sizeof(sort_item));
+    double *raw = (double *)malloc((size_t)(N > 0 ? N : 1) * 2 * sizeof(double));
+    if (!it || !raw) { free(it); free(raw); return -1; }
+    const double T = tan(eta0);
+    for (int64_t n = 0; n < N; ++n) {
+        double a = uniform01(seed, 2 * (uint64_t)n), b = uniform01(seed, 2 * (uint64_t)n + 1);
+        raw[2 * n] = atan(T * (2.0 * a - 1.0));
+        raw[2 * n + 1] = 6.28318530717958647692 * b;
+        it[n].key = raw[2 * n]; it[n].key2 = 0.0; it[n].idx = n;
+    }
+    qsort(it, (size_t)N, sizeof(sort_item), cmp_item);
+    for (int64_t n = 0; n < N; ++n) {
+        coords[2 * n] = raw[2 * it[n].idx];
+        coords[2 * n + 1] = raw[2 * it[n].idx + 1];
+    }
+    free(it); free(raw);
+    return 0;
+}
+
 /* In-place transpose of a 64x64 bit block held as 64 words (row r = a[r], column c = bit c). */
 static void transpose64(uint64_t a[64])
 {
@@ -167,6 +193,25 @@ int csg_gen_relations_4d(const double *coords, int64_t N, uint64_t *bits)
             double s2 = dx * dx + dy * dy;
             s2 = s2 + dz * dz;
             if (dt > 0.0 && dt * dt > s2)
+                row[j >> 6] |= 1ULL << (j & 63);
+        }
+    }
+    mirror_lower(bits, N, stride);
+    return 0;
+}
+
+int csg_gen_relations_ds2(const double *coords, int64_t N, uint64_t *bits)
+{
+    int64_t stride = csg_gen_stride_words(N);
+    const double PI = 3.14159265358979323846;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t i = 0; i < N; ++i) {
+        double ei = coords[2 * i], ti = coords[2 * i + 1];
+        uint64_t *row = bits + i * stride;
+        for (int64_t j = i + 1; j < N; ++j) {
+            double dth = fabs(ti - coords[2 * j + 1]);
+            double lhs = PI - fabs(PI - dth);
+            if (lhs < fabs(ei - coords[2 * j]))
                 row[j >> 6] |= 1ULL << (j & 63);
         }
     }

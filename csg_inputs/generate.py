@@ -27,7 +27,7 @@ _p_u64 = np.ctypeslib.ndpointer(dtype=np.uint64, flags="C_CONTIGUOUS")
 def build(force=False):
     if not force and os.path.exists(_LIB_PATH) and os.path.getmtime(_LIB_PATH) >= os.path.getmtime(_SRC):
         return _LIB_PATH
-    cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-ffp-contract=off", "-fPIC", "-shared", "-o", _LIB_PATH, _SRC]
+    cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-ffp-contract=off", "-fPIC", "-shared", "-o", _LIB_PATH, _SRC, "-lm"]
     subprocess.run(cmd, check=True)
     return _LIB_PATH
 
@@ -47,6 +47,10 @@ def _load():
             f = getattr(lib, name)
             f.argtypes = [_p_f64, ctypes.c_int64, _p_u64]
             f.restype = ctypes.c_int
+        lib.csg_gen_coords_ds2.argtypes = [ctypes.c_uint64, ctypes.c_int64, ctypes.c_double, _p_f64]
+        lib.csg_gen_coords_ds2.restype = ctypes.c_int
+        lib.csg_gen_relations_ds2.argtypes = [_p_f64, ctypes.c_int64, _p_u64]
+        lib.csg_gen_relations_ds2.restype = ctypes.c_int
         lib.csg_gen_hash.argtypes = [_p_u64, ctypes.c_int64]
         lib.csg_gen_hash.restype = ctypes.c_uint64
         _lib = lib
@@ -83,6 +87,29 @@ def make_causet(dim, N, seed):
     """(coords, bits) of a seeded sprinkling into the flat causal diamond."""
     coords = sprinkle(dim, N, seed)
     return coords, relations_from_coords(coords)
+
+
+def sprinkle_de_sitter(N, seed, eta0=0.5):
+    """(1+1) de Sitter slab |eta| <= eta0: conformal-time-sorted (eta, theta), shape (N, 2)."""
+    coords = np.zeros((N, 2), dtype=np.float64)
+    if N > 0 and _load().csg_gen_coords_ds2(int(seed), int(N), float(eta0), coords) != 0:
+        raise MemoryError("sprinkle_de_sitter")
+    return coords
+
+
+def relations_de_sitter(coords):
+    coords = np.ascontiguousarray(coords, dtype=np.float64)
+    N = coords.shape[0]
+    bits = np.zeros((N, stride_words(N)), dtype=np.uint64)
+    if N > 0:
+        _load().csg_gen_relations_ds2(coords, N, bits)
+    return bits
+
+
+def make_de_sitter(N, seed, eta0=0.5):
+    """(coords, bits) of a seeded sprinkling into the (1+1) de Sitter slab, the paper's benchmark workload."""
+    coords = sprinkle_de_sitter(N, seed, eta0)
+    return coords, relations_de_sitter(coords)
 
 
 def bits_hash(bits):

@@ -11,7 +11,8 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "liboracle.so")
-_SRCS = [os.path.join(_HERE, "csg_oracle.c"), os.path.join(_HERE, "alg5_packed.c")]
+_SRCS = [os.path.join(_HERE, "csg_oracle.c"), os.path.join(_HERE, "alg5_packed.c"),
+         os.path.join(_HERE, "link_oracle.c")]
 _lib = None
 
 _i64 = ctypes.c_int64
@@ -25,7 +26,7 @@ def build(force=False):
     newest = max(os.path.getmtime(s) for s in _SRCS)
     if not force and os.path.exists(_LIB_PATH) and os.path.getmtime(_LIB_PATH) >= newest:
         return _LIB_PATH
-    cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-o", _LIB_PATH] + _SRCS + ["-lm"]
+    cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-ffp-contract=off", "-fPIC", "-shared", "-o", _LIB_PATH] + _SRCS + ["-lm"]
     subprocess.run(cmd, check=True)
     return _LIB_PATH
 
@@ -54,6 +55,11 @@ def _load():
     lib.csg_alg5_counts_rows.argtypes = [_p_u64, _i64, _i64, _i64, _i64, _i64, _p_i64,
                                          ctypes.POINTER(_i64)]
     lib.csg_alg5_counts_rows.restype = None
+    lib.csg_oracle_link.argtypes = [ctypes.c_int, np.ctypeslib.ndpointer(dtype=np.float64, flags="C_CONTIGUOUS"),
+                                    _i64, _p_u8]
+    lib.csg_oracle_link.restype = None
+    lib.csg_oracle_link_dim.argtypes = [ctypes.c_int]
+    lib.csg_oracle_link_dim.restype = ctypes.c_int
     lib.csg_alg5_threads.argtypes = []
     lib.csg_alg5_threads.restype = ctypes.c_int
     _lib = lib
@@ -139,3 +145,19 @@ def alg5_counts_rows(bits, N, kmax, row_begin, row_end):
 
 def alg5_threads():
     return int(_load().csg_alg5_threads())
+
+
+GEOM_MINKOWSKI_2D, GEOM_MINKOWSKI_4D, GEOM_DESITTER_2D = 0, 1, 2
+
+
+def link(geometry, coords):
+    """Dense linking (de Sitter test PAPER.md:465): time-sorted coordinates (N, dim) ->
+    symmetric N x N byte matrix, zero diagonal."""
+    lib = _load()
+    coords = np.ascontiguousarray(coords, dtype=np.float64)
+    N, dim = coords.shape
+    assert dim == lib.csg_oracle_link_dim(int(geometry))
+    B = np.zeros((N, N), dtype=np.uint8)
+    if N:
+        lib.csg_oracle_link(int(geometry), coords, N, B)
+    return B
