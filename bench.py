@@ -215,7 +215,7 @@ def run_ours(args, cfg, rank, local_rank, world):
     tiles_mode = args.shard == "tiles" and world > 1
     seed = cfg["seed"] if tiles_mode else multigpu.ensemble_seed(cfg["seed"], rank)
     t0 = time.perf_counter()
-    _, bits = csg_inputs.make_causet(dim, N, seed)
+    coords, bits = csg_inputs.make_causet(dim, N, seed)
     gen_s = time.perf_counter() - t0
     host = torch.from_numpy(bits.view(np.int64)).pin_memory()
     d_bits = host.to("cuda", non_blocking=False)
@@ -254,6 +254,7 @@ def run_ours(args, cfg, rank, local_rank, world):
     barrier()
     clocks = sampler.stop() if rank == 0 else None
     launches = csg.csg_launch_count() - launches0
+    launches_per_step = launches // max(args.steps, 1)
     ms_total = ev0.elapsed_time(ev1)
     kernel_ms = csg.csg_kernel_ms_history(min(args.steps, 64))
     csg.csg_set_kernel_timing(False)
@@ -270,7 +271,30 @@ def run_ours(args, cfg, rank, local_rank, world):
     e2e_s = time.perf_counter() - t0
     assert (c_host == result_counts).all() and S_host == result_S, "e2e and device legs disagree"
 
-    ms_total, e2e_ms = multigpu.max_over_ranks([ms_total, 1e3 * e2e_s], device="cuda")
+    # ---- linking leg: coordinates -> relation matrix on the device, then coordinates -> action
+    geom = csg.GEOM_MINKOWSKI_4D if dim == 4 else csg.GEOM_MINKOWSKI_2D
+    coords_pinned = torch.from_numpy(coords).pin_memory()
+    d_coords = coords_pinned.to("cuda")
+    d_linked = torch.empty_like(d_bits)
+    csg.csg_set_kernel_timing(True)
+    link_ms = []
+    for it in range(args.warmup + args.steps):
+        csg.csg_link(d_coords, N, geom, d_linked)
+        torch.cuda.synchronize()
+        if it >= args.warmup:
+            link_ms.append(csg.csg_last_link_ms())
+    csg.csg_set_kernel_timing(False)
+    assert torch.equal(d_linked, d_bits), "device-linked matrix differs from the host generator's"
+    del d_linked
+    csg.csg_causet_action_host(coords_pinned, N, geom, eps, kmax)   # warm-up (library-owned matrix buffer)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        c2_host, S2_host = csg.csg_causet_action_host(coords_pinned, N, geom, eps, kmax)
+    e2e_coords_s = time.perf_counter() - t0
+    assert (c2_host == result_counts).all() and S2_host == result_S, "coordinates-in leg disagrees"
+
+    ms_total, e2e_ms, e2e_coords_ms = multigpu.max_over_ranks([ms_total, 1e3 * e2e_s, 1e3 * e2e_coords_s], device="cuda")
 
     if rank != 0:
         if dist is not None:
@@ -341,6 +365,21 @@ def run_ours(args, cfg, rank, local_rank, world):
         "gpu_launches": launches,
         "roofline": roofline,
         "cpu_baseline": cpu_baseline,
+    }
+    l_ms = sum(link_ms) / len(link_ms)
+    pairs = N * (N - 1) // 2
+    fp64_ops = {csg.GEOM_MINKOWSKI_4D: 12, csg.GEOM_MINKOWSKI_2D: 2}[geom]   # DADD/DMUL/DSETP per pair test
+    fp64_peak = 64 * 148 * 1.965e9                                           # FP64 lanes/clk/SM x SMs x max clock
+    line["link"] = {
+        "kernel": "link_kernel<%s>" % ("GEOM_M4" if dim == 4 else "GEOM_M2"), "kernel_ms": l_ms,
+        "pair_tests_per_s": pairs / (l_ms * 1e-3), "write_gbs": N * csg.csg_row_stride_words(N) * 8 / (l_ms * 1e-3) / 1e9,
+        "roofline": {"bound": "alu", "achieved": pairs * fp64_ops / (l_ms * 1e-3) / 1e12, "peak": fp64_peak / 1e12,
+                     "unit": "T fp64 instr/s", "frac": pairs * fp64_ops / (l_ms * 1e-3) / fp64_peak,
+                     "peak_source": "derived: 64 FP64 lanes/clk/SM x 148 SMs x 1.965 GHz (DESIGN.md)"},
+        "e2e_from_coords": {"value": multigpu.whole_job_rate(world * triples, e2e_steps, e2e_coords_ms), "unit": UNIT,
+                            "ms_per_step": e2e_coords_ms / e2e_steps, "h2d_bytes_per_step": N * dim * 8,
+                            "d2h_bytes_per_step": (kmax + 1) * 8 + 8,
+                            "what": "csg_causet_action_host: H2D coords + csg_link + csg_action + D2H"},
     }
     line.update(extra)
     print(json.dumps(line), flush=True)

@@ -43,7 +43,8 @@ enum {
     CSG_E_UNSUPPORTED = -7, /* smeared action in 4D (not defined by the paper) */
     CSG_E_CUDA = -8,        /* a CUDA call failed; csg_strerror(CSG_E_CUDA) carries its text */
     CSG_E_VARIANT = -9,     /* unknown variant id */
-    CSG_E_SHARD = -10       /* nshards < 1 or shard outside [0, nshards) */
+    CSG_E_SHARD = -10,      /* nshards < 1 or shard outside [0, nshards) */
+    CSG_E_GEOMETRY = -11    /* unknown geometry id */
 };
 
 #define CSG_MAX_N (1 << 22)
@@ -113,6 +114,36 @@ int64_t csg_tile_schedule(int64_t N, int shard, int nshards, int32_t *tiles_ij, 
  */
 int csg_action_host(const uint64_t *rel_bits_host, int64_t N, int dim, double eps, int kmax,
                     int64_t *counts_host, double *S_host);
+
+/*
+ * Linking (Sec. 2.2: "pairwise relations are found by identifying pairs of elements which are
+ * timelike separated"; dense, symmetric, topologically sorted adjacency matrix): builds the relation matrix
+ * that csg_action reads from the coordinates of the elements.
+ *
+ *   coords   DEVICE, N rows of dim doubles, one row per element, ALREADY sorted by the time coordinate
+ *            (first column), 8-byte aligned, read only.
+ *   geometry CSG_GEOM_MINKOWSKI_2D: (u, v) light-cone coordinates; i<j related iff u_i<u_j and v_i<v_j.
+ *            CSG_GEOM_MINKOWSKI_4D: (t, x, y, z); related iff dt>0 and dt*dt > (dx*dx+dy*dy)+dz*dz.
+ *            CSG_GEOM_DESITTER_2D:  (eta, theta); related iff pi-|pi-|dtheta|| < |deta|.
+ *            All in double, one rounding per operation, strict inequalities; the direction of a relation is
+ *            the index order.  (The two Minkowski tests are not in the paper: DESIGN.md reading A17.)
+ *   rel_bits DEVICE, N*csg_row_stride_words(N) words, 16-byte aligned; every word is overwritten (symmetric
+ *            matrix, zero diagonal, zero padding).
+ * Enqueued on `stream`, no host synchronisation.
+ */
+enum { CSG_GEOM_MINKOWSKI_2D = 0, CSG_GEOM_MINKOWSKI_4D = 1, CSG_GEOM_DESITTER_2D = 2 };
+int csg_link(const double *coords, int64_t N, int geometry, uint64_t *rel_bits, cudaStream_t stream);
+
+/*
+ * Coordinates in, action out, with HOST buffers: copies the N x dim coordinates to the device (4 MiB at
+ * N = 131072 in 4D instead of the 2 GiB matrix), csg_link into a library-owned matrix, csg_action (dim 2 for
+ * the two (1+1) geometries, 4 for Minkowski 4D), copies counts and S back and synchronises.
+ * coords_host: N*dim doubles, time-sorted; counts_host: kmax+1 int64; S_host: 1 double.
+ */
+int csg_causet_action_host(const double *coords_host, int64_t N, int geometry, double eps, int kmax,
+                           int64_t *counts_host, double *S_host);
+/* Milliseconds of the latest csg_link kernel launched while kernel timing was enabled (HOST float). */
+int csg_last_link_ms(float *ms);
 
 /*
  * Test hook: interval sizes of listed pairs.  pairs_ij DEVICE, 2*npairs int64 (i0, j0, i1, j1, ...);

@@ -6,8 +6,8 @@ There is no CPU fallback: if libcsg.so is missing, importing the compute entry p
 
 Functions carry the C names: csg_action, csg_action_host, csg_interval_sizes, csg_row_stride_words,
 csg_set_variant, csg_effective_variant, csg_set_kernel_timing, csg_last_kernel_ms, csg_kernel_ms_history,
-csg_launch_count, csg_action_partial, csg_action_finish, csg_tile_schedule,
-csg_strerror, csg_shutdown.
+csg_launch_count, csg_action_partial, csg_action_finish, csg_tile_schedule, csg_link, csg_causet_action_host,
+csg_last_link_ms, csg_strerror, csg_shutdown.
 """
 import ctypes
 import os
@@ -17,12 +17,14 @@ import numpy as np
 from . import _build
 
 VARIANT_AUTO, VARIANT_BITSET, VARIANT_TENSOR, VARIANT_TENSOR_FP4 = 0, 1, 2, 3
+GEOM_MINKOWSKI_2D, GEOM_MINKOWSKI_4D, GEOM_DESITTER_2D = 0, 1, 2
 LIB_PATH = _build.LIB_PATH
 
 EXPORTS = [
     "csg_row_stride_words", "csg_action", "csg_action_host", "csg_interval_sizes", "csg_set_variant",
     "csg_effective_variant", "csg_set_kernel_timing", "csg_last_kernel_ms", "csg_kernel_ms_history",
-    "csg_launch_count", "csg_action_partial", "csg_action_finish", "csg_tile_schedule",
+    "csg_launch_count", "csg_action_partial", "csg_action_finish", "csg_tile_schedule", "csg_link",
+    "csg_causet_action_host", "csg_last_link_ms",
     "csg_strerror", "csg_shutdown",
 ]
 
@@ -62,6 +64,12 @@ def load():
     lib.csg_action_finish.restype = ci
     lib.csg_tile_schedule.argtypes = [i64, ci, ci, vp, i64]
     lib.csg_tile_schedule.restype = i64
+    lib.csg_link.argtypes = [vp, i64, ci, vp, vp]
+    lib.csg_link.restype = ci
+    lib.csg_causet_action_host.argtypes = [vp, i64, ci, dbl, ci, vp, vp]
+    lib.csg_causet_action_host.restype = ci
+    lib.csg_last_link_ms.argtypes = [ctypes.POINTER(ctypes.c_float)]
+    lib.csg_last_link_ms.restype = ci
     lib.csg_interval_sizes.argtypes = [vp, i64, vp, i64, vp, vp]
     lib.csg_interval_sizes.restype = ci
     lib.csg_set_variant.argtypes = [ci]
@@ -168,6 +176,49 @@ def csg_tile_schedule(N, shard=0, nshards=1):
         got = int(lib.csg_tile_schedule(int(N), int(shard), int(nshards), out.ctypes.data, n))
         assert got == n
     return out
+
+
+def geometry_dim(geometry):
+    return 4 if int(geometry) == GEOM_MINKOWSKI_4D else 2
+
+
+def csg_link(coords, N, geometry, rel_bits=None, stream=None):
+    """int csg_link(coords, N, geometry, rel_bits, stream): time-sorted coordinates (CUDA float64 tensor, N x dim)
+    -> packed symmetric relation matrix (CUDA int64 tensor, N x csg_row_stride_words(N)).  Returns rel_bits."""
+    import torch
+    lib = load()
+    assert coords.is_cuda and coords.dtype == torch.float64 and coords.is_contiguous()
+    assert coords.numel() >= int(N) * geometry_dim(geometry)
+    if rel_bits is None:
+        rel_bits = torch.empty((int(N), csg_row_stride_words(N)), dtype=torch.int64, device=coords.device)
+    assert rel_bits.is_cuda and rel_bits.element_size() == 8 and rel_bits.is_contiguous()
+    assert rel_bits.numel() >= int(N) * csg_row_stride_words(N)
+    _check(lib.csg_link(coords.data_ptr(), int(N), int(geometry), rel_bits.data_ptr(), _stream_handle(stream)))
+    return rel_bits
+
+
+def csg_causet_action_host(coords, N, geometry, eps, kmax):
+    """int csg_causet_action_host(...) with HOST buffers: coords is a numpy float64 (N, dim) array or a (pinned)
+    CPU torch tensor.  Returns (counts numpy int64[kmax+1], S float)."""
+    lib = load()
+    if isinstance(coords, np.ndarray):
+        assert coords.dtype == np.float64 and coords.flags["C_CONTIGUOUS"]
+        ptr, n = coords.ctypes.data, coords.size
+    else:
+        assert not coords.is_cuda and coords.element_size() == 8 and coords.is_contiguous()
+        ptr, n = coords.data_ptr(), coords.numel()
+    assert n >= int(N) * geometry_dim(geometry)
+    counts = np.empty(max(int(kmax), 0) + 1, dtype=np.int64)
+    S = np.empty(1, dtype=np.float64)
+    _check(lib.csg_causet_action_host(ptr, int(N), int(geometry), float(eps), int(kmax), counts.ctypes.data,
+                                      S.ctypes.data))
+    return counts, float(S[0])
+
+
+def csg_last_link_ms():
+    ms = ctypes.c_float(0.0)
+    _check(load().csg_last_link_ms(ctypes.byref(ms)))
+    return float(ms.value)
 
 
 def csg_action_host(rel_bits, N, dim, eps, kmax):

@@ -14,6 +14,7 @@
 
 #include "../../include/csg.h"
 #include "bitset_kernel.cuh"
+#include "link_kernel.cuh"
 #include "tensor_kernel.cuh"
 
 namespace csg {
@@ -101,6 +102,11 @@ struct State {
     long long* d_counts = nullptr;
     size_t d_counts_bytes = 0;
     double* d_S = nullptr;
+    double* d_coords = nullptr;
+    size_t d_coords_bytes = 0;
+    // events around the latest timed linking kernel
+    cudaEvent_t link_ev0 = nullptr, link_ev1 = nullptr;
+    bool link_timed = false;
 };
 static State g;
 
@@ -342,6 +348,47 @@ static int action_device(const uint64_t* rel_bits, long long N, int dim, double 
     return finish_device(counts, N, dim, eps, kmax, S, stream);
 }
 
+static int geometry_dim(int geometry) { return geometry == CSG_GEOM_MINKOWSKI_4D ? 4 : 2; }
+
+// Linking kernel on `stream`: every word of rel_bits (N rows x stride) is overwritten.
+static int link_device(const double* coords, long long N, int geometry, uint64_t* rel_bits, cudaStream_t stream) {
+    int rc = ensure_device();
+    if (rc) return rc;
+    const long long stride = csg_row_stride_words(N);
+    const int nB = (int)((N + LK_T - 1) / LK_T);
+    const long long ntiles = (long long)nB * (nB + 1) / 2;
+    if (g.timing) {
+        if (!g.link_ev0) {
+            CSG_CUDA(cudaEventCreate(&g.link_ev0));
+            CSG_CUDA(cudaEventCreate(&g.link_ev1));
+        }
+        CSG_CUDA(cudaEventRecord(g.link_ev0, stream));
+    }
+    if (geometry == CSG_GEOM_MINKOWSKI_2D)
+        link_kernel<GEOM_M2><<<(unsigned)ntiles, LK_THREADS, 0, stream>>>(coords, N, stride, rel_bits, nB);
+    else if (geometry == CSG_GEOM_MINKOWSKI_4D)
+        link_kernel<GEOM_M4><<<(unsigned)ntiles, LK_THREADS, 0, stream>>>(coords, N, stride, rel_bits, nB);
+    else
+        link_kernel<GEOM_DS2><<<(unsigned)ntiles, LK_THREADS, 0, stream>>>(coords, N, stride, rel_bits, nB);
+    CSG_CUDA(cudaGetLastError());
+    ++g.launches;
+    if (g.timing) {
+        CSG_CUDA(cudaEventRecord(g.link_ev1, stream));
+        g.link_timed = true;
+    }
+    return CSG_OK;
+}
+
+static int ensure_buffer(void** ptr, size_t* have, size_t want) {
+    if (*have >= want) return CSG_OK;
+    if (*ptr) CSG_CUDA(cudaFree(*ptr));
+    *ptr = nullptr;
+    *have = 0;
+    CSG_CUDA(cudaMalloc(ptr, want));
+    *have = want;
+    return CSG_OK;
+}
+
 }  // namespace csg
 
 using namespace csg;
@@ -428,6 +475,55 @@ int csg_action_host(const uint64_t* rel_bits_host, int64_t N, int dim, double ep
     return CSG_OK;
 }
 
+int csg_link(const double* coords, int64_t N, int geometry, uint64_t* rel_bits, cudaStream_t stream) {
+    std::lock_guard<std::mutex> lock(g.mu);
+    if (!coords || !rel_bits) return CSG_E_NULL;
+    if (N < 1 || N > CSG_MAX_N) return CSG_E_SIZE;
+    if (geometry < CSG_GEOM_MINKOWSKI_2D || geometry > CSG_GEOM_DESITTER_2D) return CSG_E_GEOMETRY;
+    if ((reinterpret_cast<uintptr_t>(rel_bits) & 15) || (reinterpret_cast<uintptr_t>(coords) & 7)) return CSG_E_ALIGN;
+    return link_device(coords, N, geometry, rel_bits, stream);
+}
+
+int csg_causet_action_host(const double* coords_host, int64_t N, int geometry, double eps, int kmax,
+                           int64_t* counts_host, double* S_host) {
+    std::lock_guard<std::mutex> lock(g.mu);
+    if (geometry < CSG_GEOM_MINKOWSKI_2D || geometry > CSG_GEOM_DESITTER_2D) return CSG_E_GEOMETRY;
+    const int dim = geometry_dim(geometry);
+    int rc = validate(coords_host, N, dim, eps, kmax, counts_host, S_host);
+    if (rc) return rc;
+    rc = ensure_device();
+    if (rc) return rc;
+    if (!g.host_stream) CSG_CUDA(cudaStreamCreateWithFlags(&g.host_stream, cudaStreamNonBlocking));
+    const size_t coords_bytes = (size_t)N * dim * sizeof(double);
+    const size_t bits_bytes = (size_t)N * (size_t)csg_row_stride_words(N) * sizeof(uint64_t);
+    const size_t counts_bytes = (size_t)(kmax + 1) * sizeof(long long);
+    if ((rc = ensure_buffer(reinterpret_cast<void**>(&g.d_coords), &g.d_coords_bytes, coords_bytes))) return rc;
+    if ((rc = ensure_buffer(reinterpret_cast<void**>(&g.d_bits), &g.d_bits_bytes, bits_bytes))) return rc;
+    if ((rc = ensure_buffer(reinterpret_cast<void**>(&g.d_counts), &g.d_counts_bytes, counts_bytes))) return rc;
+    if (!g.d_S) CSG_CUDA(cudaMalloc(&g.d_S, sizeof(double)));
+    CSG_CUDA(cudaMemcpyAsync(g.d_coords, coords_host, coords_bytes, cudaMemcpyHostToDevice, g.host_stream));
+    rc = link_device(g.d_coords, N, geometry, g.d_bits, g.host_stream);
+    if (rc) return rc;
+    rc = action_device(g.d_bits, N, dim, eps, kmax, g.d_counts, g.d_S, g.host_stream);
+    if (rc) return rc;
+    CSG_CUDA(cudaMemcpyAsync(counts_host, g.d_counts, counts_bytes, cudaMemcpyDeviceToHost, g.host_stream));
+    CSG_CUDA(cudaMemcpyAsync(S_host, g.d_S, sizeof(double), cudaMemcpyDeviceToHost, g.host_stream));
+    CSG_CUDA(cudaStreamSynchronize(g.host_stream));
+    return CSG_OK;
+}
+
+int csg_last_link_ms(float* ms) {
+    std::lock_guard<std::mutex> lock(g.mu);
+    if (!ms) return CSG_E_NULL;
+    if (!g.link_timed) {
+        snprintf(g.cuda_msg, sizeof(g.cuda_msg), "kernel timing: no timed csg_link call so far");
+        return CSG_E_CUDA;
+    }
+    CSG_CUDA(cudaEventSynchronize(g.link_ev1));
+    CSG_CUDA(cudaEventElapsedTime(ms, g.link_ev0, g.link_ev1));
+    return CSG_OK;
+}
+
 int csg_interval_sizes(const uint64_t* rel_bits, int64_t N, const int64_t* pairs_ij, int64_t npairs, int32_t* n_out,
                        cudaStream_t stream) {
     std::lock_guard<std::mutex> lock(g.mu);
@@ -510,6 +606,7 @@ const char* csg_strerror(int code) {
         case CSG_E_UNSUPPORTED: return "smeared action is defined for dim 2 only";
         case CSG_E_CUDA: return g.cuda_msg;
         case CSG_E_VARIANT: return "unknown variant";
+        case CSG_E_GEOMETRY: return "geometry must be CSG_GEOM_MINKOWSKI_2D, _MINKOWSKI_4D or _DESITTER_2D";
         case CSG_E_SHARD: return "shard must satisfy 0 <= shard < nshards";
         default: return "unknown error code";
     }
@@ -521,6 +618,13 @@ int csg_shutdown(void) {
     if (g.d_bits) cudaFree(g.d_bits);
     if (g.d_counts) cudaFree(g.d_counts);
     if (g.d_S) cudaFree(g.d_S);
+    if (g.d_coords) cudaFree(g.d_coords);
+    if (g.link_ev0) cudaEventDestroy(g.link_ev0);
+    if (g.link_ev1) cudaEventDestroy(g.link_ev1);
+    g.link_ev0 = g.link_ev1 = nullptr;
+    g.link_timed = false;
+    g.d_coords = nullptr;
+    g.d_coords_bytes = 0;
     for (int k = 0; k < TIMING_RING; ++k) {
         if (g.ev0[k]) cudaEventDestroy(g.ev0[k]);
         if (g.ev1[k]) cudaEventDestroy(g.ev1[k]);
