@@ -368,7 +368,7 @@ def run_ours(args, cfg, rank, local_rank, world):
     }
     l_ms = sum(link_ms) / len(link_ms)
     pairs = N * (N - 1) // 2
-    fp64_ops = {csg.GEOM_MINKOWSKI_4D: 12, csg.GEOM_MINKOWSKI_2D: 2}[geom]   # DADD/DMUL/DSETP per pair test
+    fp64_ops = {csg.GEOM_MINKOWSKI_4D: 11, csg.GEOM_MINKOWSKI_2D: 2}[geom]   # DADD/DMUL/DSETP per pair test (dt>0 is an integer compare)
     fp64_peak = 64 * 148 * 1.965e9                                           # FP64 lanes/clk/SM x SMs x max clock
     line["link"] = {
         "kernel": "link_kernel<%s>" % ("GEOM_M4" if dim == 4 else "GEOM_M2"), "kernel_ms": l_ms,

@@ -30,17 +30,19 @@ struct LinkTraits {
     static constexpr int DIM = GEOM == GEOM_M4 ? 4 : 2;
 };
 
-// Is the earlier element a (coordinates a[]) related to the later element b?
+// Is the earlier element a (coordinates a[]) related to the later element b?  Branch-free.
 template <int GEOM>
 __device__ __forceinline__ bool timelike(const double* a, const double* b) {
     if (GEOM == GEOM_M2) {
-        return a[0] < b[0] && a[1] < b[1];
+        return (a[0] < b[0]) & (a[1] < b[1]);
     } else if (GEOM == GEOM_M4) {
         const double dt = __dsub_rn(b[0], a[0]), dx = __dsub_rn(b[1], a[1]);
         const double dy = __dsub_rn(b[2], a[2]), dz = __dsub_rn(b[3], a[3]);
         double s2 = __dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy));
         s2 = __dadd_rn(s2, __dmul_rn(dz, dz));
-        return dt > 0.0 && __dmul_rn(dt, dt) > s2;
+        // dt > 0.0 on the integer pipe: a double is > 0 iff its bit pattern, read as a signed integer, is > 0
+        // (a positive NaN passes here and fails the next comparison, as it does in "dt > 0.0 && ...")
+        return (__double_as_longlong(dt) > 0LL) & (__dmul_rn(dt, dt) > s2);
     } else {
         const double PI = 3.14159265358979323846;
         const double dth = fabs(__dsub_rn(a[1], b[1]));
@@ -49,15 +51,23 @@ __device__ __forceinline__ bool timelike(const double* a, const double* b) {
     }
 }
 
+// low `n` bits set (n clamped to 0..32)
+__device__ __forceinline__ uint32_t low_bits(long long n) {
+    return n <= 0 ? 0u : (n >= 32 ? 0xFFFFFFFFu : ((1u << (int)n) - 1u));
+}
+
 // coords: N x DIM doubles, one row per element, sorted by time.  rel: N rows of stride64 words, every word
 // of every row is written (zero padding).  Grid: one CTA per tile t = (I, J), I <= J, row-major over I.
+// The pair loop tests every (row, column) of the tile as (earlier, later) with no bounds or order checks; rows
+// and columns beyond N, and the lower triangle of a diagonal tile (where "earlier" is wrong), are masked
+// off the packed words afterwards.
 template <int GEOM>
 __global__ void __launch_bounds__(LK_THREADS, 2)
 link_kernel(const double* __restrict__ coords, long long N, long long stride64, uint64_t* __restrict__ rel, int nB) {
     constexpr int DIM = LinkTraits<GEOM>::DIM;
     __shared__ double ci[DIM][LK_T];
     __shared__ double cj[DIM][LK_T];
-    __shared__ __align__(16) uint32_t tr[LK_T][8 + 1];   // transposed words: row j, 32-bit word w (+1: bank spread)
+    __shared__ uint32_t tr[LK_T][8 + 1];   // transposed words: row j, 32-bit word w (+1: bank spread)
 
     // tile index -> (I, J): row I of the upper triangle holds nB - I tiles, I nB - I(I-1)/2 tiles come
     // before it; closed form, then corrected for the rounding of the square root
@@ -81,56 +91,64 @@ link_kernel(const double* __restrict__ coords, long long N, long long stride64, 
     }
     __syncthreads();
 
-    uint64_t direct[4];
+    const int row_l = 32 * warp + lane;                       // this thread's row of the tile (= tid)
+    const uint32_t rows_ok = low_bits(N - (i0 + 32 * warp));  // rows 32 warp + ii of this warp that exist
+    uint32_t direct[8];
 #pragma unroll
     for (int s = 0; s < 4; ++s) {
         const int ja = 64 * s + lane, jb = ja + 32;           // columns inside the tile
         double a[DIM], b[DIM];
 #pragma unroll
         for (int c = 0; c < DIM; ++c) { a[c] = cj[c][ja]; b[c] = cj[c][jb]; }
-        const bool va = j0 + ja < N, vb = j0 + jb < N;
         uint32_t ta = 0u, tb = 0u, keep_lo = 0u, keep_hi = 0u;
-#pragma unroll 8
-        for (int ii = 0; ii < 32; ++ii) {
-            const int il = 32 * warp + ii;                    // row inside the tile
-            double r[DIM];
+#pragma unroll 1
+        for (int i8 = 0; i8 < 32; i8 += 8) {
+            uint32_t pa8 = 0u, pb8 = 0u;
 #pragma unroll
-            for (int c = 0; c < DIM; ++c) r[c] = ci[c][il];
-            const bool vi = i0 + il < N;
-            bool pa, pb;
-            if (!diag) {
-                pa = vi && va && timelike<GEOM>(r, a);
-                pb = vi && vb && timelike<GEOM>(r, b);
-            } else {                                           // both triangles of a diagonal tile, earlier element first
-                pa = vi && va && (il < ja ? timelike<GEOM>(r, a) : (il > ja && timelike<GEOM>(a, r)));
-                pb = vi && vb && (il < jb ? timelike<GEOM>(r, b) : (il > jb && timelike<GEOM>(b, r)));
+            for (int k = 0; k < 8; ++k) {
+                const int il = 32 * warp + i8 + k;            // row inside the tile
+                double r[DIM];
+#pragma unroll
+                for (int c = 0; c < DIM; ++c) r[c] = ci[c][il];
+                const bool pa = timelike<GEOM>(r, a), pb = timelike<GEOM>(r, b);
+                const uint32_t wa = __ballot_sync(0xFFFFFFFFu, pa), wb = __ballot_sync(0xFFFFFFFFu, pb);
+                if (lane == i8 + k) { keep_lo = wa; keep_hi = wb; }
+                pa8 |= pa ? (1u << k) : 0u;
+                pb8 |= pb ? (1u << k) : 0u;
             }
-            const uint32_t wa = __ballot_sync(0xFFFFFFFFu, pa), wb = __ballot_sync(0xFFFFFFFFu, pb);
-            if (lane == ii) { keep_lo = wa; keep_hi = wb; }
-            ta |= (pa ? 1u : 0u) << ii;
-            tb |= (pb ? 1u : 0u) << ii;
+            ta |= pa8 << i8;
+            tb |= pb8 << i8;
         }
-        direct[s] = (uint64_t)keep_lo | ((uint64_t)keep_hi << 32);
-        tr[ja][warp] = ta;
-        tr[jb][warp] = tb;
-    }
-    {   // upper-triangle words: row i0 + 32 warp + lane, words 4J..4J+3
-        const long long row = i0 + 32 * warp + lane;
-        if (row < N) {
-            uint4* dst = reinterpret_cast<uint4*>(rel + row * stride64 + 4 * J);
-            dst[0] = make_uint4((uint32_t)direct[0], (uint32_t)(direct[0] >> 32), (uint32_t)direct[1], (uint32_t)(direct[1] >> 32));
-            dst[1] = make_uint4((uint32_t)direct[2], (uint32_t)(direct[2] >> 32), (uint32_t)direct[3], (uint32_t)(direct[3] >> 32));
+        // masks: existing columns / rows; on a diagonal tile keep column > row only
+        uint32_t ca = low_bits(N - (j0 + 64 * s)), cb = low_bits(N - (j0 + 64 * s + 32));
+        uint32_t ra = rows_ok, rb = rows_ok;
+        if (diag) {
+            ca &= ~low_bits(row_l + 1 - 64 * s);               // columns 64 s + bit > row_l
+            cb &= ~low_bits(row_l + 1 - 64 * s - 32);
+            ra &= low_bits(ja - 32 * warp);                    // rows 32 warp + bit < ja
+            rb &= low_bits(jb - 32 * warp);
         }
+        direct[2 * s] = keep_lo & ca;
+        direct[2 * s + 1] = keep_hi & cb;
+        tr[ja][warp] = ta & ra;
+        tr[jb][warp] = tb & rb;
     }
-    if (diag) return;
     __syncthreads();
-    {   // mirrored words: row j0 + tid, words 4I..4I+3
-        const long long row = j0 + tid;
-        if (row < N) {
-            uint4* dst = reinterpret_cast<uint4*>(rel + row * stride64 + 4 * I);
-            dst[0] = make_uint4(tr[tid][0], tr[tid][1], tr[tid][2], tr[tid][3]);
-            dst[1] = make_uint4(tr[tid][4], tr[tid][5], tr[tid][6], tr[tid][7]);
-        }
+    if (diag) {   // both triangles land in the same 256 x 256 block: row tid = upper words | mirrored words
+#pragma unroll
+        for (int w = 0; w < 8; ++w) direct[w] |= tr[tid][w];
+    }
+    const long long row = i0 + tid;
+    if (row < N) {   // upper-triangle words: row i0 + tid, words 4J..4J+3
+        uint4* dst = reinterpret_cast<uint4*>(rel + row * stride64 + 4 * J);
+        dst[0] = make_uint4(direct[0], direct[1], direct[2], direct[3]);
+        dst[1] = make_uint4(direct[4], direct[5], direct[6], direct[7]);
+    }
+    const long long rowj = j0 + tid;
+    if (!diag && rowj < N) {   // mirrored words: row j0 + tid, words 4I..4I+3
+        uint4* dst = reinterpret_cast<uint4*>(rel + rowj * stride64 + 4 * I);
+        dst[0] = make_uint4(tr[tid][0], tr[tid][1], tr[tid][2], tr[tid][3]);
+        dst[1] = make_uint4(tr[tid][4], tr[tid][5], tr[tid][6], tr[tid][7]);
     }
 }
 
