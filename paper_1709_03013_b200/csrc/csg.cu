@@ -283,6 +283,7 @@ static int interval_device(const uint64_t* rel_bits, long long N, int kmax, int 
             CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_I8, 5>, cudaFuncAttributeMaxDynamicSharedMemorySize, s8));
             CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_I8, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, s8));
             CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_FP4, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, s4));
+            CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_FP4, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, s4));
             g.attr_set = true;
         }
     }
@@ -302,7 +303,9 @@ static int interval_device(const uint64_t* rel_bits, long long N, int kmax, int 
         const int s8 = TcTraits<KIND_I8>::SMEM_BYTES, s4 = TcTraits<KIND_FP4>::SMEM_BYTES;
         // int8: operand bit TB: the accumulator holds n_ij << 2TB and n_ij <= N-2, so TB is the largest with
         // (N-2) << 2TB < 2^31; TB = 7 turns every unpack shift into a left shift (FMA pipe).
-        if (kind == KIND_FP4)
+        if (kind == KIND_FP4 && dbg != 0)   // timing ablations only (wrong counts)
+            tensor_action_kernel<KIND_FP4, 0, true><<<grid, TC_THREADS, s4, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, g.d_tiles, g.ntiles, dbg);
+        else if (kind == KIND_FP4)
             tensor_action_kernel<KIND_FP4, 0><<<grid, TC_THREADS, s4, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, g.d_tiles, g.ntiles, dbg);
         else if (N - 2 < (1LL << 17))
             tensor_action_kernel<KIND_I8, 7><<<grid, TC_THREADS, s8, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, g.d_tiles, g.ntiles, dbg);

@@ -26,6 +26,9 @@
 //     (and i<j), and bucket n_ij into a privatised shared-memory histogram (low bins) or straight into the
 //     global counts (high bins, smeared action only).  No N x N count matrix ever reaches HBM.
 //
+// `dbg` (env CSG_DEBUG, default 0; a separate ABLATE instantiation of the fp4 kernel) switches parts of the kernel off for timing ablations (1: no MMA issue, 2: no
+// expansion arithmetic, 4: no operand stores, 8: no epilogue work, 16: no fence before publishing a stage, 32: no packed-bit ring); any non-zero value gives wrong counts.
+//
 // Tiles are handed out statically from a list sorted by K-depth, longest first, in boustrophedon order over
 // the persistent clusters (one per SM pair), which balances the triangular workload without a global counter.
 #pragma once
@@ -40,21 +43,16 @@ constexpr int TC_ROWS_A = 128;             // A rows per CTA
 constexpr int TC_ROWS_B = 128;             // B rows per CTA
 constexpr int TC_ROWS = TC_ROWS_A + TC_ROWS_B;
 constexpr int TC_ROW_BYTES = 128;          // bytes per operand row per stage in smem (one 128-byte swizzle row)
-constexpr int TC_STAGES = 4;
 constexpr int TC_A_BYTES = TC_ROWS_A * TC_ROW_BYTES;  // 16 KiB
 constexpr int TC_B_BYTES = TC_ROWS_B * TC_ROW_BYTES;  // 16 KiB
-constexpr int TC_STAGE_BYTES = TC_A_BYTES + TC_B_BYTES;
 constexpr int TC_GROUP = 2;                // stages covered by one packed-bit copy
 constexpr int TC_BITS_BOX_ROWS = 128;
-constexpr int TC_BITS_BUFS = 4;
 constexpr int TC_PRODUCER_WARPS = 16;      // two sets of 8 warps; in a set: 4 warps for the A rows, 4 for the B rows
 constexpr int TC_PRODUCERS = TC_PRODUCER_WARPS * 32;
 constexpr int TC_MMA_WARP = TC_PRODUCER_WARPS;
 constexpr int TC_TMA_WARP = TC_PRODUCER_WARPS + 1;
 constexpr int TC_THREADS = TC_PRODUCERS + 64;  // + the MMA warp + the TMA warp
 constexpr int TC_HIST = 2048;              // privatised low bins per CTA
-constexpr int TC_NUM_BARS = 2 * TC_STAGES + 2 + 2 * TC_BITS_BUFS;
-constexpr int TC_OFF_BITS = TC_STAGES * TC_STAGE_BYTES;
 
 // The two operand encodings of the kernel.
 //   KIND_I8 : one relation bit -> one u8 (0 or 1 << TB); tcgen05.mma kind::i8, K = 32 per instruction, s32
@@ -70,10 +68,33 @@ struct TcTraits {
     static constexpr int BITS_ROW_BYTES = TC_GROUP * STAGE_COLS / 8;          // 32 or 64 bytes per row per copy
     static constexpr int BITS_BOX_BYTES = TC_BITS_BOX_ROWS * BITS_ROW_BYTES;
     static constexpr int BITS_BUF_BYTES = TC_ROWS * BITS_ROW_BYTES;           // 8 or 16 KiB
-    static constexpr int OFF_HIST = TC_OFF_BITS + TC_BITS_BUFS * BITS_BUF_BYTES;
+    // fp4 keeps only the B operand in shared memory (A lives in TMEM, see A_TMEM).
+#ifndef CSG_A_IN_TMEM
+#define CSG_A_IN_TMEM 1
+#endif
+    static constexpr bool A_IN_TMEM = KIND == KIND_FP4 && CSG_A_IN_TMEM;
+    static constexpr int OFF_B = A_IN_TMEM ? 0 : TC_A_BYTES;                  // B tile inside a stage
+    static constexpr int STAGE_BYTES = OFF_B + TC_B_BYTES;                    // 16 or 32 KiB
+    // Ring of operand stages (even: the two producer sets own alternate slots).  The round trip of a slot
+    // (producers arrive on `full` in the leader CTA -> MMA thread -> tcgen05.commit multicast -> `empty`) measured
+    // ~1400 clk with everything else switched off, so 4 slots cap the pace at one stage per ~340 clk before any
+    // work is done; fp4 has room for 6 (B only in shared memory, A ring = 6 x 32 TMEM columns).
+    static constexpr int STAGES = A_IN_TMEM ? 6 : 4;
+    static constexpr int BITS_BUFS = 4;
+    static constexpr int NUM_BARS = 2 * STAGES + 2 + 2 * BITS_BUFS;
+    static constexpr int OFF_BITS = STAGES * STAGE_BYTES;
+    static constexpr int OFF_HIST = OFF_BITS + BITS_BUFS * BITS_BUF_BYTES;
     static constexpr int OFF_BARS = OFF_HIST + TC_HIST * 4;
-    static constexpr int SMEM_BYTES = OFF_BARS + 8 * TC_NUM_BARS + 16 + 1024;  // + TMEM slot + alignment slack
-    static constexpr int TMEM_COLS = KIND == KIND_FP4 ? 512 : 256;            // fp4: + 256 columns of scale factors
+    static constexpr int SMEM_BYTES = OFF_BARS + 8 * NUM_BARS + 16 + 1024;    // + TMEM slot + alignment slack
+    static constexpr int TMEM_COLS = KIND == KIND_FP4 ? 512 : 256;            // fp4: + scale factors + the A ring
+    // fp4: the A operand never touches shared memory.  The A producers write their expanded rows straight into
+    // TMEM (lane = row, 32-bit column j of a K=64 slice = bytes 4j..4j+3 of the row's 32-byte slice, the same
+    // order as the K-major shared-memory row; measured with a one-nibble-per-row probe) and the MMA reads A from
+    // there: half of the operand stores and half of the tensor cores' operand reads leave the shared-memory pipe.
+    static constexpr bool A_TMEM = A_IN_TMEM;
+    static constexpr int TMEM_SF = 256;                                       // scale factors: SFA at +0, SFB at +16
+    static constexpr int TMEM_SFB = TMEM_SF + 16;
+    static constexpr int TMEM_A = 288;                                        // A ring: STAGES x 32 columns (288..479)
 };
 
 // ---------------------------------------------------------------------------------------------- PTX helpers
@@ -186,14 +207,15 @@ __device__ __forceinline__ void tmem_ld_32x32(uint32_t taddr, uint32_t (&v)[32])
     asm volatile(
         "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
         "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
-        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];\n\t"
+        "tcgen05.wait::ld.sync.aligned;"   // same asm statement: nothing that reads v[] can be scheduled above the wait
         : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
           "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]),
           "=r"(v[15]), "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]),
           "=r"(v[22]), "=r"(v[23]), "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]),
           "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
-        : "r"(taddr));
-    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+        : "r"(taddr)
+        : "memory");
 }
 
 // Shared-memory matrix descriptor: K-major operand, 128-byte swizzle, rows of 128 bytes, 8-row groups
@@ -225,6 +247,41 @@ __device__ __forceinline__ void tmem_fill_32x32(uint32_t taddr, uint32_t v) {
         "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
         "{%1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, "
         "%1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1};" ::"r"(taddr), "r"(v) : "memory");
+}
+
+// 32 lanes x 32 columns: thread t of the warp writes its 32 registers (8 x uint4) to lane (base+t), columns c..c+31.
+__device__ __forceinline__ void tmem_st_32x32(uint32_t taddr, const uint4 (&o)[8]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
+        "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};" ::"r"(taddr),
+        "r"(o[0].x), "r"(o[0].y), "r"(o[0].z), "r"(o[0].w), "r"(o[1].x), "r"(o[1].y), "r"(o[1].z), "r"(o[1].w),
+        "r"(o[2].x), "r"(o[2].y), "r"(o[2].z), "r"(o[2].w), "r"(o[3].x), "r"(o[3].y), "r"(o[3].z), "r"(o[3].w),
+        "r"(o[4].x), "r"(o[4].y), "r"(o[4].z), "r"(o[4].w), "r"(o[5].x), "r"(o[5].y), "r"(o[5].z), "r"(o[5].w),
+        "r"(o[6].x), "r"(o[6].y), "r"(o[6].z), "r"(o[6].w), "r"(o[7].x), "r"(o[7].y), "r"(o[7].z), "r"(o[7].w)
+        : "memory");
+}
+// Wait for this thread's tcgen05.st's, then order them before the mbarrier arrive that follows.  Like
+// fence_proxy_async_smem_after, it names the registers of the NEXT stage so that their arithmetic stays above it.
+__device__ __forceinline__ void tmem_wait_st_after(uint4 (&o)[8]) {
+    asm volatile("tcgen05.wait::st.sync.aligned;\n\ttcgen05.fence::before_thread_sync;"
+                 : "+r"(o[0].x), "+r"(o[0].y), "+r"(o[0].z), "+r"(o[0].w), "+r"(o[1].x), "+r"(o[1].y), "+r"(o[1].z),
+                   "+r"(o[1].w), "+r"(o[2].x), "+r"(o[2].y), "+r"(o[2].z), "+r"(o[2].w), "+r"(o[3].x), "+r"(o[3].y),
+                   "+r"(o[3].z), "+r"(o[3].w), "+r"(o[4].x), "+r"(o[4].y), "+r"(o[4].z), "+r"(o[4].w), "+r"(o[5].x),
+                   "+r"(o[5].y), "+r"(o[5].z), "+r"(o[5].w), "+r"(o[6].x), "+r"(o[6].y), "+r"(o[6].z), "+r"(o[6].w),
+                   "+r"(o[7].x), "+r"(o[7].y), "+r"(o[7].z), "+r"(o[7].w)
+                 :
+                 : "memory");
+}
+// D[tmem] (+)= A[tmem] * B[smem]^T, kind::mxf4 block scaled, over the CTA pair: each CTA's half of A sits at the
+// same address of its own TMEM.
+__device__ __forceinline__ void umma_mxf4_2cta_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t bdesc, uint32_t idesc,
+                                                  uint32_t accumulate, uint32_t tmem_sfa, uint32_t tmem_sfb) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::mxf4.block_scale.block32 [%0], [%1], %2, %3, [%5], [%6], p;\n\t}" ::"r"(tmem_d),
+        "r"(tmem_a), "l"(bdesc), "r"(idesc), "r"(accumulate), "r"(tmem_sfa), "r"(tmem_sfb) : "memory");
 }
 
 // ---------------------------------------------------------------------------------------------- bit expansion
@@ -284,36 +341,37 @@ __device__ __forceinline__ void tile_k_range(int I, int J, int& kb_begin, int& k
 // 4^TB, the accumulator holds n_ij << 2TB; the host picks the largest TB with (N-2) << 2TB < 2^31 (exact in s32).
 // KIND_FP4: TB unused (pass 0); the f32 accumulator holds 4 n_ij, exact for n_ij < 2^22.
 // tiles[t] = {I, J}: 256-row blocks, I <= J.  Grid = 2 x (number of SM pairs), cluster (2,1,1).
-template <int KIND, int TB>
+template <int KIND, int TB, bool ABLATE = false>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(TC_THREADS, 1)
 tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_t* __restrict__ rel, long long N,
                      long long stride_words, int kmax, unsigned long long* __restrict__ counts,
-                     const int2* __restrict__ tiles, int ntiles, int dbg) {
+                     const int2* __restrict__ tiles, int ntiles, int dbg_arg) {
     using T = TcTraits<KIND>;
+    const int dbg = ABLATE ? dbg_arg : 0;             // compiled out of the production instantiation
     constexpr int COLS = T::STAGE_COLS, WORDS = T::WORDS;
     extern __shared__ uint8_t smem_raw[];
     // the dynamic shared window starts at the same offset in both CTAs, so this rounding is identical in both
     const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* smem = smem_raw + (smem0 - smem_u32(smem_raw));
     unsigned int* hist = reinterpret_cast<unsigned int*>(smem + T::OFF_HIST);
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + T::OFF_BARS + 8 * TC_NUM_BARS);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + T::OFF_BARS + 8 * T::NUM_BARS);
 
     const int tid = threadIdx.x;
     const int warp = tid >> 5, lane = tid & 31;
     const uint32_t rank = cluster_ctarank();          // 0 = leader (issues the MMAs)
-    const uint32_t full0 = smem0 + T::OFF_BARS, empty0 = full0 + 8 * TC_STAGES;
-    const uint32_t tmem_full = empty0 + 8 * TC_STAGES, tmem_empty = tmem_full + 8;
-    const uint32_t bits_full0 = tmem_empty + 8, bits_empty0 = bits_full0 + 8 * TC_BITS_BUFS;
+    const uint32_t full0 = smem0 + T::OFF_BARS, empty0 = full0 + 8 * T::STAGES;
+    const uint32_t tmem_full = empty0 + 8 * T::STAGES, tmem_empty = tmem_full + 8;
+    const uint32_t bits_full0 = tmem_empty + 8, bits_empty0 = bits_full0 + 8 * T::BITS_BUFS;
 
     for (int b = tid; b < TC_HIST; b += TC_THREADS) hist[b] = 0u;
     if (tid == 0) {
-        for (int s = 0; s < TC_STAGES; ++s) {
+        for (int s = 0; s < T::STAGES; ++s) {
             mbar_init(full0 + 8 * s, TC_PRODUCER_WARPS);       // leader's copy is used: 8 warps of one producer set x 2 CTAs
             mbar_init(empty0 + 8 * s, 1);                      // multicast tcgen05.commit
         }
         mbar_init(tmem_full, 1);                               // multicast tcgen05.commit
         mbar_init(tmem_empty, 2 * TC_PRODUCER_WARPS);          // leader's copy is used
-        for (int b = 0; b < TC_BITS_BUFS; ++b) {
+        for (int b = 0; b < T::BITS_BUFS; ++b) {
             mbar_init(bits_full0 + 8 * b, 1);                  // expect_tx arrive of the TMA thread
             mbar_init(bits_empty0 + 8 * b, TC_PRODUCER_WARPS);
         }
@@ -329,9 +387,8 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
     if (KIND == KIND_FP4 && warp < 4) {
-        // every block scale = 1.0: fill TMEM columns 256..511 of all 128 lanes with UE8M0 0x7F bytes
-        for (int c = 0; c < 8; ++c)
-            tmem_fill_32x32(tmem_base + ((uint32_t)(32 * warp) << 16) + 256u + 32u * c, 0x7F7F7F7Fu);
+        // every block scale = 1.0: fill TMEM columns 256..287 of all 128 lanes with UE8M0 0x7F bytes
+        tmem_fill_32x32(tmem_base + ((uint32_t)(32 * warp) << 16) + T::TMEM_SF, 0x7F7F7F7Fu);
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
         tc_fence_before();
     }
@@ -351,30 +408,81 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
         const bool isA = prow < TC_ROWS_A;
         const int r = isA ? prow : prow - TC_ROWS_A;  // row inside this CTA's A or B operand tile
         const int rt = (int)rank * 128 + r;           // row inside the 256-row block of the cluster tile
-        const int q4 = warp & 3;                      // TMEM lane quarter this warp may read
-        const int cq = warp >> 2;                     // which 64 accumulator columns it drains
-        uint32_t gc = 0;                              // running group count: operand slot = pset + 2*(gc&1)
+        uint32_t sl = 0, sphase = 0;                  // this set's slot counter: operand slot = pset + 2*sl, and its parity
         uint32_t bb = 0, bphase = 0;                  // packed-bit ring position / parity
-        uint32_t tphase = 0;                          // parity of tmem_full
         int pending = -1;                             // ring stage written but not yet published
-        const uint32_t row_smem = smem0 + (isA ? 0 : TC_A_BYTES) + (r >> 3) * 1024 + (r & 7) * 128;
+        const uint32_t row_smem = smem0 + (isA ? 0 : T::OFF_B) + (r >> 3) * 1024 + (r & 7) * 128;
         const int sw = r & 7;
         // This thread's bytes of stage `pset` in a packed-bit buffer.  I8: 32-byte rows, TMA 32-byte swizzle
         // (16-byte halves swapped on odd groups of 4 rows).  FP4: 64-byte rows, TMA 64-byte swizzle (16-byte
         // chunk index ^ (row/2 mod 4)); the thread reads chunks 2*pset and 2*pset+1.
-        const uint32_t bits_row = smem0 + TC_OFF_BITS + prow * T::BITS_ROW_BYTES;
+        const uint32_t bits_row = smem0 + T::OFF_BITS + prow * T::BITS_ROW_BYTES;
         const uint32_t bits_c0 = KIND == KIND_FP4 ? (((2u * pset) ^ ((prow >> 1) & 3)) << 4)
                                                   : (((uint32_t)pset ^ ((prow >> 2) & 1)) << 4);
         const uint32_t bits_c1 = ((2u * pset + 1) ^ ((prow >> 1) & 3)) << 4;   // FP4 only
+        const bool a_tmem = T::A_TMEM && isA;          // warp-uniform: warps 0-3 and 8-11 hold the A rows
+        const uint32_t a_taddr0 = tmem_base + ((uint32_t)(32 * (warp & 3)) << 16) + T::TMEM_A;
         const uint32_t full_leader0 = map_to_cta(full0, 0);
         const uint32_t tmem_empty_leader = map_to_cta(tmem_empty, 0);
+        const int q4 = warp & 3;                      // TMEM lane quarter this warp may read
+        const int cq = warp >> 2;                     // which 64 accumulator columns it drains
+        uint32_t tphase = 0;                          // parity of tmem_full
+
+        // Publish this set's stage that is written but not yet visible to the MMA thread.
+        auto publish_pending = [&]() {
+            if (pending < 0) return;
+            if (a_tmem) {
+                asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+                tc_fence_before();
+            } else {
+                fence_proxy_async_smem();
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(full_leader0 + 8 * pending);
+            pending = -1;
+        };
+        // Fused epilogue of tile (eI, eJ): TMEM -> registers -> mask by R[i][j], i<j -> histogram.
+        auto epilogue = [&](int eI, int eJ) {
+            const long long i0 = (long long)eI * TC_T, j0 = (long long)eJ * TC_T;
+            const long long i = i0 + 128 * (int)rank + 32 * q4 + lane;
+            const uint32_t* relrow32 = reinterpret_cast<const uint32_t*>(rel + (i < N ? i : 0) * stride_words);
+            uint32_t relw[2];
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {             // relation bits first: their latency hides behind the wait
+                const long long jc = j0 + 32 * (2 * cq + e);
+                uint32_t rw = (i < N) ? __ldg(relrow32 + (jc >> 5)) : 0u;
+                if (jc + 31 <= i) rw = 0u;            // keep only columns j > i
+                else if (jc <= i) rw &= 0xFFFFFFFFu << (int)(i - jc + 1);
+                relw[e] = rw;
+            }
+            mbar_wait(tmem_full, tphase);
+            tphase ^= 1;
+            tc_fence_after();
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                if (dbg & 8) break;                   // ablation: no epilogue work
+                uint32_t v[32];
+                tmem_ld_32x32(tmem_base + ((uint32_t)(32 * q4) << 16) + (uint32_t)(32 * (2 * cq + e)), v);
+                const uint32_t rw = relw[e];
+#pragma unroll
+                for (int x = 0; x < 32; ++x) {
+                    const int n = KIND == KIND_FP4 ? (int)(__uint_as_float(v[x]) * 0.25f) : (int)(v[x] >> (2 * TB));
+                    if (((rw >> x) & 1u) && n <= kmax) {
+                        if (n < TC_HIST) atomicAdd(&hist[n], 1u);
+                        else atomicAdd(&counts[n], 1ULL);
+                    }
+                }
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(tmem_empty_leader);
+        };
 
         for (int rd = 0; rd < rounds; ++rd) {
             const int t = rd * G + ((rd & 1) ? (G - 1 - cl) : cl);
             if (t >= ntiles) continue;
             const int2 tile = tiles[t];
             const int I = tile.x, J = tile.y;
-            const long long i0 = (long long)I * TC_T, j0 = (long long)J * TC_T;
             int kb_begin, kb_end;                     // stages of COLS columns, [begin, end): even count
             tile_k_range<COLS>(I, J, kb_begin, kb_end);
             const int kbA = (256 * I + 255) / COLS;   // stages kb <= kbA can hold columns k <= i
@@ -382,11 +490,15 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
 
             // Software pipeline: the fence + arrive that publishes a stage is issued after the ALU work of this
             // set's next stage (its stores have drained by then); the empty-slot barrier is probed before that work.
-            for (int kb0 = kb_begin; kb0 < kb_end; kb0 += TC_GROUP, ++gc) {
-                const uint32_t stage = pset + 2 * (gc & 1), sphase = (gc >> 1) & 1;
+            for (int kb0 = kb_begin; kb0 < kb_end; kb0 += TC_GROUP) {
+                const uint32_t stage = pset + 2 * sl;
                 const int kb = kb0 + pset;
-                mbar_wait(bits_full0 + 8 * bb, bphase);
                 uint32_t w[WORDS];
+                if (dbg & 32) {                               // ablation: no packed-bit ring
+#pragma unroll
+                    for (int m = 0; m < WORDS; ++m) w[m] = 0x01234567u * (m + kb);
+                } else {
+                mbar_wait(bits_full0 + 8 * bb, bphase);
                 {
                     const uint4 v0 = lds128(bits_row + bb * T::BITS_BUF_BYTES + bits_c0);
                     w[0] = v0.x; w[1] = v0.y; w[2] = v0.z; w[3] = v0.w;
@@ -397,7 +509,8 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive_after(bits_empty0 + 8 * bb, w[0], w[WORDS - 1]);
-                if (++bb == TC_BITS_BUFS) { bb = 0; bphase ^= 1; }
+                if (++bb == T::BITS_BUFS) { bb = 0; bphase ^= 1; }
+                }
                 if (isA) {
                     if (kb <= kbA) {                          // keep k > i
                         const int rl = 256 * I + rt - COLS * kb;
@@ -411,7 +524,10 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 }
                 const bool slot_free = mbar_try(empty0 + 8 * stage, sphase ^ 1);
                 uint4 o[8];
-                if (KIND == KIND_FP4) {
+                if (dbg & 2) {                                // ablation: no expansion arithmetic
+#pragma unroll
+                    for (int m = 0; m < 8; ++m) o[m] = make_uint4(w[m % WORDS], w[(m + 1) % WORDS], w[(m + 2) % WORDS], w[(m + 3) % WORDS]);
+                } else if (KIND == KIND_FP4) {
 #pragma unroll
                     for (int m = 0; m < 8; ++m) o[m] = unpack_word_fp4(w[m % WORDS]);
                 } else {
@@ -419,48 +535,27 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                     for (int m = 0; m < 4; ++m) unpack_word<TB>(w[m], o[2 * m], o[2 * m + 1]);
                 }
                 if (pending >= 0) {                           // publish this set's previous stage to the leader's MMA thread
-                    fence_proxy_async_smem_after(o);
+                    if (dbg & 16) {}                          // ablation: no fence before the publish
+                    else if (a_tmem) tmem_wait_st_after(o);
+                    else fence_proxy_async_smem_after(o);
                     __syncwarp();
                     if (lane == 0) mbar_arrive_cluster(full_leader0 + 8 * pending);
                 }
                 if (!slot_free) mbar_wait(empty0 + 8 * stage, sphase ^ 1);
-                const uint32_t rowp = row_smem + stage * TC_STAGE_BYTES;
+                if (dbg & 4) {                                 // ablation: no operand stores
+                } else if (a_tmem) {
+                    tc_fence_after();                          // the MMAs that read this TMEM slot have completed
+                    tmem_st_32x32(a_taddr0 + 32u * stage, o);
+                } else {
+                    const uint32_t rowp = row_smem + stage * T::STAGE_BYTES;
 #pragma unroll
-                for (int c = 0; c < 8; ++c) sts128(rowp + ((c ^ sw) << 4), o[c]);
-                pending = (int)stage;
-            }
-            fence_proxy_async_smem();                          // publish the last stage of the tile
-            __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(full_leader0 + 8 * pending);
-            pending = -1;
-
-            // ---- epilogue: TMEM -> registers -> mask by R[i][j], i<j -> histogram
-            mbar_wait(tmem_full, tphase);
-            tphase ^= 1;
-            tc_fence_after();
-            const long long i = i0 + 128 * (int)rank + 32 * q4 + lane;
-            const uint32_t* relrow32 = reinterpret_cast<const uint32_t*>(rel + (i < N ? i : 0) * stride_words);
-#pragma unroll 1
-            for (int c = 2 * cq; c < 2 * cq + 2; ++c) {
-                uint32_t v[32];
-                tmem_ld_32x32(tmem_base + ((uint32_t)(32 * q4) << 16) + (uint32_t)(32 * c), v);
-                const long long jc = j0 + 32 * c;
-                uint32_t relw = (i < N) ? __ldg(relrow32 + (jc >> 5)) : 0u;
-                // keep only columns j > i
-                if (jc + 31 <= i) relw = 0u;
-                else if (jc <= i) relw &= 0xFFFFFFFFu << (int)(i - jc + 1);
-#pragma unroll
-                for (int x = 0; x < 32; ++x) {
-                    const int n = KIND == KIND_FP4 ? (int)(__uint_as_float(v[x]) * 0.25f) : (int)(v[x] >> (2 * TB));
-                    if (((relw >> x) & 1u) && n <= kmax) {
-                        if (n < TC_HIST) atomicAdd(&hist[n], 1u);
-                        else atomicAdd(&counts[n], 1ULL);
-                    }
+                    for (int c = 0; c < 8; ++c) sts128(rowp + ((c ^ sw) << 4), o[c]);
                 }
+                pending = (int)stage;
+                if (++sl == T::STAGES / 2) { sl = 0; sphase ^= 1; }
             }
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(tmem_empty_leader);
+            publish_pending();                                 // last stage of the tile
+            epilogue(I, J);
         }
     } else if (warp == TC_MMA_WARP) {
         // ================================================================== MMA issuer (leader CTA, lane 0 issues)
@@ -482,15 +577,19 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                     mbar_wait(full0 + 8 * stage, sphase);
                     tc_fence_after();
                     if (lane == 0) {
-                        const uint32_t a_addr = smem0 + stage * TC_STAGE_BYTES;
+                        const uint32_t a_addr = smem0 + stage * T::STAGE_BYTES;
                         const uint64_t adesc = make_kmajor_sw128_desc(a_addr);
-                        const uint64_t bdesc = make_kmajor_sw128_desc(a_addr + TC_A_BYTES);
+                        const uint64_t bdesc = make_kmajor_sw128_desc(a_addr + T::OFF_B);
 #pragma unroll
                         for (int kk = 0; kk < TC_ROW_BYTES / 32; ++kk) {   // 32 bytes of K per instruction: +2 in 16-byte units
                             const uint32_t acc = (kb > kb_begin || kk > 0) ? 1u : 0u;
-                            if (KIND == KIND_FP4)
+                            if (dbg & 1) continue;                          // ablation: no MMA issue
+                            if (KIND == KIND_FP4 && T::A_TMEM)
+                                umma_mxf4_2cta_ts(tmem_base, tmem_base + T::TMEM_A + 32u * stage + 8u * kk, bdesc + 2 * kk,
+                                                  TC_IDESC_FP4, acc, tmem_base + T::TMEM_SF, tmem_base + T::TMEM_SFB);
+                            else if (KIND == KIND_FP4)
                                 umma_mxf4_2cta(tmem_base, adesc + 2 * kk, bdesc + 2 * kk, TC_IDESC_FP4, acc,
-                                               tmem_base + 256u, tmem_base + 384u);
+                                               tmem_base + T::TMEM_SF, tmem_base + T::TMEM_SFB);
                             else
                                 umma_i8_2cta(tmem_base, adesc + 2 * kk, bdesc + 2 * kk, TC_IDESC, acc);
                         }
@@ -498,7 +597,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                         if (kb == kb_end - 1) umma_commit_2cta(tmem_full);
                     }
                     __syncwarp();
-                    if (++stage == TC_STAGES) { stage = 0; sphase ^= 1; }
+                    if (++stage == T::STAGES) { stage = 0; sphase ^= 1; }
                 }
                 ++done_tiles;
             }
@@ -514,14 +613,14 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 const int ia = tile.x * TC_T + 128 * (int)rank, jb = tile.y * TC_T + 128 * (int)rank;
                 int kb_begin, kb_end;
                 tile_k_range<COLS>(tile.x, tile.y, kb_begin, kb_end);
-                for (int kb0 = kb_begin; kb0 < kb_end; kb0 += TC_GROUP) {
+                for (int kb0 = kb_begin; kb0 < ((dbg & 32) ? kb_begin : kb_end); kb0 += TC_GROUP) {
                     mbar_wait(bits_empty0 + 8 * bb, bphase ^ 1);
                     const uint32_t bar = bits_full0 + 8 * bb;
-                    const uint32_t dst = smem0 + TC_OFF_BITS + bb * T::BITS_BUF_BYTES;
+                    const uint32_t dst = smem0 + T::OFF_BITS + bb * T::BITS_BUF_BYTES;
                     mbar_expect_tx(bar, T::BITS_BUF_BYTES);
                     tma_load_2d(dst, &bits_map, kb0 * (COLS / 8), ia, bar);
                     tma_load_2d(dst + T::BITS_BOX_BYTES, &bits_map, kb0 * (COLS / 8), jb, bar);
-                    if (++bb == TC_BITS_BUFS) { bb = 0; bphase ^= 1; }
+                    if (++bb == T::BITS_BUFS) { bb = 0; bphase ^= 1; }
                 }
             }
         }
