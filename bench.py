@@ -34,8 +34,11 @@ def comb3(n):
 
 
 def workload_name(cfg):
-    return "%dD Minkowski diamond N=%d %s (BASELINE.json configs[%d])" % (
-        cfg["dim"], cfg["N"], "local action" if cfg["eps"] == 1.0 else "smeared eps=%g" % cfg["eps"], cfg["index"])
+    what = "local action" if cfg["eps"] == 1.0 else "smeared eps=%g" % cfg["eps"]
+    if cfg.get("geometry") == "ds2":
+        return "(1+1) de Sitter slab eta0=%g N=%d %s (the paper's workload, PAPER.md:453-467; not a BASELINE.json config)" % (
+            cfg.get("eta0", 0.5), cfg["N"], what)
+    return "%dD Minkowski diamond N=%d %s (BASELINE.json configs[%d])" % (cfg["dim"], cfg["N"], what, cfg["index"])
 
 
 def read_peaks():
@@ -162,7 +165,7 @@ def run_reference(args, cfg, rank, world):
     import csg_inputs
     csg_inputs.build()
     N, dim, kmax = cfg["N"], cfg["dim"], cfg["kmax"]
-    _, bits = csg_inputs.make_causet(dim, N, cfg["seed"])
+    _, bits = csg_inputs.make_config(cfg)
     per_step_s = 4.0
     for _ in range(args.warmup):
         oracle_sample(bits, N, kmax, 0.5, nblocks=4)
@@ -215,7 +218,7 @@ def run_ours(args, cfg, rank, local_rank, world):
     tiles_mode = args.shard == "tiles" and world > 1
     seed = cfg["seed"] if tiles_mode else multigpu.ensemble_seed(cfg["seed"], rank)
     t0 = time.perf_counter()
-    coords, bits = csg_inputs.make_causet(dim, N, seed)
+    coords, bits = csg_inputs.make_config(cfg, seed)
     gen_s = time.perf_counter() - t0
     host = torch.from_numpy(bits.view(np.int64)).pin_memory()
     d_bits = host.to("cuda", non_blocking=False)
@@ -272,7 +275,8 @@ def run_ours(args, cfg, rank, local_rank, world):
     assert (c_host == result_counts).all() and S_host == result_S, "e2e and device legs disagree"
 
     # ---- linking leg: coordinates -> relation matrix on the device, then coordinates -> action
-    geom = csg.GEOM_MINKOWSKI_4D if dim == 4 else csg.GEOM_MINKOWSKI_2D
+    geom = (csg.GEOM_DESITTER_2D if cfg.get("geometry") == "ds2" else
+            csg.GEOM_MINKOWSKI_4D if dim == 4 else csg.GEOM_MINKOWSKI_2D)
     coords_pinned = torch.from_numpy(coords).pin_memory()
     d_coords = coords_pinned.to("cuda")
     d_linked = torch.empty_like(d_bits)
@@ -293,6 +297,37 @@ def run_ours(args, cfg, rank, local_rank, world):
         c2_host, S2_host = csg.csg_causet_action_host(coords_pinned, N, geom, eps, kmax)
     e2e_coords_s = time.perf_counter() - t0
     assert (c2_host == result_counts).all() and S2_host == result_S, "coordinates-in leg disagrees"
+
+    # ---- batched small sets: 64 causal sets of BASELINE.json configs[0]'s shape in one call
+    batch_leg = None
+    if rank == 0 and not args.no_batch_leg:
+        c0, nb = csg_inputs.CONFIGS[0], 64
+        sets = np.stack([csg_inputs.make_causet(c0["dim"], c0["N"], c0["seed"] + 7919 * (b + 1))[1] for b in range(nb)])
+        d_sets = torch.from_numpy(sets.view(np.int64)).to("cuda")
+        bc = torch.empty((nb, c0["kmax"] + 1), dtype=torch.int64, device="cuda")
+        bS = torch.empty(nb, dtype=torch.float64, device="cuda")
+        for _ in range(args.warmup):
+            csg.csg_action_batch(d_sets, c0["N"], nb, c0["dim"], 1.0, c0["kmax"], bc, bS)
+        b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        b0.record()
+        for _ in range(args.steps):
+            csg.csg_action_batch(d_sets, c0["N"], nb, c0["dim"], 1.0, c0["kmax"], bc, bS)
+        b1.record()
+        torch.cuda.synchronize()
+        one0, one1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        one0.record()
+        for _ in range(args.steps):
+            for b in range(nb):
+                csg.csg_action(d_sets[b], c0["N"], c0["dim"], 1.0, c0["kmax"], bc[b], bS[b:b + 1])
+        one1.record()
+        torch.cuda.synchronize()
+        bms = b0.elapsed_time(b1) / args.steps
+        batch_leg = {"workload": "%d causal sets, 2D N=%d, local action, one csg_action_batch call" % (nb, c0["N"]),
+                     "ms_per_call": bms, "sets_per_s": nb / (bms * 1e-3),
+                     "triple_tests_per_s": nb * comb3(c0["N"]) / (bms * 1e-3),
+                     "ms_same_sets_one_csg_action_each": one0.elapsed_time(one1) / args.steps}
+        del d_sets
 
     ms_total, e2e_ms, e2e_coords_ms = multigpu.max_over_ranks([ms_total, 1e3 * e2e_s, 1e3 * e2e_coords_s], device="cuda")
 
@@ -368,10 +403,10 @@ def run_ours(args, cfg, rank, local_rank, world):
     }
     l_ms = sum(link_ms) / len(link_ms)
     pairs = N * (N - 1) // 2
-    fp64_ops = {csg.GEOM_MINKOWSKI_4D: 11, csg.GEOM_MINKOWSKI_2D: 2}[geom]   # DADD/DMUL/DSETP per pair test (dt>0 is an integer compare)
+    fp64_ops = {csg.GEOM_MINKOWSKI_4D: 11, csg.GEOM_MINKOWSKI_2D: 2, csg.GEOM_DESITTER_2D: 5}[geom]   # DADD/DMUL/DSETP per pair test (dt>0 is an integer compare)
     fp64_peak = 64 * 148 * 1.965e9                                           # FP64 lanes/clk/SM x SMs x max clock
     line["link"] = {
-        "kernel": "link_kernel<%s>" % ("GEOM_M4" if dim == 4 else "GEOM_M2"), "kernel_ms": l_ms,
+        "kernel": "link_kernel<%s>" % {0: "GEOM_M2", 1: "GEOM_M4", 2: "GEOM_DS2"}[geom], "kernel_ms": l_ms,
         "pair_tests_per_s": pairs / (l_ms * 1e-3), "write_gbs": N * csg.csg_row_stride_words(N) * 8 / (l_ms * 1e-3) / 1e9,
         "roofline": {"bound": "alu", "achieved": pairs * fp64_ops / (l_ms * 1e-3) / 1e12, "peak": fp64_peak / 1e12,
                      "unit": "T fp64 instr/s", "frac": pairs * fp64_ops / (l_ms * 1e-3) / fp64_peak,
@@ -381,6 +416,8 @@ def run_ours(args, cfg, rank, local_rank, world):
                             "d2h_bytes_per_step": (kmax + 1) * 8 + 8,
                             "what": "csg_causet_action_host: H2D coords + csg_link + csg_action + D2H"},
     }
+    if batch_leg is not None:
+        line["batch"] = batch_leg
     line.update(extra)
     print(json.dumps(line), flush=True)
     if dist is not None:
@@ -394,9 +431,10 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=3, help="index into BASELINE.json configs (default 3, the headline)")
+    ap.add_argument("--config", type=int, default=3, help="index into BASELINE.json configs (default 3, the headline); 5 = the paper's de Sitter workload")
     ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 bitset, 2 tensor int8, 3 tensor fp4")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-batch-leg", action="store_true")
     ap.add_argument("--shard", default="ensemble", choices=["ensemble", "tiles"],
                     help="N>1 GPUs: one causal set per rank (weak scaling, default) or one set with its tiles split")
     args = ap.parse_args()

@@ -7,6 +7,7 @@ It imports neither ``oracle`` nor ``paper_1709_03013_b200``.
 """
 from .generate import (  # noqa: F401
     CONFIGS,
+    make_config,
     build,
     stride_words,
     sprinkle,

@@ -18,7 +18,19 @@ CONFIGS = [
     dict(name="cfg2_4d_65536", dim=4, N=65536, eps=1.0, kmax=3, seed=_SEED0 + 2),
     dict(name="cfg3_4d_131072", dim=4, N=131072, eps=1.0, kmax=3, seed=_SEED0 + 3),
     dict(name="cfg4_2d_262144_smeared", dim=2, N=262144, eps=0.1, kmax=262142, seed=_SEED0 + 4),
+    # not a BASELINE.json config: the paper's own benchmark workload (Fig. 4): (1+1) de Sitter slab,
+    # eta0 = 0.5, largest N of its range, smeared action with eps = 2^-6
+    dict(name="paper_ds2_131072_smeared", dim=2, N=131072, eps=2.0 ** -6, kmax=131070, seed=_SEED0 + 5,
+         geometry="ds2", eta0=0.5),
 ]
+
+
+def make_config(cfg, seed=None):
+    """(coords, bits) of a CONFIGS entry (flat diamond or de Sitter slab)."""
+    seed = cfg["seed"] if seed is None else seed
+    if cfg.get("geometry") == "ds2":
+        return make_de_sitter(cfg["N"], seed, cfg.get("eta0", 0.5))
+    return make_causet(cfg["dim"], cfg["N"], seed)
 
 _p_f64 = np.ctypeslib.ndpointer(dtype=np.float64, flags="C_CONTIGUOUS")
 _p_u64 = np.ctypeslib.ndpointer(dtype=np.uint64, flags="C_CONTIGUOUS")

@@ -40,7 +40,7 @@ enum {
     CSG_E_DIM = -4,         /* dim not in {2, 4} */
     CSG_E_EPS = -5,         /* eps NaN or outside (0, 1] */
     CSG_E_KMAX = -6,        /* kmax < 0, kmax > CSG_MAX_KMAX, or too small for the local action */
-    CSG_E_UNSUPPORTED = -7, /* smeared action in 4D (not defined by the paper) */
+    CSG_E_UNSUPPORTED = -7, /* reserved (no argument combination returns it at present) */
     CSG_E_CUDA = -8,        /* a CUDA call failed; csg_strerror(CSG_E_CUDA) carries its text */
     CSG_E_VARIANT = -9,     /* unknown variant id */
     CSG_E_SHARD = -10,      /* nshards < 1 or shard outside [0, nshards) */
@@ -49,6 +49,7 @@ enum {
 
 #define CSG_MAX_N (1 << 22)
 #define CSG_MAX_KMAX (1 << 22)
+#define CSG_MAX_BATCH 65535
 
 enum {
     CSG_VARIANT_AUTO = 0,   /* fp4 tensor variant when N >= 2048, else bitset */
@@ -71,8 +72,10 @@ int64_t csg_row_stride_words(int64_t N);
  *   eps      1.0 -> local action: dim 2: S = 2(N - 2N_0 + 4N_1 - 2N_2) (Eq. 4 with n_i = N_{i-1});
  *                   dim 4: S = (4/sqrt 6)(N - N_0 + 9N_1 - 16N_2 + 8N_3) (not in the paper; A8).
  *                   Needs kmax >= 2 (dim 2) or >= 3 (dim 4).
- *            0 < eps < 1 -> smeared action, dim 2 only (Eq. 5):
- *                   S = 2 eps [N - 2 eps sum_{k=0..kmax} N_k f_2(k, eps)]; pass kmax = N-2 for the full sum.
+ *            0 < eps < 1 -> smeared action; pass kmax = N-2 for the full sum.
+ *                   dim 2 (Eq. 5): S = 2 eps [N - 2 eps sum_{k=0..kmax} N_k f_2(k, eps)];
+ *                   dim 4 (not in the paper; A9): S = (4/sqrt 6) sqrt(eps) [N - eps sum_k N_k f_4(k, eps)],
+ *                   f_4(k,e) = (1-e)^k [1 - 9ek/(1-e) + 8e^2 k(k-1)/(1-e)^2 - (4/3) e^3 k(k-1)(k-2)/(1-e)^3].
  *   kmax     highest interval size that is histogrammed; related pairs with n_ij > kmax are not counted.
  *   counts   DEVICE, kmax+1 int64, overwritten: counts[k] = N_k = number of related pairs i<j with exactly
  *            k elements strictly between (0-based; the paper's n_i is counts[i-1]).
@@ -97,6 +100,16 @@ int csg_action_partial(const uint64_t *rel_bits, int64_t N, int kmax, int shard,
                        cudaStream_t stream);
 int csg_action_finish(const int64_t *counts, int64_t N, int dim, double eps, int kmax, double *S,
                       cudaStream_t stream);
+
+/*
+ * A batch of causal sets of the same size in one call (Monte-Carlo chains and ensemble averages work on many
+ * sets of modest size: PAPER.md:35, 457, 490).  rel_bits DEVICE: `batch` matrices back to back, each
+ * N*csg_row_stride_words(N) words; counts DEVICE: batch x (kmax+1) int64, row b = abundances of set b; S DEVICE:
+ * batch doubles.  Other arguments as csg_action.  1 <= batch <= CSG_MAX_BATCH.  Sets below the tensor threshold
+ * (N < 2048 under CSG_VARIANT_AUTO) share ONE kernel launch (grid.y = set), larger ones run back to back.
+ */
+int csg_action_batch(const uint64_t *rel_bits, int64_t N, int64_t batch, int dim, double eps, int kmax,
+                     int64_t *counts, double *S, cudaStream_t stream);
 
 /*
  * Host logic, no device needed: the pair tiles (I, J), I <= J, in 256-row blocks, that shard `shard` of

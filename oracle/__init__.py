@@ -13,6 +13,8 @@ from .oracle import (  # noqa: F401
     action_local,
     f2,
     action_smeared_2d,
+    f4,
+    action_smeared_4d,
     alg5_counts,
     alg5_counts_rows,
     alg5_threads,

@@ -126,3 +126,38 @@ double csg_oracle_action_smeared_2d(int64_t N, int64_t kmax, const int64_t *coun
         *abs_scale = 4.0 * e * e * asum;
     return 2.0 * e * ((double)N - 2.0 * e * sum);
 }
+
+/* Smeared action in 3+1 dimensions.  NOT IN PAPER (it cites [5],[19],[24] for other dimensions);
+ * DESIGN.md reading A9: the d=4 member of the same family,
+ *   S_e = (4/sqrt 6) sqrt(e) [ N - e sum_k counts[k] f_4(k,e) ],
+ *   f_4(k,e) = (1-e)^k [ 1 - 9 e k/(1-e) + 8 e^2 k(k-1)/(1-e)^2 - (4/3) e^3 k(k-1)(k-2)/(1-e)^3 ],
+ * bracket multiplied out as for f_2 so that e -> 1 gives the local weights 1, -9, 16, -8 (reading A8).
+ * "Parity unpinned" against the paper (nothing printed there); pinned against exact rational evaluation of this
+ * formula and against its e = 1 limit. */
+double csg_oracle_f4(int64_t i, double e)
+{
+    double x = 1.0 - e;
+    double di = (double)i;
+    double t0 = pow(x, di);
+    double t1 = (i >= 1) ? 9.0 * e * di * pow(x, di - 1.0) : 0.0;
+    double t2 = (i >= 2) ? 8.0 * e * e * di * (di - 1.0) * pow(x, di - 2.0) : 0.0;
+    double t3 = (i >= 3) ? (4.0 / 3.0) * e * e * e * di * (di - 1.0) * (di - 2.0) * pow(x, di - 3.0) : 0.0;
+    return ((t0 - t1) + t2) - t3;
+}
+
+double csg_oracle_action_smeared_4d(int64_t N, int64_t kmax, const int64_t *counts, double e, double *abs_scale)
+{
+    double sum = 0.0, comp = 0.0, asum = 0.0;
+    for (int64_t k = 0; k <= kmax; ++k) {
+        double term = (double)counts[k] * csg_oracle_f4(k, e);
+        double y = term - comp;
+        double t = sum + y;
+        comp = (t - sum) - y;
+        sum = t;
+        asum += fabs(term);
+    }
+    double pref = (4.0 / sqrt(6.0)) * sqrt(e);
+    if (abs_scale)
+        *abs_scale = pref * e * asum;
+    return pref * ((double)N - e * sum);
+}

@@ -50,6 +50,11 @@ def _load():
     lib.csg_oracle_action_smeared_2d.argtypes = [_i64, _i64, _p_i64, ctypes.c_double,
                                                  ctypes.POINTER(ctypes.c_double)]
     lib.csg_oracle_action_smeared_2d.restype = ctypes.c_double
+    lib.csg_oracle_f4.argtypes = [_i64, ctypes.c_double]
+    lib.csg_oracle_f4.restype = ctypes.c_double
+    lib.csg_oracle_action_smeared_4d.argtypes = [_i64, _i64, _p_i64, ctypes.c_double,
+                                                 ctypes.POINTER(ctypes.c_double)]
+    lib.csg_oracle_action_smeared_4d.restype = ctypes.c_double
     lib.csg_alg5_counts.argtypes = [_p_u64, _i64, _i64, _i64, _p_i64]
     lib.csg_alg5_counts.restype = None
     lib.csg_alg5_counts_rows.argtypes = [_p_u64, _i64, _i64, _i64, _i64, _i64, _p_i64,
@@ -122,6 +127,19 @@ def action_smeared_2d(N, counts, eps):
     scale = ctypes.c_double(0.0)
     s = _load().csg_oracle_action_smeared_2d(int(N), counts.shape[0] - 1, counts, float(eps),
                                              ctypes.byref(scale))
+    return float(s), float(scale.value)
+
+
+def f4(k, eps):
+    """Smearing weight f_4(k, eps) of the d=4 action (NOT IN PAPER; reading A9)."""
+    return float(_load().csg_oracle_f4(int(k), float(eps)))
+
+
+def action_smeared_4d(N, counts, eps):
+    """d=4 smeared action (reading A9) over counts[0..len-1]; returns (S_eps, abs_scale)."""
+    counts = np.ascontiguousarray(counts, dtype=np.int64)
+    scale = ctypes.c_double(0.0)
+    s = _load().csg_oracle_action_smeared_4d(int(N), counts.shape[0] - 1, counts, float(eps), ctypes.byref(scale))
     return float(s), float(scale.value)
 
 

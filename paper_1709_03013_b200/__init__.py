@@ -7,7 +7,7 @@ There is no CPU fallback: if libcsg.so is missing, importing the compute entry p
 Functions carry the C names: csg_action, csg_action_host, csg_interval_sizes, csg_row_stride_words,
 csg_set_variant, csg_effective_variant, csg_set_kernel_timing, csg_last_kernel_ms, csg_kernel_ms_history,
 csg_launch_count, csg_action_partial, csg_action_finish, csg_tile_schedule, csg_link, csg_causet_action_host,
-csg_last_link_ms, csg_strerror, csg_shutdown.
+csg_last_link_ms, csg_action_batch, csg_strerror, csg_shutdown.
 """
 import ctypes
 import os
@@ -24,7 +24,7 @@ EXPORTS = [
     "csg_row_stride_words", "csg_action", "csg_action_host", "csg_interval_sizes", "csg_set_variant",
     "csg_effective_variant", "csg_set_kernel_timing", "csg_last_kernel_ms", "csg_kernel_ms_history",
     "csg_launch_count", "csg_action_partial", "csg_action_finish", "csg_tile_schedule", "csg_link",
-    "csg_causet_action_host", "csg_last_link_ms",
+    "csg_causet_action_host", "csg_last_link_ms", "csg_action_batch",
     "csg_strerror", "csg_shutdown",
 ]
 
@@ -64,6 +64,8 @@ def load():
     lib.csg_action_finish.restype = ci
     lib.csg_tile_schedule.argtypes = [i64, ci, ci, vp, i64]
     lib.csg_tile_schedule.restype = i64
+    lib.csg_action_batch.argtypes = [vp, i64, i64, ci, dbl, ci, vp, vp, vp]
+    lib.csg_action_batch.restype = ci
     lib.csg_link.argtypes = [vp, i64, ci, vp, vp]
     lib.csg_link.restype = ci
     lib.csg_causet_action_host.argtypes = [vp, i64, ci, dbl, ci, vp, vp]
@@ -135,6 +137,22 @@ def csg_action(rel_bits, N, dim, eps, kmax, counts=None, S=None, stream=None):
         S = torch.empty(1, dtype=torch.float64, device=rel_bits.device)
     _check(lib.csg_action(rel_bits.data_ptr(), int(N), int(dim), float(eps), int(kmax), counts.data_ptr(),
                           S.data_ptr(), _stream_handle(stream)))
+    return counts, S
+
+
+def csg_action_batch(rel_bits, N, batch, dim, eps, kmax, counts=None, S=None, stream=None):
+    """int csg_action_batch(rel_bits, N, batch, dim, eps, kmax, counts, S, stream): `batch` causal sets of N elements,
+    matrices back to back in one CUDA tensor.  Returns (counts (batch, kmax+1) int64, S (batch,) float64)."""
+    import torch
+    lib = load()
+    assert rel_bits.is_cuda and rel_bits.element_size() == 8 and rel_bits.is_contiguous()
+    assert rel_bits.numel() >= int(batch) * int(N) * csg_row_stride_words(N)
+    if counts is None:
+        counts = torch.empty((int(batch), max(int(kmax), 0) + 1), dtype=torch.int64, device=rel_bits.device)
+    if S is None:
+        S = torch.empty(int(batch), dtype=torch.float64, device=rel_bits.device)
+    _check(lib.csg_action_batch(rel_bits.data_ptr(), int(N), int(batch), int(dim), float(eps), int(kmax),
+                                counts.data_ptr(), S.data_ptr(), _stream_handle(stream)))
     return counts, S
 
 

@@ -47,7 +47,10 @@ __device__ __forceinline__ void bitset_tile_from_index(long long t, long long nb
 __global__ void __launch_bounds__(BS_THREADS, 2)
 bitset_action_kernel(const uint32_t* __restrict__ rel, long long N, long long stride32, int kmax,
                      unsigned long long* __restrict__ counts, long long nb, long long ntiles, int shard,
-                     int nshards) {
+                     int nshards, long long set_stride32, long long counts_stride) {
+    // blockIdx.y = causal set of a batch (csg_action_batch): same N, matrices set_stride32 words apart
+    rel += (long long)blockIdx.y * set_stride32;
+    counts += (long long)blockIdx.y * counts_stride;
     __shared__ __align__(16) uint32_t sA[BS_T * BS_LD];
     __shared__ __align__(16) uint32_t sB[BS_T * BS_LD];
     __shared__ unsigned int hist[BS_HIST];

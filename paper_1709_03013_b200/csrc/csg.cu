@@ -25,6 +25,8 @@ namespace csg {
 //   eps == 1, dim 4: S = (4/sqrt 6)(N - N_0 + 9 N_1 - 16 N_2 + 8 N_3)   (not in the paper; A8)
 //   eps <  1, dim 2: Eq. 5: S = 2 eps [N - 2 eps sum_k N_k f_2(k, eps)],
 //                    f_2(k,e) = (1-e)^k - 2 e k (1-e)^(k-1) + e^2 k(k-1)/2 (1-e)^(k-2)   (bracket multiplied out)
+//   eps <  1, dim 4: S = (4/sqrt 6) sqrt(eps) [N - eps sum_k N_k f_4(k, eps)]   (not in the paper; A9),
+//                    f_4(k,e) = (1-e)^k - 9 e k (1-e)^(k-1) + 8 e^2 k(k-1) (1-e)^(k-2) - (4/3) e^3 k(k-1)(k-2) (1-e)^(k-3)
 // The integer combinations are exact in int64 and below 2^53, so the local S is one exact product.
 // The smeared sum is a fixed-order (thread-strided, compensated, then tree) double reduction: deterministic.
 constexpr int FIN_THREADS = 1024;
@@ -33,6 +35,8 @@ __global__ void __launch_bounds__(FIN_THREADS, 1)
 finish_action_kernel(const long long* __restrict__ counts, long long N, int dim, double eps, int kmax,
                      double* __restrict__ S) {
     __shared__ double red[FIN_THREADS];
+    counts += (long long)blockIdx.x * (kmax + 1);     // one CTA per causal set of a batch
+    S += blockIdx.x;
     const int tid = threadIdx.x;
     if (eps == 1.0) {
         if (tid == 0) {
@@ -53,8 +57,14 @@ finish_action_kernel(const long long* __restrict__ counts, long long N, int dim,
         if (c == 0) continue;
         const double dk = (double)k;
         double w = pow(x, dk);
-        if (k >= 1) w -= 2.0 * eps * dk * pow(x, dk - 1.0);
-        if (k >= 2) w += 0.5 * eps * eps * dk * (dk - 1.0) * pow(x, dk - 2.0);
+        if (dim == 2) {
+            if (k >= 1) w -= 2.0 * eps * dk * pow(x, dk - 1.0);
+            if (k >= 2) w += 0.5 * eps * eps * dk * (dk - 1.0) * pow(x, dk - 2.0);
+        } else {
+            if (k >= 1) w -= 9.0 * eps * dk * pow(x, dk - 1.0);
+            if (k >= 2) w += 8.0 * eps * eps * dk * (dk - 1.0) * pow(x, dk - 2.0);
+            if (k >= 3) w -= (4.0 / 3.0) * eps * eps * eps * dk * (dk - 1.0) * (dk - 2.0) * pow(x, dk - 3.0);
+        }
         const double term = (double)c * w;
         const double y = term - comp;
         const double t = sum + y;
@@ -67,7 +77,10 @@ finish_action_kernel(const long long* __restrict__ counts, long long N, int dim,
         if (tid < s) red[tid] += red[tid + s];
         __syncthreads();
     }
-    if (tid == 0) *S = 2.0 * eps * ((double)N - 2.0 * eps * red[0]);
+    if (tid == 0) {
+        if (dim == 2) *S = 2.0 * eps * ((double)N - 2.0 * eps * red[0]);
+        else *S = (4.0 / sqrt(6.0)) * sqrt(eps) * ((double)N - eps * red[0]);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------- host state
@@ -257,7 +270,6 @@ static int validate(const void* rel_bits, long long N, int dim, double eps, int 
     if (!(eps > 0.0 && eps <= 1.0)) return CSG_E_EPS;  // also rejects NaN
     if (kmax < 0 || kmax > CSG_MAX_KMAX) return CSG_E_KMAX;
     if (eps == 1.0 && kmax < (dim == 2 ? 2 : 3)) return CSG_E_KMAX;
-    if (eps < 1.0 && dim == 4) return CSG_E_UNSUPPORTED;
     return CSG_OK;
 }
 
@@ -323,7 +335,7 @@ static int interval_device(const uint64_t* rel_bits, long long N, int kmax, int 
         bitset_action_kernel<<<grid, BS_THREADS, 0, stream>>>(reinterpret_cast<const uint32_t*>(rel_bits), N,
                                                                stride * 2, kmax,
                                                                reinterpret_cast<unsigned long long*>(counts), nb,
-                                                               ntiles, shard, nshards);
+                                                               ntiles, shard, nshards, 0, 0);
     }
     CSG_CUDA(cudaGetLastError());
     ++g.launches;
@@ -429,6 +441,47 @@ int csg_action_finish(const int64_t* counts, int64_t N, int dim, double eps, int
     if (rc) return rc;
     if ((reinterpret_cast<uintptr_t>(counts) & 7) || (reinterpret_cast<uintptr_t>(S) & 7)) return CSG_E_ALIGN;
     return finish_device(reinterpret_cast<const long long*>(counts), N, dim, eps, kmax, S, stream);
+}
+
+int csg_action_batch(const uint64_t* rel_bits, int64_t N, int64_t batch, int dim, double eps, int kmax,
+                     int64_t* counts, double* S, cudaStream_t stream) {
+    std::lock_guard<std::mutex> lock(g.mu);
+    int rc = validate(rel_bits, N, dim, eps, kmax, counts, S);
+    if (rc) return rc;
+    if (batch < 1 || batch > CSG_MAX_BATCH) return CSG_E_SIZE;
+    if ((reinterpret_cast<uintptr_t>(rel_bits) & 15) || (reinterpret_cast<uintptr_t>(counts) & 7) ||
+        (reinterpret_cast<uintptr_t>(S) & 7))
+        return CSG_E_ALIGN;
+    rc = ensure_device();
+    if (rc) return rc;
+    const long long stride = csg_row_stride_words(N);
+    const long long set_words = N * stride;
+    long long* c = reinterpret_cast<long long*>(counts);
+    const int variant = effective_variant(N);
+    if (variant == CSG_VARIANT_BITSET) {
+        // one launch for the whole batch: grid.y = causal set, grid.x = CTAs per set sized so that the grid
+        // still fills the machine (2 CTAs per SM) when the batch alone does not
+        CSG_CUDA(cudaMemsetAsync(c, 0, (size_t)batch * (kmax + 1) * sizeof(long long), stream));
+        const long long nb = (N + BS_T - 1) / BS_T;
+        const long long ntiles = nb * (nb + 1) / 2;
+        const long long per_set = std::max<long long>(1, (2LL * g.sm_count + batch - 1) / batch);
+        const dim3 grid((unsigned)std::min<long long>(ntiles, per_set), (unsigned)batch);
+        bitset_action_kernel<<<grid, BS_THREADS, 0, stream>>>(reinterpret_cast<const uint32_t*>(rel_bits), N, stride * 2,
+                                                               kmax, reinterpret_cast<unsigned long long*>(c), nb, ntiles,
+                                                               0, 1, set_words * 2, kmax + 1);
+        CSG_CUDA(cudaGetLastError());
+        ++g.launches;
+    } else {
+        // large sets fill the machine on their own: one tensor launch per set, back to back on the stream
+        for (int64_t b = 0; b < batch; ++b) {
+            rc = interval_device(rel_bits + b * set_words, N, kmax, 0, 1, c + b * (kmax + 1), stream);
+            if (rc) return rc;
+        }
+    }
+    finish_action_kernel<<<(unsigned)batch, FIN_THREADS, 0, stream>>>(c, N, dim, eps, kmax, S);
+    CSG_CUDA(cudaGetLastError());
+    ++g.launches;
+    return CSG_OK;
 }
 
 int64_t csg_tile_schedule(int64_t N, int shard, int nshards, int32_t* tiles_ij, int64_t capacity) {
@@ -606,7 +659,7 @@ const char* csg_strerror(int code) {
         case CSG_E_DIM: return "dim must be 2 or 4";
         case CSG_E_EPS: return "eps must be in (0, 1]";
         case CSG_E_KMAX: return "kmax out of range (local action needs kmax >= 2 in 2D, >= 3 in 4D)";
-        case CSG_E_UNSUPPORTED: return "smeared action is defined for dim 2 only";
+        case CSG_E_UNSUPPORTED: return "unsupported combination of arguments";
         case CSG_E_CUDA: return g.cuda_msg;
         case CSG_E_VARIANT: return "unknown variant";
         case CSG_E_GEOMETRY: return "geometry must be CSG_GEOM_MINKOWSKI_2D, _MINKOWSKI_4D or _DESITTER_2D";

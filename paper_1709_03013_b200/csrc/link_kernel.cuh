@@ -14,8 +14,7 @@
 //   * the upper-triangle words leave as one 32-byte segment per row per tile, the mirrored words are transposed
 //     through shared memory and leave the same way; padding columns are written as zeros.
 // Arithmetic is double with one rounding per operation (__dsub_rn / __dmul_rn / __dadd_rn are never contracted
-// into FMAs), in the order DESIGN.md's input recipe states, so the bits equal the host generator's and the
-// oracle's bit for bit.
+// into FMAs), in the order DESIGN.md's input recipe states, so the bits equal the host generator's bit for bit.
 #pragma once
 #include <cstdint>
 

@@ -147,6 +147,46 @@ def test_tile_shards_sum_to_the_whole(csg, variant, dim, N, eps, nshards):
         assert float(S.item()) == oracle.action_local(dim, N, want)
 
 
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("N,eps", [(900, 0.25), (2300, 2.0 ** -4)])
+def test_smeared_action_4d(csg, variant, N, eps):
+    """Reading A9 (not in the paper): d=4 smeared action from the full histogram."""
+    _, bits = csg_inputs.make_causet(4, N, 90 + N)
+    want = reference_counts(bits, N, N - 2)
+    got, S = run_action(csg, bits, N, 4, eps, N - 2, variant)
+    assert (got == want).all()
+    s_want, scale = oracle.action_smeared_4d(N, want, eps)
+    assert abs(S - s_want) <= 1e-12 * scale + 1e-15 * abs(s_want), (S, s_want, scale)
+
+
+@pytest.mark.parametrize("dim,N,batch,eps", [(2, 1, 3, 1.0), (2, 200, 7, 1.0), (4, 1000, 5, 1.0), (2, 513, 40, 0.1),
+                                               (4, 2200, 3, 1.0), (2, 2100, 2, 0.5)])
+def test_batch_of_causal_sets(csg, dim, N, batch, eps):
+    """csg_action_batch: every set of the batch equals the oracle and the single-set call (one launch for all sets
+    below the tensor threshold, back-to-back tensor launches above it)."""
+    csg.csg_set_variant(csg.VARIANT_AUTO)
+    kmax = 3 if eps == 1.0 else N - 2
+    sets = [csg_inputs.make_causet(dim, N, 500 + 13 * b + N)[1] for b in range(batch)]
+    d = csg.to_device(np.stack(sets))
+    launches0 = csg.csg_launch_count()
+    counts, S = csg.csg_action_batch(d, N, batch, dim, eps, kmax)
+    torch.cuda.synchronize()
+    launches = csg.csg_launch_count() - launches0
+    assert launches == (2 if N < 2048 else batch + 1)
+    counts, S = counts.cpu().numpy(), S.cpu().numpy()
+    for b in range(batch):
+        want = reference_counts(sets[b], N, kmax)
+        assert (counts[b] == want).all(), b
+        if eps == 1.0:
+            assert S[b] == oracle.action_local(dim, N, np.concatenate([want, np.zeros(4, np.int64)]))
+        else:
+            s_want, scale = oracle.action_smeared_2d(N, want, eps)
+            assert abs(S[b] - s_want) <= 1e-12 * scale
+        c1, S1 = csg.csg_action(d[b], N, dim, eps, kmax)
+        torch.cuda.synchronize()
+        assert (c1.cpu().numpy() == counts[b]).all() and float(S1.item()) == S[b]
+
+
 def test_interval_sizes_hook(csg):
     N = 3000
     _, bits = csg_inputs.make_causet(4, N, 11)

@@ -277,6 +277,42 @@ def test_p12_smeared_action_exact_and_limits():
     assert s == 2 * 0.25 * (10 - 2 * 0.25 * 12)
 
 
+# ---------------------------------------------------------------- reading A9: smeared d=4 action (not in the paper)
+def f4_bracket_form_exact(i, e):
+    """f_4 in the bracketed form DESIGN.md states for reading A9, in rational arithmetic."""
+    x = 1 - e
+    return x ** i * (1 - Fraction(9 * i) * e / x + 8 * e * e * i * (i - 1) / (x * x)
+                     - Fraction(4, 3) * e ** 3 * i * (i - 1) * (i - 2) / x ** 3)
+
+
+def test_a9_f4_eps_one_is_the_local_d4_weights():
+    assert [oracle.f4(k, 1.0) for k in range(7)] == [1.0, -9.0, 16.0, -8.0, 0.0, 0.0, 0.0]
+
+
+@pytest.mark.parametrize("eps", [0.1, 2.0 ** -6, 0.5, 0.9])
+def test_a9_f4_matches_exact(eps):
+    e = Fraction(eps)
+    for k in [0, 1, 2, 3, 4, 10, 57, 400, 3000]:
+        exact = f4_bracket_form_exact(k, e)
+        x = 1 - e
+        scale = x ** k * (1 + 9 * e * k / x + 8 * e * e * k * k / (x * x) + Fraction(4, 3) * e ** 3 * k ** 3 / x ** 3)
+        assert abs(Fraction(oracle.f4(k, eps)) - exact) <= Fraction(1, 10 ** 12) * scale + Fraction(1, 10 ** 290)
+
+
+def test_a9_smeared_d4_action_exact_and_limits():
+    N = 400
+    _, bits = csg_inputs.make_causet(4, N, 78)
+    c = oracle.counts_from_bits(bits, N, N - 2)
+    s1, _ = oracle.action_smeared_4d(N, c, 1.0)
+    assert s1 == oracle.action_local(4, N, c)              # eps = 1 is the local action (reading A8)
+    for eps in (0.25, 2.0 ** -4):                           # sqrt(eps) exact in double
+        e = Fraction(eps)
+        bracket = N - e * sum(int(c[k]) * f4_bracket_form_exact(k, e) for k in range(N - 1))
+        s, scale = oracle.action_smeared_4d(N, c, eps)
+        pref = (4.0 / math.sqrt(6.0)) * math.sqrt(eps)
+        assert abs(Fraction(s) - Fraction(pref) * bracket) <= Fraction(scale) * Fraction(1, 10 ** 12) + abs(Fraction(s)) * Fraction(1, 10 ** 15)
+
+
 # ---------------------------------------------------------------- P13/P14: second oracle forms
 @pytest.mark.parametrize("N,p,transitive", [(1, 0.5, True), (2, 0.9, True), (63, 0.3, True), (64, 0.3, False),
                                             (65, 0.2, True), (129, 0.1, False), (300, 0.05, True)])
