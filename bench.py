@@ -410,7 +410,8 @@ def run_ours(args, cfg, rank, local_rank, world):
         "pair_tests_per_s": pairs / (l_ms * 1e-3), "write_gbs": N * csg.csg_row_stride_words(N) * 8 / (l_ms * 1e-3) / 1e9,
         "roofline": {"bound": "alu", "achieved": pairs * fp64_ops / (l_ms * 1e-3) / 1e12, "peak": fp64_peak / 1e12,
                      "unit": "T fp64 instr/s", "frac": pairs * fp64_ops / (l_ms * 1e-3) / fp64_peak,
-                     "peak_source": "derived: 64 FP64 lanes/clk/SM x 148 SMs x 1.965 GHz (DESIGN.md)"},
+                     "peak_source": "derived: 64 FP64 lanes/clk/SM x 148 SMs x 1.965 GHz (DESIGN.md)",
+                     "traffic": read_traffic("link_kernel<%s>" % {0: "GEOM_M2", 1: "GEOM_M4", 2: "GEOM_DS2"}[geom])},
         "e2e_from_coords": {"value": multigpu.whole_job_rate(world * triples, e2e_steps, e2e_coords_ms), "unit": UNIT,
                             "ms_per_step": e2e_coords_ms / e2e_steps, "h2d_bytes_per_step": N * dim * 8,
                             "d2h_bytes_per_step": (kmax + 1) * 8 + 8,
