@@ -187,6 +187,19 @@ def test_batch_of_causal_sets(csg, dim, N, batch, eps):
         assert (c1.cpu().numpy() == counts[b]).all() and float(S1.item()) == S[b]
 
 
+def test_sharded_call_on_one_rank(csg):
+    """multigpu.csg_action_sharded without a process group is one shard of one: same result as csg_action."""
+    from paper_1709_03013_b200 import multigpu
+    _, bits = csg_inputs.make_causet(4, 2700, 12)
+    d = csg.to_device(bits)
+    csg.csg_set_variant(csg.VARIANT_AUTO)
+    c1, S1 = multigpu.csg_action_sharded(d, 2700, 4, 1.0, 3)
+    c2, S2 = csg.csg_action(d, 2700, 4, 1.0, 3)
+    torch.cuda.synchronize()
+    assert (c1.cpu().numpy() == oracle.alg5_counts(bits, 2700, 3)).all()
+    assert torch.equal(c1, c2) and float(S1.item()) == float(S2.item())
+
+
 def test_interval_sizes_hook(csg):
     N = 3000
     _, bits = csg_inputs.make_causet(4, N, 11)
