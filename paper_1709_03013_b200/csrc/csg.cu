@@ -117,6 +117,13 @@ struct State {
     double* d_S = nullptr;
     double* d_coords = nullptr;
     size_t d_coords_bytes = 0;
+    // pipelined host path: row chunks copied on copy_stream, each chunk's tiles launched as soon as it landed
+    cudaStream_t copy_stream = nullptr;
+    std::vector<cudaEvent_t> chunk_ev;
+    long long chunk_N = -1;
+    int2* d_chunk_tiles = nullptr;
+    std::vector<int> chunk_off;         // chunk c owns tiles [chunk_off[c], chunk_off[c+1]) of d_chunk_tiles
+    std::vector<long long> chunk_row_end;
     // events around the latest timed linking kernel
     cudaEvent_t link_ev0 = nullptr, link_ev1 = nullptr;
     bool link_timed = false;
@@ -274,6 +281,50 @@ static int validate(const void* rel_bits, long long N, int dim, double eps, int 
 }
 
 // Interval kernel over the tiles of one shard: counts (kmax+1 int64, overwritten) <- this shard's abundances.
+// TMA descriptor + dynamic shared memory opt-in of the tensor kernels.
+static int ensure_tensor_ready(int kind, const uint64_t* rel_bits, long long N, long long stride) {
+    int rc = ensure_bits_map(kind, rel_bits, N, stride);
+    if (rc) return rc;
+    if (!g.attr_set) {
+        const int s8 = TcTraits<KIND_I8>::SMEM_BYTES, s4 = TcTraits<KIND_FP4>::SMEM_BYTES;
+        CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_I8, 7>, cudaFuncAttributeMaxDynamicSharedMemorySize, s8));
+        CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_I8, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, s8));
+        CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_I8, 5>, cudaFuncAttributeMaxDynamicSharedMemorySize, s8));
+        CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_I8, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, s8));
+        CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_FP4, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, s4));
+        CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_FP4, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, s4));
+        g.attr_set = true;
+    }
+    return CSG_OK;
+}
+
+// One launch of the tensor kernel over a tile list (counts are added to, not zeroed).
+static int launch_tensor(int kind, const uint64_t* rel_bits, long long N, long long stride, int kmax, long long* counts,
+                         const int2* d_tiles, int ntiles, cudaStream_t stream) {
+    const int grid = 2 * std::max(1, std::min(ntiles, g.sm_count / 2));   // one CTA pair per SM pair
+    unsigned long long* c64 = reinterpret_cast<unsigned long long*>(counts);
+    const char* dbg_env = getenv("CSG_DEBUG");
+    const int dbg = dbg_env ? atoi(dbg_env) : 0;
+    const int s8 = TcTraits<KIND_I8>::SMEM_BYTES, s4 = TcTraits<KIND_FP4>::SMEM_BYTES;
+    // int8: operand bit TB: the accumulator holds n_ij << 2TB and n_ij <= N-2, so TB is the largest with
+    // (N-2) << 2TB < 2^31; TB = 7 turns every unpack shift into a left shift (FMA pipe).
+    if (kind == KIND_FP4 && dbg != 0)   // timing ablations only (wrong counts)
+        tensor_action_kernel<KIND_FP4, 0, true><<<grid, TC_THREADS, s4, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, d_tiles, ntiles, dbg);
+    else if (kind == KIND_FP4)
+        tensor_action_kernel<KIND_FP4, 0><<<grid, TC_THREADS, s4, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, d_tiles, ntiles, dbg);
+    else if (N - 2 < (1LL << 17))
+        tensor_action_kernel<KIND_I8, 7><<<grid, TC_THREADS, s8, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, d_tiles, ntiles, dbg);
+    else if (N - 2 < (1LL << 19))
+        tensor_action_kernel<KIND_I8, 6><<<grid, TC_THREADS, s8, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, d_tiles, ntiles, dbg);
+    else if (N - 2 < (1LL << 21))
+        tensor_action_kernel<KIND_I8, 5><<<grid, TC_THREADS, s8, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, d_tiles, ntiles, dbg);
+    else
+        tensor_action_kernel<KIND_I8, 4><<<grid, TC_THREADS, s8, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, d_tiles, ntiles, dbg);
+    CSG_CUDA(cudaGetLastError());
+    ++g.launches;
+    return CSG_OK;
+}
+
 static int interval_device(const uint64_t* rel_bits, long long N, int kmax, int shard, int nshards,
                            long long* counts, cudaStream_t stream) {
     int rc = ensure_device();
@@ -286,18 +337,8 @@ static int interval_device(const uint64_t* rel_bits, long long N, int kmax, int 
     if (tensor) {
         rc = ensure_tiles(N, shard, nshards, stream);
         if (rc) return rc;
-        rc = ensure_bits_map(kind, rel_bits, N, stride);
+        rc = ensure_tensor_ready(kind, rel_bits, N, stride);
         if (rc) return rc;
-        if (!g.attr_set) {
-            const int s8 = TcTraits<KIND_I8>::SMEM_BYTES, s4 = TcTraits<KIND_FP4>::SMEM_BYTES;
-            CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_I8, 7>, cudaFuncAttributeMaxDynamicSharedMemorySize, s8));
-            CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_I8, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, s8));
-            CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_I8, 5>, cudaFuncAttributeMaxDynamicSharedMemorySize, s8));
-            CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_I8, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, s8));
-            CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_FP4, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, s4));
-            CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_FP4, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, s4));
-            g.attr_set = true;
-        }
     }
     const int slot = (int)(g.timed_calls % TIMING_RING);
     if (g.timing) {
@@ -308,25 +349,8 @@ static int interval_device(const uint64_t* rel_bits, long long N, int kmax, int 
         CSG_CUDA(cudaEventRecord(g.ev0[slot], stream));
     }
     if (tensor) {
-        const int grid = 2 * std::max(1, std::min(g.ntiles, g.sm_count / 2));   // one CTA pair per SM pair
-        unsigned long long* c64 = reinterpret_cast<unsigned long long*>(counts);
-        const char* dbg_env = getenv("CSG_DEBUG");
-        const int dbg = dbg_env ? atoi(dbg_env) : 0;
-        const int s8 = TcTraits<KIND_I8>::SMEM_BYTES, s4 = TcTraits<KIND_FP4>::SMEM_BYTES;
-        // int8: operand bit TB: the accumulator holds n_ij << 2TB and n_ij <= N-2, so TB is the largest with
-        // (N-2) << 2TB < 2^31; TB = 7 turns every unpack shift into a left shift (FMA pipe).
-        if (kind == KIND_FP4 && dbg != 0)   // timing ablations only (wrong counts)
-            tensor_action_kernel<KIND_FP4, 0, true><<<grid, TC_THREADS, s4, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, g.d_tiles, g.ntiles, dbg);
-        else if (kind == KIND_FP4)
-            tensor_action_kernel<KIND_FP4, 0><<<grid, TC_THREADS, s4, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, g.d_tiles, g.ntiles, dbg);
-        else if (N - 2 < (1LL << 17))
-            tensor_action_kernel<KIND_I8, 7><<<grid, TC_THREADS, s8, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, g.d_tiles, g.ntiles, dbg);
-        else if (N - 2 < (1LL << 19))
-            tensor_action_kernel<KIND_I8, 6><<<grid, TC_THREADS, s8, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, g.d_tiles, g.ntiles, dbg);
-        else if (N - 2 < (1LL << 21))
-            tensor_action_kernel<KIND_I8, 5><<<grid, TC_THREADS, s8, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, g.d_tiles, g.ntiles, dbg);
-        else
-            tensor_action_kernel<KIND_I8, 4><<<grid, TC_THREADS, s8, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, g.d_tiles, g.ntiles, dbg);
+        rc = launch_tensor(kind, rel_bits, N, stride, kmax, counts, g.d_tiles, g.ntiles, stream);
+        if (rc) return rc;
     } else {
         const long long nb = (N + BS_T - 1) / BS_T;
         const long long ntiles = nb * (nb + 1) / 2;
@@ -336,9 +360,9 @@ static int interval_device(const uint64_t* rel_bits, long long N, int kmax, int 
                                                                stride * 2, kmax,
                                                                reinterpret_cast<unsigned long long*>(counts), nb,
                                                                ntiles, shard, nshards, 0, 0);
+        CSG_CUDA(cudaGetLastError());
+        ++g.launches;
     }
-    CSG_CUDA(cudaGetLastError());
-    ++g.launches;
     if (g.timing) {
         CSG_CUDA(cudaEventRecord(g.ev1[slot], stream));
         ++g.timed_calls;
@@ -361,6 +385,78 @@ static int action_device(const uint64_t* rel_bits, long long N, int dim, double 
     int rc = interval_device(rel_bits, N, kmax, 0, 1, counts, stream);
     if (rc) return rc;
     return finish_device(counts, N, dim, eps, kmax, S, stream);
+}
+
+// Host matrix -> device in row chunks, the tiles whose LATER row block lies in a chunk launched as soon as that chunk
+// has landed (a tile (I, J) reads rows of blocks I <= J only).  The work of chunk c grows like (c+1)^2 - c^2, so the
+// copies of all but the first chunks hide behind the tiles of the chunks before them: the 2 GiB copy of N = 131072
+// (38 ms over PCIe) costs a few ms instead.  Tensor variants and large matrices only; counts must be zeroed by the
+// caller of this function on `stream` beforehand (done here).
+constexpr int HOST_CHUNKS = 16;
+constexpr long long HOST_PIPELINE_MIN_BYTES = 32LL << 20;
+
+static int ensure_chunk_tiles(long long N, cudaStream_t stream) {
+    if (g.chunk_N == N && g.d_chunk_tiles) return CSG_OK;
+    const int nB = (int)((N + TC_T - 1) / TC_T);
+    const int blocks_per_chunk = (nB + HOST_CHUNKS - 1) / HOST_CHUNKS;
+    const int nchunks = (nB + blocks_per_chunk - 1) / blocks_per_chunk;
+    std::vector<int2> all;
+    build_tile_schedule(N, 0, 1, all);
+    std::vector<std::vector<int2>> per(nchunks);
+    for (const int2& t : all) per[t.y / blocks_per_chunk].push_back(t);   // keeps the deepest-first, patch order
+    std::vector<int2> flat;
+    g.chunk_off.assign(1, 0);
+    g.chunk_row_end.clear();
+    for (int c = 0; c < nchunks; ++c) {
+        flat.insert(flat.end(), per[c].begin(), per[c].end());
+        g.chunk_off.push_back((int)flat.size());
+        g.chunk_row_end.push_back(std::min<long long>(N, (long long)(c + 1) * blocks_per_chunk * TC_T));
+    }
+    if (g.d_chunk_tiles) {
+        CSG_CUDA(cudaStreamSynchronize(stream));
+        CSG_CUDA(cudaFree(g.d_chunk_tiles));
+        g.d_chunk_tiles = nullptr;
+    }
+    CSG_CUDA(cudaMalloc(&g.d_chunk_tiles, flat.size() * sizeof(int2)));
+    CSG_CUDA(cudaMemcpyAsync(g.d_chunk_tiles, flat.data(), flat.size() * sizeof(int2), cudaMemcpyHostToDevice, stream));
+    CSG_CUDA(cudaStreamSynchronize(stream));   // `flat` is a local
+    while ((int)g.chunk_ev.size() < nchunks + 1) {
+        cudaEvent_t e;
+        CSG_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        g.chunk_ev.push_back(e);
+    }
+    g.chunk_N = N;
+    return CSG_OK;
+}
+
+static int interval_host_pipelined(const uint64_t* rel_bits_host, uint64_t* d_bits, long long N, int kmax, int kind,
+                                   long long* counts, cudaStream_t stream) {
+    const long long stride = csg_row_stride_words(N);
+    int rc = ensure_chunk_tiles(N, stream);
+    if (rc) return rc;
+    rc = ensure_tensor_ready(kind, d_bits, N, stride);
+    if (rc) return rc;
+    if (!g.copy_stream) CSG_CUDA(cudaStreamCreateWithFlags(&g.copy_stream, cudaStreamNonBlocking));
+    CSG_CUDA(cudaMemsetAsync(counts, 0, (size_t)(kmax + 1) * sizeof(long long), stream));
+    // the copies must not overtake work of an earlier call that still reads d_bits on `stream`
+    CSG_CUDA(cudaEventRecord(g.chunk_ev.back(), stream));
+    CSG_CUDA(cudaStreamWaitEvent(g.copy_stream, g.chunk_ev.back(), 0));
+    const int nchunks = (int)g.chunk_row_end.size();
+    long long row0 = 0;
+    for (int c = 0; c < nchunks; ++c) {
+        const long long row1 = g.chunk_row_end[c];
+        CSG_CUDA(cudaMemcpyAsync(d_bits + row0 * stride, rel_bits_host + row0 * stride,
+                                 (size_t)(row1 - row0) * stride * sizeof(uint64_t), cudaMemcpyHostToDevice, g.copy_stream));
+        CSG_CUDA(cudaEventRecord(g.chunk_ev[c], g.copy_stream));
+        CSG_CUDA(cudaStreamWaitEvent(stream, g.chunk_ev[c], 0));
+        const int nt = g.chunk_off[c + 1] - g.chunk_off[c];
+        if (nt > 0) {
+            rc = launch_tensor(kind, d_bits, N, stride, kmax, counts, g.d_chunk_tiles + g.chunk_off[c], nt, stream);
+            if (rc) return rc;
+        }
+        row0 = row1;
+    }
+    return CSG_OK;
 }
 
 static int geometry_dim(int geometry) { return geometry == CSG_GEOM_MINKOWSKI_4D ? 4 : 2; }
@@ -522,8 +618,16 @@ int csg_action_host(const uint64_t* rel_bits_host, int64_t N, int dim, double ep
         g.d_counts_bytes = counts_bytes;
     }
     if (!g.d_S) CSG_CUDA(cudaMalloc(&g.d_S, sizeof(double)));
-    CSG_CUDA(cudaMemcpyAsync(g.d_bits, rel_bits_host, bits_bytes, cudaMemcpyHostToDevice, g.host_stream));
-    rc = action_device(g.d_bits, N, dim, eps, kmax, g.d_counts, g.d_S, g.host_stream);
+    const int variant = effective_variant(N);
+    if (variant != CSG_VARIANT_BITSET && bits_bytes >= (size_t)HOST_PIPELINE_MIN_BYTES) {
+        rc = interval_host_pipelined(rel_bits_host, g.d_bits, N, kmax, variant == CSG_VARIANT_TENSOR_FP4 ? KIND_FP4 : KIND_I8,
+                                     g.d_counts, g.host_stream);
+        if (rc) return rc;
+        rc = finish_device(g.d_counts, N, dim, eps, kmax, g.d_S, g.host_stream);
+    } else {
+        CSG_CUDA(cudaMemcpyAsync(g.d_bits, rel_bits_host, bits_bytes, cudaMemcpyHostToDevice, g.host_stream));
+        rc = action_device(g.d_bits, N, dim, eps, kmax, g.d_counts, g.d_S, g.host_stream);
+    }
     if (rc) return rc;
     CSG_CUDA(cudaMemcpyAsync(counts_host, g.d_counts, counts_bytes, cudaMemcpyDeviceToHost, g.host_stream));
     CSG_CUDA(cudaMemcpyAsync(S_host, g.d_S, sizeof(double), cudaMemcpyDeviceToHost, g.host_stream));
@@ -675,6 +779,13 @@ int csg_shutdown(void) {
     if (g.d_counts) cudaFree(g.d_counts);
     if (g.d_S) cudaFree(g.d_S);
     if (g.d_coords) cudaFree(g.d_coords);
+    if (g.d_chunk_tiles) cudaFree(g.d_chunk_tiles);
+    g.d_chunk_tiles = nullptr;
+    g.chunk_N = -1;
+    for (cudaEvent_t e : g.chunk_ev) cudaEventDestroy(e);
+    g.chunk_ev.clear();
+    if (g.copy_stream) cudaStreamDestroy(g.copy_stream);
+    g.copy_stream = nullptr;
     if (g.link_ev0) cudaEventDestroy(g.link_ev0);
     if (g.link_ev1) cudaEventDestroy(g.link_ev1);
     g.link_ev0 = g.link_ev1 = nullptr;

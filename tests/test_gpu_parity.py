@@ -187,6 +187,29 @@ def test_batch_of_causal_sets(csg, dim, N, batch, eps):
         assert (c1.cpu().numpy() == counts[b]).all() and float(S1.item()) == S[b]
 
 
+@pytest.mark.parametrize("dim,N,eps", [(2, 16384, 1.0), (4, 20001, 1.0), (2, 17000, 0.1)])
+def test_host_entry_point_pipelined(csg, dim, N, eps):
+    """Matrices of 32 MiB and more go to the device in row chunks, each chunk's tiles launched as it lands: same
+    counts and S as the device-resident call and as Algorithm 5; pinned and pageable host memory; repeatable."""
+    _, bits = csg_inputs.make_causet(dim, N, 4000 + N)
+    kmax = 3 if eps == 1.0 else N - 2
+    csg.csg_set_variant(csg.VARIANT_AUTO)
+    want = oracle.alg5_counts(bits, N, kmax)
+    counts, S = csg.csg_action_host(bits, N, dim, eps, kmax)                      # pageable
+    assert (counts == want).all()
+    pinned = torch.from_numpy(bits.view(np.int64)).pin_memory()
+    for _ in range(2):
+        counts2, S2 = csg.csg_action_host(pinned, N, dim, eps, kmax)
+        assert (counts2 == want).all() and S2 == S
+    c_dev, S_dev = csg.csg_action(csg.to_device(bits), N, dim, eps, kmax)
+    torch.cuda.synchronize()
+    assert (c_dev.cpu().numpy() == want).all() and float(S_dev.item()) == S
+    csg.csg_set_variant(csg.VARIANT_TENSOR)                                       # int8 kind through the same path
+    counts3, S3 = csg.csg_action_host(pinned, N, dim, eps, kmax)
+    csg.csg_set_variant(csg.VARIANT_AUTO)
+    assert (counts3 == want).all() and S3 == S
+
+
 def test_sharded_call_on_one_rank(csg):
     """multigpu.csg_action_sharded without a process group is one shard of one: same result as csg_action."""
     from paper_1709_03013_b200 import multigpu
