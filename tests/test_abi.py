@@ -46,6 +46,7 @@ def test_variant_setter(lib):
     assert csg.csg_effective_variant(1 << 17) == csg.VARIANT_BITSET
     csg.csg_set_variant(csg.VARIANT_AUTO)
     assert csg.csg_effective_variant(1024) == csg.VARIANT_BITSET
+    assert csg.csg_effective_variant(1025) == csg.VARIANT_TENSOR_FP4
     assert csg.csg_effective_variant(1 << 17) == csg.VARIANT_TENSOR_FP4
     with pytest.raises(csg.CsgError) as e:
         csg.csg_set_variant(7)

@@ -112,6 +112,19 @@ def test_tile_shards_partition_the_upper_triangle(N, nshards):
         assert d[-20:].max() <= 20 and d[:20].min() >= d.max() - 20
 
 
+def test_patch_schedule_keeps_concurrent_tiles_on_few_row_blocks():
+    """What the L2 claim of DESIGN.md rests on: for a matrix larger than L2, the 74 tiles that run at the same time
+    (one per SM pair, consecutive in the schedule) touch a few dozen 256-row blocks, not ~148 as in diagonal order."""
+    import paper_1709_03013_b200 as csg
+    t = csg.csg_tile_schedule(131072)
+    G = 74
+    touched = [len(set(t[r:r + G, 0]) | set(t[r:r + G, 1])) for r in range(0, len(t) - G, G)]
+    assert np.mean(touched) <= 40 and max(touched) <= 2 * (8 + 9) + 4
+    small = csg.csg_tile_schedule(16384)                     # fits L2: plain depth order
+    d = small[:, 1] - small[:, 0]
+    assert (np.diff(d) <= 0).all()
+
+
 def test_multigpu_rate_helpers():
     from paper_1709_03013_b200 import multigpu
     assert multigpu.ensemble_seed(7, 3) == 3007
