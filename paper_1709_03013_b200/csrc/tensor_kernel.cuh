@@ -27,7 +27,7 @@
 //     global counts (high bins, smeared action only).  No N x N count matrix ever reaches HBM.
 //
 // `dbg` (env CSG_DEBUG, default 0; a separate ABLATE instantiation of the fp4 kernel) switches parts of the kernel off for timing ablations (1: no MMA issue, 2: no
-// expansion arithmetic, 4: no operand stores, 8: no epilogue work, 16: no fence before publishing a stage, 32: no packed-bit ring); any non-zero value gives wrong counts.
+// expansion arithmetic, 4: no operand stores, 8: no epilogue work, 16: no fence before publishing a stage, 32: no packed-bit ring, 64: producers free-running, no MMA thread, no epilogue); any non-zero value gives wrong counts.
 //
 // Tiles are handed out statically from a list sorted by K-depth, longest first, in boustrophedon order over
 // the persistent clusters (one per SM pair), which balances the triangular workload without a global counter.
@@ -438,11 +438,12 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 fence_proxy_async_smem();
             }
             __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(full_leader0 + 8 * pending);
+            if (lane == 0 && !(dbg & 64)) mbar_arrive_cluster(full_leader0 + 8 * pending);
             pending = -1;
         };
         // Fused epilogue of tile (eI, eJ): TMEM -> registers -> mask by R[i][j], i<j -> histogram.
         auto epilogue = [&](int eI, int eJ) {
+            if (dbg & 64) return;
             const long long i0 = (long long)eI * TC_T, j0 = (long long)eJ * TC_T;
             const long long i = i0 + 128 * (int)rank + 32 * q4 + lane;
             const uint32_t* relrow32 = reinterpret_cast<const uint32_t*>(rel + (i < N ? i : 0) * stride_words);
@@ -522,7 +523,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
 #pragma unroll
                     for (int m = 0; m < WORDS; ++m) w[m] &= keep_lt(lim, m);
                 }
-                const bool slot_free = mbar_try(empty0 + 8 * stage, sphase ^ 1);
+                const bool slot_free = (dbg & 64) ? true : mbar_try(empty0 + 8 * stage, sphase ^ 1);   // 64: free-running producers
                 uint4 o[8];
                 if (dbg & 2) {                                // ablation: no expansion arithmetic
 #pragma unroll
@@ -539,7 +540,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                     else if (a_tmem) tmem_wait_st_after(o);
                     else fence_proxy_async_smem_after(o);
                     __syncwarp();
-                    if (lane == 0) mbar_arrive_cluster(full_leader0 + 8 * pending);
+                    if (lane == 0 && !(dbg & 64)) mbar_arrive_cluster(full_leader0 + 8 * pending);
                 }
                 if (!slot_free) mbar_wait(empty0 + 8 * stage, sphase ^ 1);
                 if (dbg & 4) {                                 // ablation: no operand stores
@@ -559,7 +560,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
         }
     } else if (warp == TC_MMA_WARP) {
         // ================================================================== MMA issuer (leader CTA, lane 0 issues)
-        if (rank == 0) {
+        if (rank == 0 && !(dbg & 64)) {
             uint32_t stage = 0, sphase = 0, ephase = 0;
             int done_tiles = 0;
             for (int rd = 0; rd < rounds; ++rd) {
