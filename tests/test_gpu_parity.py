@@ -268,6 +268,19 @@ def degree_invariants(bits, N):
     return int(outdeg.sum()), int((indeg * outdeg).sum())
 
 
+def golden_histogram(name):
+    """Line of tests/golden/config_histograms.txt for this config (written by tests/golden/make_config_goldens.py,
+    which calls only the oracle), or None."""
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "config_histograms.txt")
+    for ln in open(path):
+        f = ln.split()
+        if f and f[0] == name:
+            return dict(N=int(f[1]), kmax=int(f[2]), bits_hash=int(f[3], 16), sha256=f[4], total=int(f[5]),
+                        head=[int(x) for x in f[6:14]])
+    return None
+
+
 def check_config(csg, cfg, full_reference):
     N, dim = cfg["N"], cfg["dim"]
     _, bits = csg_inputs.make_causet(dim, N, cfg["seed"])
@@ -295,8 +308,18 @@ def check_config(csg, cfg, full_reference):
     got = csg.csg_interval_sizes(d, N, torch.from_numpy(pairs).cuda()).cpu().numpy()
     for (i, j), n in zip(pairs[:60], got[:60]):
         assert n == oracle.pair_interval(bits, N, i, j)
-    # (4) exact reference histogram where Algorithm 5 finishes in reasonable time
-    if full_reference:
+    # (4) the WHOLE histogram against the oracle's stored one (Algorithm 5 over the full config, minutes of CPU, run
+    #     once by tests/golden/make_config_goldens.py); the bitset hash ties the stored line to this very input
+    gold = golden_histogram(cfg["name"])
+    if gold is not None:
+        import hashlib
+        assert gold["N"] == N and csg_inputs.bits_hash(bits) == gold["bits_hash"]
+        assert int(full.sum()) == gold["total"] and [int(x) for x in full[:8]] == gold["head"]
+        assert hashlib.sha256(np.ascontiguousarray(full, dtype="<i8").tobytes()).hexdigest() == gold["sha256"]
+        if cfg["eps"] == 1.0:
+            assert float(S.item()) == oracle.action_local(dim, N, full[:4])
+    # (5) else the reference histogram computed now, where Algorithm 5 finishes in reasonable time
+    elif full_reference:
         want = oracle.alg5_counts(bits, N, cfg["kmax"])
         assert (counts == want).all(), (counts, want)
         if cfg["eps"] == 1.0:
