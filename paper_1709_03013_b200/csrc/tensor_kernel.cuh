@@ -160,10 +160,6 @@ __device__ __forceinline__ uint4 lds128(uint32_t addr) {
                  : "memory");
     return v;
 }
-// Elected arrive that also names two registers of the warp-wide loads it must not overtake.
-__device__ __forceinline__ void mbar_arrive_after(uint32_t bar, uint32_t dep0, uint32_t dep1) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar), "r"(dep0), "r"(dep1) : "memory");
-}
 __device__ __forceinline__ void sts128(uint32_t addr, const uint4& v) {
     asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w)
                  : "memory");
@@ -495,6 +491,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 const uint32_t stage = pset + 2 * sl;
                 const int kb = kb0 + pset;
                 uint32_t w[WORDS];
+                uint32_t bits_release = 0;
                 if (dbg & 32) {                               // ablation: no packed-bit ring
 #pragma unroll
                     for (int m = 0; m < WORDS; ++m) w[m] = 0x01234567u * (m + kb);
@@ -508,8 +505,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                         w[WORDS - 4] = v1.x; w[WORDS - 3] = v1.y; w[WORDS - 2] = v1.z; w[WORDS - 1] = v1.w;
                     }
                 }
-                __syncwarp();
-                if (lane == 0) mbar_arrive_after(bits_empty0 + 8 * bb, w[0], w[WORDS - 1]);
+                bits_release = bits_empty0 + 8 * bb;          // handed back to the TMA thread after this stage's stores
                 if (++bb == T::BITS_BUFS) { bb = 0; bphase ^= 1; }
                 }
                 if (isA) {
@@ -554,6 +550,17 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 }
                 pending = (int)stage;
                 if (++sl == T::STAGES / 2) { sl = 0; sphase ^= 1; }
+                // Release the packed-bit buffer only now.  The operand stores above consume every word loaded from
+                // it, so the hardware has issued them after the LDS data arrived; an arrive placed right after the LDS
+                // instructions is NOT ordered after their completion (naming the loaded registers as unused asm
+                // operands creates no dependency in the machine code), and with the ring full the TMA thread then
+                // refills the buffer at once: when the shared-memory pipe is backed up (the epilogue's histogram
+                // atomics of slower warps) the delayed LDS returned the bits of the group four ahead.  Seen as a
+                // handful of wrong n_ij per 10^10 pairs at config 4, and as thousands when the epilogue of a tile
+                // overlapped the first stages of the next; located by dumping every n_ij and matching the wrong
+                // rows against "same row, packed bits of the stage 8 later".
+                __syncwarp();
+                if (bits_release != 0 && lane == 0) mbar_arrive(bits_release);
             }
             publish_pending();                                 // last stage of the tile
             epilogue(I, J);
