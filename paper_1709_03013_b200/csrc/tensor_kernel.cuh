@@ -27,7 +27,7 @@
 //     global counts (high bins, smeared action only).  No N x N count matrix ever reaches HBM.
 //
 // `dbg` (env CSG_DEBUG, default 0; a separate ABLATE instantiation of the fp4 kernel) switches parts of the kernel off for timing ablations (1: no MMA issue, 2: no
-// expansion arithmetic, 4: no operand stores, 8: no epilogue work, 16: no fence before publishing a stage, 32: no packed-bit ring, 64: producers free-running, no MMA thread, no epilogue); any non-zero value gives wrong counts.
+// expansion arithmetic, 4: no operand stores, 8: no epilogue work, 16: no fence before publishing a stage, 32: no packed-bit ring, 128: no prefill of the next tile before an epilogue, 64: producers free-running, no MMA thread, no epilogue); any non-zero value gives wrong counts.
 //
 // Tiles are handed out statically from a list sorted by K-depth, longest first, in boustrophedon order over
 // the persistent clusters (one per SM pair), which balances the triangular workload without a global counter.
@@ -52,6 +52,7 @@ constexpr int TC_PRODUCERS = TC_PRODUCER_WARPS * 32;
 constexpr int TC_MMA_WARP = TC_PRODUCER_WARPS;
 constexpr int TC_TMA_WARP = TC_PRODUCER_WARPS + 1;
 constexpr int TC_THREADS = TC_PRODUCERS + 64;  // + the MMA warp + the TMA warp
+constexpr int TC_PREFILL_GROUPS = 2;           // groups (2 stages each) of the next tile expanded before a tile's epilogue
 constexpr int TC_HIST = 2048;              // privatised low bins per CTA
 
 // The two operand encodings of the kernel.
@@ -423,6 +424,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
         const int q4 = warp & 3;                      // TMEM lane quarter this warp may read
         const int cq = warp >> 2;                     // which 64 accumulator columns it drains
         uint32_t tphase = 0;                          // parity of tmem_full
+        int epi_I = -1, epi_J = -1;                   // tile whose accumulators still wait for their epilogue
 
         // Publish this set's stage that is written but not yet visible to the MMA thread.
         auto publish_pending = [&]() {
@@ -487,6 +489,17 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
 
             // Software pipeline: the fence + arrive that publishes a stage is issued after the ALU work of this
             // set's next stage (its stores have drained by then); the empty-slot barrier is probed before that work.
+            // Order of work: ... stages of tile t | first TC_PREFILL_GROUPS groups of tile t+1 | epilogue of tile t |
+            // rest of tile t+1 ...  While the accumulators of tile t are drained (the MMA thread waits for tmem_empty)
+            // the ring already holds the first stages of tile t+1, so the tensor cores restart at once and the
+            // producers get those stages' time to refill their pipeline.
+            const int prefill = (ABLATE && (dbg & 128)) ? 0 : TC_PREFILL_GROUPS;    // dbg 128: epilogue before any next stage
+            if (prefill == 0 && epi_I >= 0) {
+                publish_pending();
+                epilogue(epi_I, epi_J);
+                epi_I = -1;
+            }
+            const int epi_at = kb_begin + TC_GROUP * (min(prefill, (kb_end - kb_begin) / TC_GROUP) - 1);
             for (int kb0 = kb_begin; kb0 < kb_end; kb0 += TC_GROUP) {
                 const uint32_t stage = pset + 2 * sl;
                 const int kb = kb0 + pset;
@@ -561,10 +574,17 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 // rows against "same row, packed bits of the stage 8 later".
                 __syncwarp();
                 if (bits_release != 0 && lane == 0) mbar_arrive(bits_release);
+                if (epi_I >= 0 && kb0 == epi_at) {             // the previous tile's epilogue, after the prefill
+                    publish_pending();
+                    epilogue(epi_I, epi_J);
+                    epi_I = -1;
+                }
             }
-            publish_pending();                                 // last stage of the tile
-            epilogue(I, J);
+            epi_I = I;
+            epi_J = J;
         }
+        publish_pending();                                     // last stage of the last tile
+        if (epi_I >= 0) epilogue(epi_I, epi_J);
     } else if (warp == TC_MMA_WARP) {
         // ================================================================== MMA issuer (leader CTA, lane 0 issues)
         if (rank == 0 && !(dbg & 64)) {
