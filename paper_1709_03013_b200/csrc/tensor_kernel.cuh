@@ -52,6 +52,10 @@ constexpr int TC_PRODUCERS = TC_PRODUCER_WARPS * 32;
 constexpr int TC_MMA_WARP = TC_PRODUCER_WARPS;
 constexpr int TC_TMA_WARP = TC_PRODUCER_WARPS + 1;
 constexpr int TC_THREADS = TC_PRODUCERS + 64;  // + the MMA warp + the TMA warp
+#ifndef CSG_WHOLE_GROUP
+#define CSG_WHOLE_GROUP 1
+#endif
+constexpr bool TC_WHOLE_GROUP = CSG_WHOLE_GROUP != 0;   // a producer set expands both stages of every second group
 constexpr int TC_PREFILL_GROUPS = 2;           // groups (2 stages each) of the next tile expanded before a tile's epilogue
 constexpr int TC_HIST = 2048;              // privatised low bins per CTA
 
@@ -370,7 +374,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
         mbar_init(tmem_empty, 2 * TC_PRODUCER_WARPS);          // leader's copy is used
         for (int b = 0; b < T::BITS_BUFS; ++b) {
             mbar_init(bits_full0 + 8 * b, 1);                  // expect_tx arrive of the TMA thread
-            mbar_init(bits_empty0 + 8 * b, TC_PRODUCER_WARPS);
+            mbar_init(bits_empty0 + 8 * b, TC_WHOLE_GROUP ? TC_PRODUCER_WARPS / 2 : TC_PRODUCER_WARPS);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -398,14 +402,17 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
 
     if (warp < TC_PRODUCER_WARPS) {
         // ================================================================== producers + epilogue
-        // Two producer sets of 8 warps; set p expands stage p of every 2-stage group (one row per thread), so a
-        // warp has two stage times for the serial chain wait -> expand -> fence -> arrive -> store of its stage.
+        // Two producer sets of 8 warps, one row per thread.  TC_WHOLE_GROUP (default): set p expands both stages of
+        // every second 2-stage group (one buffer wait, one release and one trip through the loop per two stages);
+        // otherwise set p expands stage p of every group.  Either way a warp has two stage times for the serial
+        // chain wait -> expand -> fence -> arrive -> store of a stage.
         const int pset = warp >> 3;                   // 0 or 1: which stage of each group this thread expands
         const int prow = tid & 255;                   // row 0..255 of this CTA's staged rows
         const bool isA = prow < TC_ROWS_A;
         const int r = isA ? prow : prow - TC_ROWS_A;  // row inside this CTA's A or B operand tile
         const int rt = (int)rank * 128 + r;           // row inside the 256-row block of the cluster tile
         uint32_t sl = 0, sphase = 0;                  // this set's slot counter: operand slot = pset + 2*sl, and its parity
+        uint32_t gsel = 0, slot0 = 0, spar = 0;       // TC_WHOLE_GROUP: running group count, first slot of the group, use parity
         uint32_t bb = 0, bphase = 0;                  // packed-bit ring position / parity
         int pending = -1;                             // ring stage written but not yet published
         const uint32_t row_smem = smem0 + (isA ? 0 : T::OFF_B) + (r >> 3) * 1024 + (r & 7) * 128;
@@ -500,28 +507,10 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 epi_I = -1;
             }
             const int epi_at = kb_begin + TC_GROUP * (min(prefill, (kb_end - kb_begin) / TC_GROUP) - 1);
-            for (int kb0 = kb_begin; kb0 < kb_end; kb0 += TC_GROUP) {
-                const uint32_t stage = pset + 2 * sl;
-                const int kb = kb0 + pset;
-                uint32_t w[WORDS];
-                uint32_t bits_release = 0;
-                if (dbg & 32) {                               // ablation: no packed-bit ring
-#pragma unroll
-                    for (int m = 0; m < WORDS; ++m) w[m] = 0x01234567u * (m + kb);
-                } else {
-                mbar_wait(bits_full0 + 8 * bb, bphase);
-                {
-                    const uint4 v0 = lds128(bits_row + bb * T::BITS_BUF_BYTES + bits_c0);
-                    w[0] = v0.x; w[1] = v0.y; w[2] = v0.z; w[3] = v0.w;
-                    if (KIND == KIND_FP4) {
-                        const uint4 v1 = lds128(bits_row + bb * T::BITS_BUF_BYTES + bits_c1);
-                        w[WORDS - 4] = v1.x; w[WORDS - 3] = v1.y; w[WORDS - 2] = v1.z; w[WORDS - 1] = v1.w;
-                    }
-                }
-                bits_release = bits_empty0 + 8 * bb;          // handed back to the TMA thread after this stage's stores
-                if (++bb == T::BITS_BUFS) { bb = 0; bphase ^= 1; }
-                }
-                if (isA) {
+            // One stage of one row: open-range mask, expansion, publish of this warp's previous stage, store.
+            auto do_stage = [&](int kb, uint32_t stage, uint32_t eparity, uint32_t (&w)[WORDS]) {
+                if (dbg & 256) {                              // ablation: no open-range masks
+                } else if (isA) {
                     if (kb <= kbA) {                          // keep k > i
                         const int rl = 256 * I + rt - COLS * kb;
 #pragma unroll
@@ -532,7 +521,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
 #pragma unroll
                     for (int m = 0; m < WORDS; ++m) w[m] &= keep_lt(lim, m);
                 }
-                const bool slot_free = (dbg & 64) ? true : mbar_try(empty0 + 8 * stage, sphase ^ 1);   // 64: free-running producers
+                const bool slot_free = (dbg & 64) ? true : mbar_try(empty0 + 8 * stage, eparity);   // 64: free-running producers
                 uint4 o[8];
                 if (dbg & 2) {                                // ablation: no expansion arithmetic
 #pragma unroll
@@ -544,14 +533,14 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
 #pragma unroll
                     for (int m = 0; m < 4; ++m) unpack_word<TB>(w[m], o[2 * m], o[2 * m + 1]);
                 }
-                if (pending >= 0) {                           // publish this set's previous stage to the leader's MMA thread
+                if (pending >= 0) {                           // publish this warp's previous stage to the leader's MMA thread
                     if (dbg & 16) {}                          // ablation: no fence before the publish
                     else if (a_tmem) tmem_wait_st_after(o);
                     else fence_proxy_async_smem_after(o);
                     __syncwarp();
                     if (lane == 0 && !(dbg & 64)) mbar_arrive_cluster(full_leader0 + 8 * pending);
                 }
-                if (!slot_free) mbar_wait(empty0 + 8 * stage, sphase ^ 1);
+                if (!slot_free) mbar_wait(empty0 + 8 * stage, eparity);
                 if (dbg & 4) {                                 // ablation: no operand stores
                 } else if (a_tmem) {
                     tc_fence_after();                          // the MMAs that read this TMEM slot have completed
@@ -562,18 +551,77 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                     for (int c = 0; c < 8; ++c) sts128(rowp + ((c ^ sw) << 4), o[c]);
                 }
                 pending = (int)stage;
-                if (++sl == T::STAGES / 2) { sl = 0; sphase ^= 1; }
-                // Release the packed-bit buffer only now.  The operand stores above consume every word loaded from
-                // it, so the hardware has issued them after the LDS data arrived; an arrive placed right after the LDS
-                // instructions is NOT ordered after their completion (naming the loaded registers as unused asm
-                // operands creates no dependency in the machine code), and with the ring full the TMA thread then
-                // refills the buffer at once: when the shared-memory pipe is backed up (the epilogue's histogram
-                // atomics of slower warps) the delayed LDS returned the bits of the group four ahead.  Seen as a
-                // handful of wrong n_ij per 10^10 pairs at config 4, and as thousands when the epilogue of a tile
-                // overlapped the first stages of the next; located by dumping every n_ij and matching the wrong
-                // rows against "same row, packed bits of the stage 8 later".
-                __syncwarp();
-                if (bits_release != 0 && lane == 0) mbar_arrive(bits_release);
+            };
+            for (int kb0 = kb_begin; kb0 < kb_end; kb0 += TC_GROUP) {
+                // The packed-bit buffer is released only after the operand stores that consume every word loaded from
+                // it: the hardware has then issued them after the LDS data arrived.  An arrive placed right after the
+                // LDS instructions is NOT ordered after their completion (naming the loaded registers as unused asm
+                // operands creates no dependency in the machine code), and with the ring full the TMA thread refills
+                // the buffer at once: when the shared-memory pipe was backed up (the epilogue's histogram atomics of
+                // slower warps) the delayed LDS returned the bits of the group four ahead.  Seen as a handful of wrong
+                // n_ij per 10^10 pairs at config 4, and as thousands when the epilogue of a tile overlapped the first
+                // stages of the next; located by dumping every n_ij and matching the wrong rows against "same row,
+                // packed bits of the stage 8 later".
+                if (TC_WHOLE_GROUP) {
+                    // set p expands BOTH stages of every second group: one buffer wait, one release and one pass
+                    // through the loop overhead per two stages
+                    if ((int)(gsel & 1u) == pset) {
+                        uint32_t w0[WORDS], w1[WORDS];
+                        const bool ring = !(dbg & 32);
+                        if (ring) {
+                            mbar_wait(bits_full0 + 8 * bb, bphase);
+                            const uint32_t base = bits_row + bb * T::BITS_BUF_BYTES;
+                            if (KIND == KIND_FP4) {
+                                const uint32_t z = (prow >> 1) & 3;
+                                const uint4 v0 = lds128(base + ((0u ^ z) << 4)), v1 = lds128(base + ((1u ^ z) << 4));
+                                const uint4 v2 = lds128(base + ((2u ^ z) << 4)), v3 = lds128(base + ((3u ^ z) << 4));
+                                w0[0] = v0.x; w0[1] = v0.y; w0[2] = v0.z; w0[3] = v0.w;
+                                w0[WORDS - 4] = v1.x; w0[WORDS - 3] = v1.y; w0[WORDS - 2] = v1.z; w0[WORDS - 1] = v1.w;
+                                w1[0] = v2.x; w1[1] = v2.y; w1[2] = v2.z; w1[3] = v2.w;
+                                w1[WORDS - 4] = v3.x; w1[WORDS - 3] = v3.y; w1[WORDS - 2] = v3.z; w1[WORDS - 1] = v3.w;
+                            } else {
+                                const uint32_t z = (prow >> 2) & 1;
+                                const uint4 v0 = lds128(base + ((0u ^ z) << 4)), v1 = lds128(base + ((1u ^ z) << 4));
+                                w0[0] = v0.x; w0[1] = v0.y; w0[2] = v0.z; w0[3] = v0.w;
+                                w1[0] = v1.x; w1[1] = v1.y; w1[2] = v1.z; w1[3] = v1.w;
+                            }
+                        } else {
+#pragma unroll
+                            for (int m = 0; m < WORDS; ++m) { w0[m] = 0x01234567u * (m + kb0); w1[m] = 0x089abcdu * (m + kb0); }
+                        }
+                        do_stage(kb0, slot0, spar ^ 1, w0);
+                        do_stage(kb0 + 1, slot0 + 1, spar ^ 1, w1);
+                        __syncwarp();
+                        if (ring && lane == 0) mbar_arrive(bits_empty0 + 8 * bb);
+                    }
+                    ++gsel;
+                    slot0 += 2;
+                    if (slot0 == (uint32_t)T::STAGES) { slot0 = 0; spar ^= 1; }
+                    if (++bb == T::BITS_BUFS) { bb = 0; bphase ^= 1; }
+                } else {
+                    const uint32_t stage = pset + 2 * sl;
+                    const int kb = kb0 + pset;
+                    uint32_t w[WORDS];
+                    uint32_t bits_release = 0;
+                    if (dbg & 32) {                               // ablation: no packed-bit ring
+#pragma unroll
+                        for (int m = 0; m < WORDS; ++m) w[m] = 0x01234567u * (m + kb);
+                    } else {
+                        mbar_wait(bits_full0 + 8 * bb, bphase);
+                        const uint4 v0 = lds128(bits_row + bb * T::BITS_BUF_BYTES + bits_c0);
+                        w[0] = v0.x; w[1] = v0.y; w[2] = v0.z; w[3] = v0.w;
+                        if (KIND == KIND_FP4) {
+                            const uint4 v1 = lds128(bits_row + bb * T::BITS_BUF_BYTES + bits_c1);
+                            w[WORDS - 4] = v1.x; w[WORDS - 3] = v1.y; w[WORDS - 2] = v1.z; w[WORDS - 1] = v1.w;
+                        }
+                        bits_release = bits_empty0 + 8 * bb;
+                        if (++bb == T::BITS_BUFS) { bb = 0; bphase ^= 1; }
+                    }
+                    do_stage(kb, stage, sphase ^ 1, w);
+                    if (++sl == T::STAGES / 2) { sl = 0; sphase ^= 1; }
+                    __syncwarp();
+                    if (bits_release != 0 && lane == 0) mbar_arrive(bits_release);
+                }
                 if (epi_I >= 0 && kb0 == epi_at) {             // the previous tile's epilogue, after the prefill
                     publish_pending();
                     epilogue(epi_I, epi_J);
