@@ -55,3 +55,22 @@ def test_pack_dense_roundtrip():
     up, bits = csg_inputs.random_poset_bits(130, 0.2, seed=0)
     B = unpack(bits, 130)[:, :130]
     assert (np.triu(B, 1) == up).all() and (B == B.T).all()
+
+
+def test_golden_histogram_file_is_what_the_oracle_writes():
+    """tests/golden/config_histograms.txt (used by the GPU parity tests at the large configs) is the output of
+    tests/golden/make_config_goldens.py, which calls only the oracle: regenerate the cheap line (config 1) and
+    compare; check that every line is tied to the bitset the generator produces for that config name."""
+    import importlib.util
+    import os
+    here = os.path.dirname(os.path.abspath(__file__))
+    spec = importlib.util.spec_from_file_location("make_config_goldens", os.path.join(here, "golden", "make_config_goldens.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    stored = {ln.split()[0]: ln.strip() for ln in open(mod.OUT) if ln.strip() and not ln.startswith("#")}
+    assert mod.line_for(1) == stored[csg_inputs.CONFIGS[1]["name"]]
+    names = {c["name"]: c for c in csg_inputs.CONFIGS}
+    for name, ln in stored.items():
+        f = ln.split()
+        assert name in names and int(f[1]) == names[name]["N"] and int(f[2]) == names[name]["N"] - 2
+        assert len(f[4]) == 64 and int(f[5]) >= sum(int(x) for x in f[6:14])
