@@ -399,7 +399,7 @@ static int action_device(const uint64_t* rel_bits, long long N, int dim, double 
 // copies of all but the first chunks hide behind the tiles of the chunks before them: the 2 GiB copy of N = 131072
 // (38 ms over PCIe) costs a few ms instead.  Tensor variants and large matrices only; counts must be zeroed by the
 // caller of this function on `stream` beforehand (done here).
-constexpr int HOST_CHUNKS = 16;
+constexpr int HOST_CHUNKS = 32;
 constexpr long long HOST_PIPELINE_MIN_BYTES = 32LL << 20;
 
 static int ensure_chunk_tiles(long long N, cudaStream_t stream) {
