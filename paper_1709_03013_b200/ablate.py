@@ -1,0 +1,50 @@
+"""Timing ablations of the fp4 tensor kernel (developer aid; profiles/r1f… and r1g… quote its output).
+
+    python -m paper_1709_03013_b200.ablate --config 2 --debug 0,14,9,63,64
+
+For every value of --debug the environment variable CSG_DEBUG is set, which makes csg_action launch the ABLATE
+instantiation of tensor_action_kernel with parts switched off (bits: 1 no MMA issue, 2 no expansion arithmetic, 4 no
+operand stores, 8 no epilogue work, 16 no fence before publishing a stage, 32 no packed-bit ring, 64 free-running
+producers, 128 no prefill before the epilogue, 256 no open-range masks; any non-zero value gives WRONG counts), and the
+CUDA-event time of the interval kernel (csg_last_kernel_ms) of four calls is printed.  Needs a B200.
+"""
+import argparse
+import os
+import sys
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def main():
+    import torch
+    import csg_inputs
+    import paper_1709_03013_b200 as csg
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--config", type=int, default=2, help="index into csg_inputs.CONFIGS")
+    ap.add_argument("--debug", default="0,14,9,63,64", help="comma-separated CSG_DEBUG values")
+    ap.add_argument("--runs", type=int, default=4)
+    args = ap.parse_args()
+    csg.load()
+    cfg = csg_inputs.CONFIGS[args.config]
+    N, dim = cfg["N"], cfg["dim"]
+    _, bits = csg_inputs.make_config(cfg)
+    d = csg.to_device(bits)
+    csg.csg_set_variant(csg.VARIANT_TENSOR_FP4)
+    csg.csg_set_kernel_timing(True)
+    for dbg in [int(x) for x in args.debug.split(",")]:
+        os.environ["CSG_DEBUG"] = str(dbg)
+        ms = []
+        for _ in range(args.runs):
+            csg.csg_action(d, N, dim, 1.0, 3)
+            torch.cuda.synchronize()
+            ms.append(csg.csg_last_kernel_ms())
+        print("%s CSG_DEBUG=%-4d kernel ms %s" % (cfg["name"], dbg, " ".join("%.3f" % m for m in ms)), flush=True)
+    os.environ.pop("CSG_DEBUG", None)
+    csg.csg_set_kernel_timing(False)
+    csg.csg_set_variant(csg.VARIANT_AUTO)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,54 @@
+"""Repeated launches: the full histogram must be identical to the oracle's on every run, through the device-resident
+call and through the chunked host call.  (A race between the packed-bit ring's LDS reads and the TMA refill once lost
+a handful of n_ij per 10^10 pairs; it only showed under repetition or at the largest configuration.)"""
+import numpy as np
+import pytest
+
+import csg_inputs
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def csg():
+    import paper_1709_03013_b200 as m
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    if m._build.needs_build():
+        m.build()
+    m.load()
+    m.csg_set_variant(m.VARIANT_AUTO)
+    return m
+
+
+@pytest.mark.parametrize("dim,N,reps", [(2, 16384, 12), (4, 16384, 8), (2, 9000, 12)])
+def test_repeated_full_histograms(csg, dim, N, reps):
+    _, bits = csg_inputs.make_causet(dim, N, 777 + N)
+    want = oracle.alg5_counts(bits, N, N - 2)
+    d = csg.to_device(bits)
+    pinned = torch.from_numpy(bits.view(np.int64)).pin_memory()
+    for r in range(reps):
+        c, _ = csg.csg_action(d, N, dim, 1.0, N - 2)
+        torch.cuda.synchronize()
+        assert (c.cpu().numpy() == want).all(), ("device", r)
+        ch, _ = csg.csg_action_host(pinned, N, dim, 1.0, N - 2)
+        assert (ch == want).all(), ("host", r)
+
+
+@pytest.mark.slow
+def test_config4_is_run_to_run_identical(csg):
+    cfg = csg_inputs.CONFIGS[4]
+    N = cfg["N"]
+    _, bits = csg_inputs.make_config(cfg)
+    d = csg.to_device(bits)
+    first = None
+    for r in range(3):
+        c, S = csg.csg_action(d, N, 2, cfg["eps"], N - 2)
+        torch.cuda.synchronize()
+        c = c.cpu().numpy()
+        if first is None:
+            first = (c, float(S.item()))
+        else:
+            assert (c == first[0]).all() and float(S.item()) == first[1], r
