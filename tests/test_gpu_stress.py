@@ -52,3 +52,19 @@ def test_config4_is_run_to_run_identical(csg):
             first = (c, float(S.item()))
         else:
             assert (c == first[0]).all() and float(S.item()) == first[1], r
+
+
+@pytest.mark.slow
+def test_config4_int8_kind_equals_fp4_kind(csg):
+    """N = 262144 is the only configuration that takes the int8 kind's TB = 6 operand encoding (n_ij << 12 in s32)."""
+    cfg = csg_inputs.CONFIGS[4]
+    N = cfg["N"]
+    _, bits = csg_inputs.make_config(cfg)
+    d = csg.to_device(bits)
+    csg.csg_set_variant(csg.VARIANT_TENSOR_FP4)
+    a, Sa = csg.csg_action(d, N, 2, cfg["eps"], N - 2)
+    csg.csg_set_variant(csg.VARIANT_TENSOR)
+    b, Sb = csg.csg_action(d, N, 2, cfg["eps"], N - 2)
+    torch.cuda.synchronize()
+    csg.csg_set_variant(csg.VARIANT_AUTO)
+    assert torch.equal(a, b) and float(Sa.item()) == float(Sb.item())
