@@ -137,9 +137,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
         "{\n\t.reg .pred p;\n\t"
         "WAIT_%=:\n\t"
         "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-        "@p bra DONE_%=;\n\t"
-        "bra WAIT_%=;\n\t"
-        "DONE_%=:\n\t}" ::"r"(bar), "r"(parity) : "memory");
+        "@!p bra WAIT_%=;\n\t}" ::"r"(bar), "r"(parity) : "memory");   // one branch, not taken when the phase is complete
 }
 // One non-blocking probe of the barrier phase; lets the caller overlap the probe latency with other work.
 __device__ __forceinline__ bool mbar_try(uint32_t bar, uint32_t parity) {
