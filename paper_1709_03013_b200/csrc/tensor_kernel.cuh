@@ -6,31 +6,41 @@
 // masked by R[i][j] -- a dense contraction over k, so it runs on the 5th-generation tensor cores:
 //
 //   * a cluster of two CTAs (one SM pair) owns a 256 x 256 tile of pairs (rows i of block I, rows j of block J)
-//     and sweeps K from the first column of block I to the last column of block J in stages of 128 columns.
-//     CTA rank p holds rows i0+128p.. of the A operand and rows j0+128p.. of the B operand, so each SM expands
-//     256 rows per stage for a 256 x 256 x 128 product (the single-CTA form needed 384 rows per 128 x 256 x 128),
-//     and each tensor core reads half of B from its own shared memory and half from its peer's;
-//   * per CTA one TMA thread streams the packed bits of its 256 rows (32 bytes = 2 stages per row per copy,
-//     32-byte-swizzled 2D boxes of 128 rows) into a 4-deep shared-memory ring: whole sectors, one issuing thread;
-//   * 16 producer warps in two sets of 8 (one row per thread; set p takes stage p of every 2-stage copy) read 16
-//     bytes per stage from that ring, expand the bits to bytes (0 or 1 << TB) and store them into a 4-stage
-//     ring of K-major, 128-byte-swizzled operand tiles.  The order
-//     of the 32 k's inside a 32-bit word is permuted (bits q, q+8, q+16, q+24 share one 32-bit store); both
-//     operands use the same permutation and the MMA sums over k, so the result is unchanged;
-//   * one thread of the leader CTA issues tcgen05.mma.cta_group::2.kind::i8 (M=256, N=256, K=32, u8 x u8 -> s32,
-//     exact) four times per stage; each CTA's 128 accumulator rows live in 256 columns of its own TMEM;
-//     tcgen05.commit (multicast) hands the stage back to the producers of both CTAs;
-//   * the open range i<k<j costs nothing in the steady state: only the first two stages of a tile (columns of
-//     block I) need the k>i mask and only the last two (columns of block J) need the k<j mask;
-//   * fused epilogue: the producer warps read their CTA's accumulators back with tcgen05.ld, test bit R[i][j]
-//     (and i<j), and bucket n_ij into a privatised shared-memory histogram (low bins) or straight into the
-//     global counts (high bins, smeared action only).  No N x N count matrix ever reaches HBM.
+//     and sweeps K from the first column of block I to the last column of block J in stages of 128 (int8 kind)
+//     or 256 (fp4 kind) columns.  CTA rank p holds rows i0+128p.. of the A operand and rows j0+128p.. of the B
+//     operand, so each SM expands 256 rows per stage for a 256 x 256 x stage product, and each tensor core reads
+//     half of B from its own shared memory and half from its peer's;
+//   * per CTA one TMA thread streams the packed bits of its 256 rows (one copy = a group of 2 stages per row,
+//     32- or 64-byte-swizzled 2D boxes of 128 rows) into a 4-deep shared-memory ring: whole sectors, one issuing
+//     thread; rows >= N and columns beyond the row are zero-filled by the TMA unit;
+//   * 16 producer warps in two sets of 8, one row per thread.  Set p expands both stages of every second group
+//     (TC_WHOLE_GROUP; the older split "set p takes stage p of every group" remains as a compile-time option):
+//     LDS.128 of the row's bits -> open-range mask where needed -> shifts/ANDs -> operand tile.  The B tile is a
+//     K-major, 128-byte-swizzled shared-memory tile (UMMA canonical layout); the A tile is the same for the int8
+//     kind and lives in TMEM for the fp4 kind (tcgen05.st, lane = row; see TcTraits).  The order of the k's
+//     inside a 32-bit word is permuted identically for both operands; the MMA sums over k, so nothing changes.
+//     The packed-bit buffer goes back to the TMA thread only after the stores that consume its words (see the
+//     comment in the stage loop: an arrive placed right after the LDS instructions was a race);
+//   * one thread of the leader CTA issues tcgen05.mma.cta_group::2 four times per stage (kind::i8: u8 x u8 -> s32;
+//     kind::mxf4 with unit block scales: e2m1 x e2m1 -> f32 holding exact integers); each CTA's 128 accumulator
+//     rows live in 256 columns of its own TMEM; tcgen05.commit (multicast) hands the stage back to the producers
+//     of both CTAs.  Operand ring: 4 stages (int8), 6 stages (fp4);
+//   * the open range i<k<j costs nothing in the steady state: only the stages that overlap block I need the k>i
+//     mask and only those that overlap block J the k<j mask;
+//   * fused epilogue by the producer warps: tcgen05.ld of their CTA's accumulators, bit R[i][j] (and i<j), n_ij
+//     into a privatised shared-memory histogram (bins < 2048) or straight into the global counts (higher bins,
+//     smeared action only).  The first two groups of the NEXT tile are expanded before the epilogue of a tile, so
+//     the tensor cores restart as soon as the accumulators are drained.  No N x N count matrix ever reaches HBM.
 //
-// `dbg` (env CSG_DEBUG, default 0; a separate ABLATE instantiation of the fp4 kernel) switches parts of the kernel off for timing ablations (1: no MMA issue, 2: no
-// expansion arithmetic, 4: no operand stores, 8: no epilogue work, 16: no fence before publishing a stage, 32: no packed-bit ring, 128: no prefill of the next tile before an epilogue, 64: producers free-running, no MMA thread, no epilogue); any non-zero value gives wrong counts.
+// `dbg` (env CSG_DEBUG, default 0; a separate ABLATE instantiation of the fp4 kernel, see
+// paper_1709_03013_b200/ablate.py) switches parts of the kernel off for timing ablations (1: no MMA issue, 2: no
+// expansion arithmetic, 4: no operand stores, 8: no epilogue work, 16: no fence before publishing a stage, 32: no
+// packed-bit ring, 64: producers free-running with no MMA thread and no epilogue, 128: no prefill of the next tile
+// before an epilogue, 256: no open-range masks); any non-zero value gives wrong counts.
 //
-// Tiles are handed out statically from a list sorted by K-depth, longest first, in boustrophedon order over
-// the persistent clusters (one per SM pair), which balances the triangular workload without a global counter.
+// Tiles come from a host-built list (csg.cu: build_tile_schedule: deepest first, for large matrices in L2-sized
+// patches) and are dealt in boustrophedon order over the persistent clusters (one per SM pair), which balances
+// the triangular workload without a global counter.
 #pragma once
 #include <cuda.h>
 
