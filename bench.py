@@ -272,7 +272,7 @@ def run_ours(args, cfg, rank, local_rank, world):
     for _ in range(e2e_steps):
         c_host, S_host = csg.csg_action_host(host, N, dim, eps, kmax)
     e2e_s = time.perf_counter() - t0
-    assert (c_host == result_counts).all() and S_host == result_S, "e2e and device legs disagree"
+    checks = {"e2e_equals_device": bool((c_host == result_counts).all() and S_host == result_S)}
 
     # ---- linking leg: coordinates -> relation matrix on the device, then coordinates -> action
     geom = (csg.GEOM_DESITTER_2D if cfg.get("geometry") == "ds2" else
@@ -288,7 +288,7 @@ def run_ours(args, cfg, rank, local_rank, world):
         if it >= args.warmup:
             link_ms.append(csg.csg_last_link_ms())
     csg.csg_set_kernel_timing(False)
-    assert torch.equal(d_linked, d_bits), "device-linked matrix differs from the host generator's"
+    checks["linked_matrix_equals_generator"] = bool(torch.equal(d_linked, d_bits))
     del d_linked
     csg.csg_causet_action_host(coords_pinned, N, geom, eps, kmax)   # warm-up (library-owned matrix buffer)
     barrier()
@@ -296,7 +296,10 @@ def run_ours(args, cfg, rank, local_rank, world):
     for _ in range(e2e_steps):
         c2_host, S2_host = csg.csg_causet_action_host(coords_pinned, N, geom, eps, kmax)
     e2e_coords_s = time.perf_counter() - t0
-    assert (c2_host == result_counts).all() and S2_host == result_S, "coordinates-in leg disagrees"
+    checks["coords_in_equals_device"] = bool((c2_host == result_counts).all() and S2_host == result_S)
+    for name, ok in checks.items():
+        if not ok:
+            print("bench.py: CHECK FAILED: %s" % name, file=sys.stderr, flush=True)
 
     # ---- batched small sets: 64 causal sets of BASELINE.json configs[0]'s shape in one call
     batch_leg = None
@@ -398,6 +401,7 @@ def run_ours(args, cfg, rank, local_rank, world):
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": N * csg.csg_row_stride_words(N) * 8,
                 "d2h_bytes_per_step": (kmax + 1) * 8 + 8, "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps},
         "gpu_launches": launches,
+        "checks": checks,   # the legs of this run agree with each other (parity with the oracle is the tests' job)
         "roofline": roofline,
         "cpu_baseline": cpu_baseline,
     }
