@@ -116,6 +116,7 @@ struct State {
     size_t d_counts_bytes = 0;
     double* d_S = nullptr;
     double* d_coords = nullptr;
+    unsigned int* d_progress = nullptr;     // finished-tile counter of the running tensor launch (drift throttle)
     size_t d_coords_bytes = 0;
     // pipelined host path: row chunks copied on copy_stream, each chunk's tiles launched as soon as it landed
     cudaStream_t copy_stream = nullptr;
@@ -300,6 +301,7 @@ static int ensure_tensor_ready(int kind, const uint64_t* rel_bits, long long N, 
         CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_I8, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, s8));
         CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_FP4, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, s4));
         CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_FP4, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, s4));
+        CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_FP4, 0, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, s4));
         g.attr_set = true;
     }
     return CSG_OK;
@@ -309,6 +311,18 @@ static int ensure_tensor_ready(int kind, const uint64_t* rel_bits, long long N, 
 static int launch_tensor(int kind, const uint64_t* rel_bits, long long N, long long stride, int kmax, long long* counts,
                          const int2* d_tiles, int ntiles, cudaStream_t stream) {
     const int grid = 2 * std::max(1, std::min(ntiles, g.sm_count / 2));   // one CTA pair per SM pair
+    // Drift throttle (tensor_kernel.cuh, TC_MAX_LEAD).  Measured: config 4 (N = 262144, full histogram) 1022 -> 929 ms,
+    // DRAM reads 2.55 -> 0.67 TB per launch, SM clock under the power cap 1.67 -> 1.86 GHz; config 3 (kmax = 3)
+    // 106.6 -> 107.5 ms, the de Sitter workload (N = 131072, full histogram) 109.9 -> 111.4 ms.  So it is switched on
+    // only for matrices of more than 4 GiB, where a cluster walks through thousands of rounds.
+    unsigned int* progress = nullptr;
+    const bool drifts = kind == KIND_FP4 && N * stride * 8 > (4LL << 30);
+    if (drifts && ntiles > 16 * (grid / 2) && !getenv("CSG_NO_THROTTLE")) {
+        // a ring of counters, one per launch, so that launches in flight on different streams do not share one
+        if (!g.d_progress) CSG_CUDA(cudaMalloc(&g.d_progress, 64 * sizeof(unsigned int)));
+        progress = g.d_progress + (g.launches & 63);
+        CSG_CUDA(cudaMemsetAsync(progress, 0, sizeof(unsigned int), stream));
+    }
     unsigned long long* c64 = reinterpret_cast<unsigned long long*>(counts);
     const char* dbg_env = getenv("CSG_DEBUG");
     const int dbg = dbg_env ? atoi(dbg_env) : 0;
@@ -316,17 +330,19 @@ static int launch_tensor(int kind, const uint64_t* rel_bits, long long N, long l
     // int8: operand bit TB: the accumulator holds n_ij << 2TB and n_ij <= N-2, so TB is the largest with
     // (N-2) << 2TB < 2^31; TB = 7 turns every unpack shift into a left shift (FMA pipe).
     if (kind == KIND_FP4 && dbg != 0)   // timing ablations only (wrong counts)
-        tensor_action_kernel<KIND_FP4, 0, true><<<grid, TC_THREADS, s4, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, d_tiles, ntiles, dbg);
+        tensor_action_kernel<KIND_FP4, 0, true><<<grid, TC_THREADS, s4, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, d_tiles, ntiles, dbg, progress);
+    else if (kind == KIND_FP4 && progress != nullptr)
+        tensor_action_kernel<KIND_FP4, 0, false, true><<<grid, TC_THREADS, s4, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, d_tiles, ntiles, dbg, progress);
     else if (kind == KIND_FP4)
-        tensor_action_kernel<KIND_FP4, 0><<<grid, TC_THREADS, s4, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, d_tiles, ntiles, dbg);
+        tensor_action_kernel<KIND_FP4, 0><<<grid, TC_THREADS, s4, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, d_tiles, ntiles, dbg, progress);
     else if (N - 2 < (1LL << 17))
-        tensor_action_kernel<KIND_I8, 7><<<grid, TC_THREADS, s8, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, d_tiles, ntiles, dbg);
+        tensor_action_kernel<KIND_I8, 7><<<grid, TC_THREADS, s8, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, d_tiles, ntiles, dbg, progress);
     else if (N - 2 < (1LL << 19))
-        tensor_action_kernel<KIND_I8, 6><<<grid, TC_THREADS, s8, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, d_tiles, ntiles, dbg);
+        tensor_action_kernel<KIND_I8, 6><<<grid, TC_THREADS, s8, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, d_tiles, ntiles, dbg, progress);
     else if (N - 2 < (1LL << 21))
-        tensor_action_kernel<KIND_I8, 5><<<grid, TC_THREADS, s8, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, d_tiles, ntiles, dbg);
+        tensor_action_kernel<KIND_I8, 5><<<grid, TC_THREADS, s8, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, d_tiles, ntiles, dbg, progress);
     else
-        tensor_action_kernel<KIND_I8, 4><<<grid, TC_THREADS, s8, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, d_tiles, ntiles, dbg);
+        tensor_action_kernel<KIND_I8, 4><<<grid, TC_THREADS, s8, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, d_tiles, ntiles, dbg, progress);
     CSG_CUDA(cudaGetLastError());
     ++g.launches;
     return CSG_OK;
@@ -786,6 +802,8 @@ int csg_shutdown(void) {
     if (g.d_counts) cudaFree(g.d_counts);
     if (g.d_S) cudaFree(g.d_S);
     if (g.d_coords) cudaFree(g.d_coords);
+    if (g.d_progress) cudaFree(g.d_progress);
+    g.d_progress = nullptr;
     if (g.d_chunk_tiles) cudaFree(g.d_chunk_tiles);
     g.d_chunk_tiles = nullptr;
     g.chunk_N = -1;

@@ -66,6 +66,7 @@ constexpr int TC_THREADS = TC_PRODUCERS + 64;  // + the MMA warp + the TMA warp
 #define CSG_WHOLE_GROUP 1
 #endif
 constexpr bool TC_WHOLE_GROUP = CSG_WHOLE_GROUP != 0;   // a producer set expands both stages of every second group
+constexpr int TC_MAX_LEAD = 1;                 // rounds a cluster may run ahead of the average (L2 sharing inside a patch)
 constexpr int TC_PREFILL_GROUPS = 2;           // groups (2 stages each) of the next tile expanded before a tile's epilogue
 constexpr int TC_HIST = 2048;              // privatised low bins per CTA
 
@@ -350,11 +351,12 @@ __device__ __forceinline__ void tile_k_range(int I, int J, int& kb_begin, int& k
 // 4^TB, the accumulator holds n_ij << 2TB; the host picks the largest TB with (N-2) << 2TB < 2^31 (exact in s32).
 // KIND_FP4: TB unused (pass 0); the f32 accumulator holds 4 n_ij, exact for n_ij < 2^22.
 // tiles[t] = {I, J}: 256-row blocks, I <= J.  Grid = 2 x (number of SM pairs), cluster (2,1,1).
-template <int KIND, int TB, bool ABLATE = false>
+template <int KIND, int TB, bool ABLATE = false, bool THROTTLE = false>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(TC_THREADS, 1)
 tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_t* __restrict__ rel, long long N,
                      long long stride_words, int kmax, unsigned long long* __restrict__ counts,
-                     const int2* __restrict__ tiles, int ntiles, int dbg_arg) {
+                     const int2* __restrict__ tiles, int ntiles, int dbg_arg, unsigned int* __restrict__ progress_arg) {
+    unsigned int* const progress = THROTTLE ? progress_arg : nullptr;   // compiled out of the instantiations that do not throttle
     using T = TcTraits<KIND>;
     const int dbg = ABLATE ? dbg_arg : 0;             // compiled out of the production instantiation
     constexpr int COLS = T::STAGE_COLS, WORDS = T::WORDS;
@@ -490,6 +492,8 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive_cluster(tmem_empty_leader);
+            // one count per finished tile of this cluster (throttle of the TMA threads, see below)
+            if (progress != nullptr && rank == 0 && tid == 0) atomicAdd(progress, 1u);
         };
 
         for (int rd = 0; rd < rounds; ++rd) {
@@ -697,6 +701,16 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 const int ia = tile.x * TC_T + 128 * (int)rank, jb = tile.y * TC_T + 128 * (int)rank;
                 int kb_begin, kb_end;
                 tile_k_range<COLS>(tile.x, tile.y, kb_begin, kb_end);
+                // Keep the clusters within TC_MAX_LEAD rounds of the average: the schedule has no barrier between rounds,
+                // and with a slow, variable epilogue (full histogram) the clusters of a patch drift apart until none of
+                // them shares row segments in L2 any more (config 4: 2.55 TB of DRAM reads per launch, L2 hit rate
+                // 38 %).  A cluster starts round rd only when (rd - TC_MAX_LEAD) * G tiles are finished in total; the
+                // slowest cluster never waits (everybody else has finished at least as many), so no deadlock, and the
+                // makespan of the static deal is unchanged.  Only the TMA thread polls; everything downstream starves.
+                if (progress != nullptr && rd > TC_MAX_LEAD) {
+                    const unsigned int need = (unsigned int)(rd - TC_MAX_LEAD) * (unsigned int)G;
+                    while (*reinterpret_cast<volatile unsigned int*>(progress) < need) __nanosleep(200);
+                }
                 for (int kb0 = kb_begin; kb0 < ((dbg & 32) ? kb_begin : kb_end); kb0 += TC_GROUP) {
                     mbar_wait(bits_empty0 + 8 * bb, bphase ^ 1);
                     const uint32_t bar = bits_full0 + 8 * bb;
