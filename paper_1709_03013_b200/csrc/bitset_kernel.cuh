@@ -101,8 +101,10 @@ bitset_action_kernel(const uint32_t* __restrict__ rel, long long N, long long st
                 *reinterpret_cast<uint4*>(&sB[r * BS_LD + 4 * (tid & 7)]) = vb;
             }
             __syncthreads();
+            // only the 128-bit quads that hold columns of this tile's K range (short ranges dominate at small N)
+            const int nq = (int)min((long long)(BS_KW / 4), (kw_end - kw0 + 3) >> 2);
 #pragma unroll 2
-            for (int kq = 0; kq < BS_KW / 4; ++kq) {
+            for (int kq = 0; kq < nq; ++kq) {
                 uint4 a4[4], b4[4];
 #pragma unroll
                 for (int a = 0; a < 4; ++a)
