@@ -64,7 +64,8 @@ int64_t csg_row_stride_words(int64_t N);
 
 /*
  * Interval abundances and action of one causal set.  All work is enqueued on `stream`; no host
- * synchronisation happens inside (the first call for a new N also builds the cached tile schedule).
+ * synchronisation happens inside (the first call for a new N also builds the cached tile schedule; after that
+ * warm-up call the function only enqueues a memset and two kernels and can be captured in a CUDA graph).
  *
  *   rel_bits DEVICE, N*csg_row_stride_words(N) words, layout above, 16-byte aligned, read only.
  *   N        number of elements, 1 <= N <= CSG_MAX_N (N = 1, 2 are valid: no triples).
