@@ -1,7 +1,7 @@
 """ORACLE package -- test infrastructure only.
 
 Plain CPU restatement of the paper's hot path (PAPER.md:395 naive action algorithm; Eq. 4 / Eq. 5;
-Algorithm 5; dense linking).  Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+Algorithm 5; dense linking; 2D orders from coordinates).  Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
 ``--impl reference`` legs may import this package.  It never imports ``paper_1709_03013_b200``.
 """
 from .oracle import (  # noqa: F401
@@ -18,6 +18,9 @@ from .oracle import (  # noqa: F401
     alg5_counts,
     alg5_counts_rows,
     alg5_threads,
+    dominance2d_counts,
+    dominance2d_counts_rows,
+    dominance2d_relations,
     link,
     GEOM_MINKOWSKI_2D,
     GEOM_MINKOWSKI_4D,

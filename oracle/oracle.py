@@ -12,7 +12,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "liboracle.so")
 _SRCS = [os.path.join(_HERE, "csg_oracle.c"), os.path.join(_HERE, "alg5_packed.c"),
-         os.path.join(_HERE, "link_oracle.c")]
+         os.path.join(_HERE, "link_oracle.c"), os.path.join(_HERE, "dominance2d.c")]
 _lib = None
 
 _i64 = ctypes.c_int64
@@ -22,11 +22,13 @@ _p_i64 = np.ctypeslib.ndpointer(dtype=np.int64, flags="C_CONTIGUOUS")
 
 
 def build(force=False):
-    """Compile the oracle with gcc (plain -O2; OpenMP only drives Algorithm 5's pair loop)."""
+    """Compile the oracle with gcc (plain -O2; OpenMP only drives the pair loops of Algorithm 5 and of the
+    coordinate route; -mpopcnt because Algorithm 5's bit count IS the popcnt instruction, Alg. 3 --
+    without it gcc calls a table routine and the restated algorithm runs 2.5x slower than the paper's own)."""
     newest = max(os.path.getmtime(s) for s in _SRCS)
     if not force and os.path.exists(_LIB_PATH) and os.path.getmtime(_LIB_PATH) >= newest:
         return _LIB_PATH
-    cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-ffp-contract=off", "-fPIC", "-shared", "-o", _LIB_PATH] + _SRCS + ["-lm"]
+    cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-mpopcnt", "-ffp-contract=off", "-fPIC", "-shared", "-o", _LIB_PATH] + _SRCS + ["-lm"]
     subprocess.run(cmd, check=True)
     return _LIB_PATH
 
@@ -65,6 +67,13 @@ def _load():
     lib.csg_oracle_link.restype = None
     lib.csg_oracle_link_dim.argtypes = [ctypes.c_int]
     lib.csg_oracle_link_dim.restype = ctypes.c_int
+    _p_f64 = np.ctypeslib.ndpointer(dtype=np.float64, flags="C_CONTIGUOUS")
+    lib.csg_dominance2d_counts.argtypes = [_p_f64, _i64, _i64, _p_i64]
+    lib.csg_dominance2d_counts.restype = ctypes.c_int
+    lib.csg_dominance2d_counts_rows.argtypes = [_p_f64, _i64, _i64, _i64, _i64, _p_i64]
+    lib.csg_dominance2d_counts_rows.restype = ctypes.c_int
+    lib.csg_dominance2d_relations.argtypes = [_p_f64, _i64]
+    lib.csg_dominance2d_relations.restype = _i64
     lib.csg_alg5_threads.argtypes = []
     lib.csg_alg5_threads.restype = ctypes.c_int
     _lib = lib
@@ -159,6 +168,41 @@ def alg5_counts_rows(bits, N, kmax, row_begin, row_end):
     _load().csg_alg5_counts_rows(bits, N, bits.shape[1], kmax, int(row_begin), int(row_end), counts,
                                  ctypes.byref(tests))
     return counts, int(tests.value)
+
+
+def dominance2d_counts(coords, kmax):
+    """Interval abundances of a random 2D order straight from its (u, v) coordinates: n_ab = number of points
+    strictly inside the rectangle spanned by a related pair (PAPER.md:395 for a 2D order; SURVEY pin P6).  No
+    relation matrix is involved.  coords: (N, 2), any order, no repeated u or v."""
+    coords = np.ascontiguousarray(coords, dtype=np.float64)
+    assert coords.ndim == 2 and coords.shape[1] == 2, coords.shape
+    counts = np.zeros(kmax + 1, dtype=np.int64)
+    rc = _load().csg_dominance2d_counts(coords, coords.shape[0], int(kmax), counts)
+    if rc != 0:
+        raise ValueError("dominance2d_counts: %s" % ("repeated coordinate" if rc == -1 else "out of memory"))
+    return counts
+
+
+def dominance2d_counts_rows(coords, kmax, row_begin, row_end):
+    """dominance2d_counts restricted to related pairs whose lower element is one of coords[row_begin:row_end]
+    (the split by first element of alg5_counts_rows when coords are in time order)."""
+    coords = np.ascontiguousarray(coords, dtype=np.float64)
+    assert coords.ndim == 2 and coords.shape[1] == 2, coords.shape
+    counts = np.zeros(kmax + 1, dtype=np.int64)
+    rc = _load().csg_dominance2d_counts_rows(coords, coords.shape[0], int(kmax), int(row_begin), int(row_end), counts)
+    if rc != 0:
+        raise ValueError("dominance2d_counts_rows: %s" % ("repeated coordinate" if rc == -1 else "out of memory"))
+    return counts
+
+
+def dominance2d_relations(coords):
+    """Number of related pairs of a random 2D order = C(N,2) - inversions (SURVEY pin P5), from coordinates."""
+    coords = np.ascontiguousarray(coords, dtype=np.float64)
+    assert coords.ndim == 2 and coords.shape[1] == 2, coords.shape
+    r = int(_load().csg_dominance2d_relations(coords, coords.shape[0]))
+    if r < 0:
+        raise ValueError("dominance2d_relations: %s" % ("repeated coordinate" if r == -1 else "out of memory"))
+    return r
 
 
 def alg5_threads():

@@ -219,6 +219,82 @@ def test_p6_dominance_counting_2d(N, seed):
     assert (got == want).all()
 
 
+# ---------------------------------------------------------------- P5/P6 as a second oracle form: oracle/dominance2d.c
+def brute_force_rectangles(coords):
+    """O(N^3) from the coordinates alone: for every pair with u_a<u_b and v_a<v_b count the points strictly inside
+    the rectangle.  Catches a wrong strictness, a swapped axis or an off-by-one in the prefix sums."""
+    u, v = coords[:, 0], coords[:, 1]
+    N = len(u)
+    h = np.zeros(max(N - 1, 1), dtype=np.int64)
+    for a in range(N):
+        for b in range(N):
+            if u[a] < u[b] and v[a] < v[b]:
+                h[int(((u > u[a]) & (u < u[b]) & (v > v[a]) & (v < v[b])).sum())] += 1
+    return h
+
+
+@pytest.mark.parametrize("N,seed", [(2, 1), (3, 2), (7, 3), (64, 4), (211, 5)])
+def test_dominance2d_against_brute_force_rectangles(N, seed):
+    coords = csg_inputs.sprinkle(2, N, seed)
+    rng = np.random.default_rng(seed)
+    shuffled = coords[rng.permutation(N)]               # the element order must not matter
+    want = brute_force_rectangles(coords)
+    assert (oracle.dominance2d_counts(coords, N - 2) == want[: N - 1]).all()
+    assert (oracle.dominance2d_counts(shuffled, N - 2) == want[: N - 1]).all()
+    assert oracle.dominance2d_relations(shuffled) == want.sum()
+
+
+@pytest.mark.parametrize("N,seed", [(1, 9), (2, 9), (257, 9), (1000, 10), (3000, 12), (1024, csg_inputs.CONFIGS[0]["seed"])])
+def test_dominance2d_equals_triple_loop(N, seed):
+    """The coordinate route and the definition on the relation matrix give the same histogram."""
+    coords, bits = csg_inputs.make_causet(2, N, seed)
+    kmax = max(N - 2, 0)
+    want = oracle.counts_from_bits(bits, N, kmax)
+    assert (oracle.dominance2d_counts(coords, kmax) == want).all()
+    assert oracle.dominance2d_relations(coords) == want.sum()
+    if N >= 257:                                         # kmax truncation drops exactly the higher bins
+        assert (oracle.dominance2d_counts(coords, 5) == want[:6]).all()
+
+
+def test_dominance2d_equals_alg5_at_config1():
+    cfg = csg_inputs.CONFIGS[1]
+    coords, bits = csg_inputs.make_config(cfg)
+    N = cfg["N"]
+    want = oracle.alg5_counts(bits, N, N - 2)
+    got = oracle.dominance2d_counts(coords, N - 2)
+    assert (got == want).all()
+    assert oracle.dominance2d_relations(coords) == want.sum()
+
+
+def test_dominance2d_row_blocks_equal_alg5_row_blocks():
+    """Split by first element: each block equals Algorithm 5 on the same rows, and the blocks add up."""
+    N = 2500
+    coords, bits = csg_inputs.make_causet(2, N, 77)
+    total = np.zeros(N - 1, dtype=np.int64)
+    for r0, r1 in [(0, 1), (1, 640), (640, 1999), (1999, N)]:
+        part = oracle.dominance2d_counts_rows(coords, N - 2, r0, r1)
+        want, _ = oracle.alg5_counts_rows(bits, N, N - 2, r0, r1)
+        assert (part == want).all(), (r0, r1)
+        total += part
+    assert (total == oracle.dominance2d_counts(coords, N - 2)).all()
+
+
+def test_dominance2d_hand_cases():
+    # a chain along the diagonal: N_k = N-1-k; an antichain along the anti-diagonal: nothing related
+    N = 9
+    t = np.arange(N, dtype=np.float64) / N
+    assert oracle.dominance2d_counts(np.stack([t, t], 1), N - 2).tolist() == [N - 1 - k for k in range(N - 1)]
+    assert oracle.dominance2d_counts(np.stack([t, t[::-1]], 1), N - 2).sum() == 0
+    assert oracle.dominance2d_relations(np.stack([t, t[::-1]], 1)) == 0
+    # four corners of a square and its centre: (0,0)<(1,1) holds the centre only -> one pair with n=1; the centre
+    # is linked to both; (0,1) and (1,0) are related to nothing but... (0,1) vs (1,0): unrelated
+    pts = np.array([[0.0, 0.0], [1.0, 1.0], [0.5, 0.5], [0.25, 0.9], [0.9, 0.25]])
+    # related pairs: 0<2, 2<1, 0<1 (n=3: holds 2, 3, 4), 0<3 (n=0), 3<1 (n=0), 0<4 (n=0), 4<1 (n=0)
+    assert oracle.dominance2d_counts(pts, 3).tolist() == [6, 0, 0, 1]
+    with pytest.raises(ValueError):
+        oracle.dominance2d_counts(np.array([[0.1, 0.2], [0.1, 0.3]]), 0)
+
+
 # ---------------------------------------------------------------- P10: statistics over seeds
 def test_p10_statistics_2d_orders():
     N, seeds = 128, 120
