@@ -17,7 +17,17 @@
  * No function throws; every function returns a CSG_* code (0 = success) unless stated otherwise.
  * There is no CPU fallback: without a CUDA device every compute entry point returns CSG_E_CUDA.
  * Pointers are tagged DEVICE or HOST.  The caller owns every buffer it passes; the library keeps a small
- * cached device workspace (tile schedule, counters) that csg_shutdown() frees.  Inputs are never modified.
+ * cached device workspace (tile schedules, counters, events) that csg_shutdown() frees.  Inputs are never modified.
+ *
+ * Devices and threads.  Every call works on the CURRENT CUDA device (cudaGetDevice); DEVICE pointers and the stream
+ * must belong to it.  Cached state is kept per device, so one process may drive several GPUs (switch devices with
+ * cudaSetDevice between calls).  The entry points are thread-safe (one internal mutex; they only enqueue work).
+ * Stream-ordered calls (csg_action, csg_action_partial/_finish, csg_action_batch, csg_link, csg_interval_sizes) may
+ * be in flight on different streams at the same time: cached tile schedules are immutable once built and are never
+ * freed or rebuilt before csg_shutdown().  The HOST-buffer calls (csg_action_host, csg_causet_action_host) run on
+ * an internal stream per device, share library-owned device buffers and return synchronised; they serialise.
+ * csg_shutdown() must not be called while work of this library is still in flight, and it invalidates every CUDA
+ * graph that captured a call of this library (the graph holds pointers into the cached workspace).
  */
 #ifndef CSG_H_
 #define CSG_H_
@@ -35,14 +45,14 @@ typedef struct CUstream_st *cudaStream_t;
 enum {
     CSG_OK = 0,
     CSG_E_NULL = -1,        /* a required pointer is NULL */
-    CSG_E_SIZE = -2,        /* N < 1, N > CSG_MAX_N, or npairs < 0 */
+    CSG_E_SIZE = -2,        /* N < 1, N > CSG_MAX_N, npairs < 0, a tile index outside the matrix, iters < 1 */
     CSG_E_ALIGN = -3,       /* rel_bits not 16-byte aligned, counts/S not 8-byte aligned */
     CSG_E_DIM = -4,         /* dim not in {2, 4} */
     CSG_E_EPS = -5,         /* eps NaN or outside (0, 1] */
     CSG_E_KMAX = -6,        /* kmax < 0, kmax > CSG_MAX_KMAX, or too small for the local action */
-    CSG_E_UNSUPPORTED = -7, /* reserved (no argument combination returns it at present) */
+    CSG_E_UNSUPPORTED = -7, /* csg_tile_interval_sizes while the bitset variant is selected */
     CSG_E_CUDA = -8,        /* a CUDA call failed; csg_strerror(CSG_E_CUDA) carries its text */
-    CSG_E_VARIANT = -9,     /* unknown variant id */
+    CSG_E_VARIANT = -9,     /* unknown variant id or mode */
     CSG_E_SHARD = -10,      /* nshards < 1 or shard outside [0, nshards) */
     CSG_E_GEOMETRY = -11    /* unknown geometry id */
 };
@@ -63,9 +73,10 @@ enum {
 int64_t csg_row_stride_words(int64_t N);
 
 /*
- * Interval abundances and action of one causal set.  All work is enqueued on `stream`; no host
- * synchronisation happens inside (the first call for a new N also builds the cached tile schedule; after that
- * warm-up call the function only enqueues a memset and two kernels and can be captured in a CUDA graph).
+ * Interval abundances and action of one causal set.  All work is enqueued on `stream`.  The FIRST call for a new
+ * (device, N) builds that size's tile schedule and copies it to the device with one blocking cudaMemcpy; every later
+ * call with that N -- whatever other sizes were run in between, on whatever stream -- only enqueues a memset and
+ * two kernels, synchronises nothing, and can be captured in a CUDA graph.
  *
  *   rel_bits DEVICE, N*csg_row_stride_words(N) words, layout above, 16-byte aligned, read only.
  *   N        number of elements, 1 <= N <= CSG_MAX_N (N = 1, 2 are valid: no triples).
@@ -95,7 +106,10 @@ int csg_action(const uint64_t *rel_bits, int64_t N, int dim, double eps, int kma
  *   add up to those of csg_action (the caller sums them, e.g. ncclAllReduce).  0 <= shard < nshards.
  * csg_action_finish: steps a4/a5 on summed abundances: counts DEVICE (read only), S DEVICE, 1 double;
  *   N, dim, eps, kmax as in csg_action.  csg_action == partial(shard 0 of 1) followed by finish.
- * Both enqueue on `stream` and do not synchronise.
+ * Both enqueue on `stream` and do not synchronise (first call per (N, shard, nshards): as csg_action).
+ * Which pairs a shard covers: tensor variants -- the tiles csg_tile_schedule lists for it; bitset variant (N <= 1024
+ * under CSG_VARIANT_AUTO) -- every nshards-th 64 x 64 tile of its own depth-sorted enumeration, which
+ * csg_tile_schedule does not describe.  Either way the shards of one N partition the related pairs exactly.
  */
 int csg_action_partial(const uint64_t *rel_bits, int64_t N, int kmax, int shard, int nshards, int64_t *counts,
                        cudaStream_t stream);
@@ -118,6 +132,7 @@ int csg_action_batch(const uint64_t *rel_bits, int64_t N, int64_t batch, int dim
  * 8 x 9 blocks so that concurrently running tiles share rows in L2).  tiles_ij HOST, 2*capacity int32
  * (I0, J0, I1, J1, ...), may be NULL; returns the number of tiles of the shard (or a negative CSG_E_* code);
  * at most `capacity` tiles are written.  The shards of one N partition the upper triangle exactly.
+ * Describes the tensor variants only (see csg_action_partial).
  */
 int64_t csg_tile_schedule(int64_t N, int shard, int nshards, int32_t *tiles_ij, int64_t capacity);
 
@@ -125,6 +140,10 @@ int64_t csg_tile_schedule(int64_t N, int shard, int nshards, int32_t *tiles_ij, 
  * Same computation with HOST buffers (the end-to-end call): copies rel_bits to the device (pinned or
  * pageable host memory), runs csg_action on an internal stream, copies counts and S back and
  * synchronises.  rel_bits_host: N*stride words; counts_host: kmax+1 int64; S_host: 1 double.
+ * Matrices of 32 MiB and more go over in 32 row chunks on a copy stream while ONE persistent launch of the
+ * interval kernel already runs: after each chunk the copy stream publishes the number of rows landed
+ * (cuStreamWriteValue32) and a tile starts when the rows it reads are there (overlap of the
+ * transfer with the computation).
  */
 int csg_action_host(const uint64_t *rel_bits_host, int64_t N, int dim, double eps, int kmax,
                     int64_t *counts_host, double *S_host);
@@ -166,10 +185,45 @@ int csg_last_link_ms(float *ms);
 int csg_interval_sizes(const uint64_t *rel_bits, int64_t N, const int64_t *pairs_ij, int64_t npairs,
                        int32_t *n_out, cudaStream_t stream);
 
+/*
+ * Test hook for the tensor variants: every interval size of whole 256 x 256 tiles, computed by the SAME kernel,
+ * tile sweep, open-range masks and accumulators as csg_action (its epilogue writes n_ij instead of bucketing it).
+ * tiles_ij_host HOST, 2*ntiles int32 (I0, J0, I1, J1, ...), 256-row blocks with 0 <= I <= J < ceil(N/256);
+ * n_out DEVICE, ntiles*256*256 int32: n_out[(t*256 + r)*256 + c] = n_ij for i = 256 I_t + r, j = 256 J_t + c if
+ * i < j < N and bit (i,j) is set, else -1.  Uses the variant csg_action would use for this N (CSG_E_UNSUPPORTED
+ * for the bitset variant).  Synchronises `stream` before it returns.  0 <= ntiles <= 32768.
+ */
+int csg_tile_interval_sizes(const uint64_t *rel_bits, int64_t N, const int32_t *tiles_ij_host, int64_t ntiles,
+                            int32_t *n_out, cudaStream_t stream);
+
 /* Choose the kernel variant for later csg_action calls (CSG_VARIANT_*); returns CSG_E_VARIANT if unknown. */
 int csg_set_variant(int variant);
 /* The variant csg_action would run for this N under the current setting (CSG_VARIANT_BITSET, _TENSOR or _TENSOR_FP4). */
 int csg_effective_variant(int64_t N);
+
+/*
+ * Measurement / test aid like csg_set_variant: the drift throttle of the fp4 tensor kernel (clusters of the
+ * persistent grid are kept within one round of each other so that concurrently running tiles share rows in L2).
+ * CSG_THROTTLE_AUTO: on for matrices above 4 GiB only; _ON: on whenever a launch has more tiles than clusters;
+ * _OFF: never.  In every mode it is used only if the runtime reports that the whole grid can be resident at once,
+ * and a wait that lasts longer than a few ms switches it off inside the kernel.  Results never depend on it.
+ */
+enum { CSG_THROTTLE_AUTO = 0, CSG_THROTTLE_ON = 1, CSG_THROTTLE_OFF = 2 };
+int csg_set_throttle(int mode);
+
+/*
+ * Measurement aid: the roofline denominators measured on the current device.  Runs a bare kernel (no producers, no
+ * memory traffic) and returns its CUDA-event time in *ms (HOST) and the work it did in *units (HOST):
+ *   CSG_PEAK_MMA_MXF4  the interval kernel's own instruction, tcgen05.mma.cta_group::2.kind::mxf4 block32, M = N = 256,
+ *                      K = 64, A from TMEM, issued back to back by one thread per SM pair; units = MACs
+ *   CSG_PEAK_MMA_I8    the same for kind::i8 (K = 32, both operands in shared memory); units = MACs
+ *   CSG_PEAK_ALU_MIX   the bitset variant's inner mix, 1 AND + 1 POPC + 1 ADD per step on 32-bit words; units = lane-steps
+ *                      (one lane-step = 32 ordered-triple tests)
+ *   CSG_PEAK_ALU_POPC / CSG_PEAK_ALU_LOP3   one POPC / one LOP3 per step; units = lane-steps
+ * iters: 4-MMA groups per SM pair (tensor) or loop trips of 8 steps per thread (ALU).  Synchronises the device.
+ */
+enum { CSG_PEAK_MMA_MXF4 = 0, CSG_PEAK_MMA_I8 = 1, CSG_PEAK_ALU_MIX = 2, CSG_PEAK_ALU_POPC = 3, CSG_PEAK_ALU_LOP3 = 4 };
+int csg_measure_peak(int what, int iters, float *ms, double *units);
 
 /*
  * Measurement aids.  csg_set_kernel_timing(1) makes csg_action bracket its dominant kernel (the interval

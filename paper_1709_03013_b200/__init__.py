@@ -7,7 +7,8 @@ There is no CPU fallback: if libcsg.so is missing, importing the compute entry p
 Functions carry the C names: csg_action, csg_action_host, csg_interval_sizes, csg_row_stride_words,
 csg_set_variant, csg_effective_variant, csg_set_kernel_timing, csg_last_kernel_ms, csg_kernel_ms_history,
 csg_launch_count, csg_action_partial, csg_action_finish, csg_tile_schedule, csg_link, csg_causet_action_host,
-csg_last_link_ms, csg_action_batch, csg_strerror, csg_shutdown.
+csg_last_link_ms, csg_action_batch, csg_tile_interval_sizes, csg_set_throttle, csg_measure_peak, csg_strerror,
+csg_shutdown.
 """
 import ctypes
 import os
@@ -18,13 +19,16 @@ from . import _build
 
 VARIANT_AUTO, VARIANT_BITSET, VARIANT_TENSOR, VARIANT_TENSOR_FP4 = 0, 1, 2, 3
 GEOM_MINKOWSKI_2D, GEOM_MINKOWSKI_4D, GEOM_DESITTER_2D = 0, 1, 2
+THROTTLE_AUTO, THROTTLE_ON, THROTTLE_OFF = 0, 1, 2
+PEAK_MMA_MXF4, PEAK_MMA_I8, PEAK_ALU_MIX, PEAK_ALU_POPC, PEAK_ALU_LOP3 = 0, 1, 2, 3, 4
 LIB_PATH = _build.LIB_PATH
 
 EXPORTS = [
     "csg_row_stride_words", "csg_action", "csg_action_host", "csg_interval_sizes", "csg_set_variant",
     "csg_effective_variant", "csg_set_kernel_timing", "csg_last_kernel_ms", "csg_kernel_ms_history",
     "csg_launch_count", "csg_action_partial", "csg_action_finish", "csg_tile_schedule", "csg_link",
-    "csg_causet_action_host", "csg_last_link_ms", "csg_action_batch",
+    "csg_causet_action_host", "csg_last_link_ms", "csg_action_batch", "csg_tile_interval_sizes", "csg_set_throttle",
+    "csg_measure_peak",
     "csg_strerror", "csg_shutdown",
 ]
 
@@ -74,6 +78,12 @@ def load():
     lib.csg_last_link_ms.restype = ci
     lib.csg_interval_sizes.argtypes = [vp, i64, vp, i64, vp, vp]
     lib.csg_interval_sizes.restype = ci
+    lib.csg_tile_interval_sizes.argtypes = [vp, i64, vp, i64, vp, vp]
+    lib.csg_tile_interval_sizes.restype = ci
+    lib.csg_set_throttle.argtypes = [ci]
+    lib.csg_set_throttle.restype = ci
+    lib.csg_measure_peak.argtypes = [ci, ci, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_double)]
+    lib.csg_measure_peak.restype = ci
     lib.csg_set_variant.argtypes = [ci]
     lib.csg_set_variant.restype = ci
     lib.csg_effective_variant.argtypes = [i64]
@@ -267,6 +277,33 @@ def csg_interval_sizes(rel_bits, N, pairs_ij, n_out=None, stream=None):
     _check(lib.csg_interval_sizes(rel_bits.data_ptr(), int(N), pairs_ij.data_ptr(), npairs, n_out.data_ptr(),
                                   _stream_handle(stream)))
     return n_out
+
+
+def csg_tile_interval_sizes(rel_bits, N, tiles_ij, n_out=None, stream=None):
+    """Test hook: all n_ij of the listed 256 x 256 tiles from the tensor kernel itself.  tiles_ij: (ntiles, 2) int
+    array-like of block pairs I <= J.  Returns a CUDA int32 tensor (ntiles, 256, 256), -1 where (i, j) is no related
+    pair; synchronised."""
+    import torch
+    lib = load()
+    tiles = np.ascontiguousarray(np.asarray(tiles_ij, dtype=np.int32).reshape(-1, 2))
+    assert rel_bits.is_cuda and rel_bits.element_size() == 8 and rel_bits.is_contiguous()
+    if n_out is None:
+        n_out = torch.empty((tiles.shape[0], 256, 256), dtype=torch.int32, device=rel_bits.device)
+    assert n_out.is_cuda and n_out.dtype == torch.int32 and n_out.numel() >= tiles.shape[0] * 65536
+    _check(lib.csg_tile_interval_sizes(rel_bits.data_ptr(), int(N), tiles.ctypes.data, tiles.shape[0], n_out.data_ptr(),
+                                       _stream_handle(stream)))
+    return n_out
+
+
+def csg_set_throttle(mode):
+    _check(load().csg_set_throttle(int(mode)))
+
+
+def csg_measure_peak(what, iters):
+    """int csg_measure_peak(what, iters, ms, units): returns (ms, units) of one bare peak kernel (PEAK_* ids)."""
+    ms, units = ctypes.c_float(0.0), ctypes.c_double(0.0)
+    _check(load().csg_measure_peak(int(what), int(iters), ctypes.byref(ms), ctypes.byref(units)))
+    return float(ms.value), float(units.value)
 
 
 def csg_set_variant(variant):

@@ -4,6 +4,7 @@ import subprocess
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libcsg.so")
+ABLATE_LIB_PATH = os.path.join(_HERE, "libcsg_ablate.so")    # -DCSG_ABLATE build, only ever loaded by ablate.py
 _CSRC = os.path.join(_HERE, "csrc")
 _INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 
@@ -23,16 +24,23 @@ def needs_build():
     return any(os.path.getmtime(s) > t for s in _sources())
 
 
-def build(force=False, verbose=False):
-    """nvcc -gencode arch=compute_100a,code=sm_100a -lineinfo -O3 -> paper_1709_03013_b200/libcsg.so"""
-    if not force and not needs_build():
-        return LIB_PATH
+def build(force=False, verbose=False, ablate=False, defines=()):
+    """nvcc -gencode arch=compute_100a,code=sm_100a -lineinfo -O3 -> paper_1709_03013_b200/libcsg.so
+    ablate=True builds libcsg_ablate.so instead: the same sources with -DCSG_ABLATE, i.e. with the timing-ablation
+    switches of the fp4 kernel and csg_set_debug compiled in (wrong counts when set; never the product library)."""
+    out = ABLATE_LIB_PATH if ablate else LIB_PATH
+    if not force and not ablate and not defines and not needs_build():
+        return out
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     cmd = [
         nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-        "-shared", "-Xcompiler", "-fPIC", "-o", LIB_PATH, os.path.join(_CSRC, "csg.cu"),
+        "-shared", "-Xcompiler", "-fPIC", "-o", out, os.path.join(_CSRC, "csg.cu"),
     ]
+    if ablate:
+        cmd.insert(1, "-DCSG_ABLATE")
+    for d in defines:
+        cmd.insert(1, "-D" + d)
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
     subprocess.run(cmd, check=True)
-    return LIB_PATH
+    return out

@@ -16,6 +16,7 @@
 #include "bitset_kernel.cuh"
 #include "link_kernel.cuh"
 #include "tensor_kernel.cuh"
+#include "peak_kernels.cuh"
 
 namespace csg {
 
@@ -84,52 +85,78 @@ finish_action_kernel(const long long* __restrict__ counts, long long N, int dim,
 }
 
 // ---------------------------------------------------------------------------------------------- host state
+// One mutex serialises the entry points (they only enqueue work, so it is held for microseconds).  Settings are
+// process-wide; everything that lives on a device (cached tile lists, events, the host path's buffers) is kept per
+// CUDA device ordinal and looked up from cudaGetDevice() on every call, so a process may drive several GPUs.
+// Cached device objects are created on first use and released ONLY by csg_shutdown(): a CUDA graph that captured a
+// csg_action call keeps pointing at valid memory however many other sizes are run in between.
 constexpr int TIMING_RING = 64;
+constexpr int PROGRESS_RING = 64;
+constexpr int MAX_DEVICES = 64;
 
-struct State {
-    std::mutex mu;
-    int variant = CSG_VARIANT_AUTO;
-    bool timing = false;
+struct TileList {                       // tile schedule of one (N, shard, nshards) on the device
+    long long N;
+    int shard, nshards;
+    int2* d;
+    int n;
+};
+struct ChunkTiles {                     // the same tiles grouped by the row chunk of the host-matrix pipeline
+    long long N;
+    int2* d;
+    int n;
+    std::vector<int> off;               // chunk c owns tiles [off[c], off[c+1])
+    std::vector<long long> row_end;
+};
+struct BitsMap {                        // TMA descriptor of a relation matrix (passed to the kernel by value)
+    const void* ptr;
+    long long N;
+    int kind;
+    CUtensorMap map;
+};
+
+struct Device {
+    int ordinal = -1;
+    int sm_count = 0;
+    bool attr_set = false;
+    int wait_clusters = -1;             // cudaOccupancyMaxActiveClusters of the WAIT instantiation (throttle needs all resident)
+    std::vector<TileList> tiles;
+    std::vector<ChunkTiles*> chunk_tiles;
+    std::vector<BitsMap> maps;          // small ring, oldest replaced
+    size_t maps_next = 0;
     // ring of event pairs around the interval kernel of the latest TIMING_RING timed calls
     cudaEvent_t ev0[TIMING_RING] = {}, ev1[TIMING_RING] = {};
     long long timed_calls = 0;
-    long long launches = 0;
-    char cuda_msg[256] = "no CUDA error recorded";
-    // cached tile schedule of the tensor variant
-    long long tiles_N = -1;
-    int tiles_shard = 0, tiles_nshards = 1;
-    int2* d_tiles = nullptr;
-    int ntiles = 0;
-    std::vector<int2> h_tiles;
-    int sm_count = 0;
-    bool attr_set = false;
-    // TMA descriptor of the relation matrix seen as N rows of stride*8 bytes (cached per pointer and N)
-    void* encode_tiled = nullptr;
-    CUtensorMap bits_map[2];            // [KIND_I8], [KIND_FP4]
-    const void* map_ptr[2] = {nullptr, nullptr};
-    long long map_N[2] = {-1, -1};
+    unsigned int* d_progress = nullptr; // PROGRESS_RING finished-tile counters, one per launch in flight (drift throttle)
+    unsigned int* d_rows_ready = nullptr;   // rows of the host matrix landed so far (gate of csg_action_host)
     // end-to-end (host buffer) path
-    cudaStream_t host_stream = nullptr;
+    cudaStream_t host_stream = nullptr, copy_stream = nullptr;
     uint64_t* d_bits = nullptr;
     size_t d_bits_bytes = 0;
     long long* d_counts = nullptr;
     size_t d_counts_bytes = 0;
     double* d_S = nullptr;
     double* d_coords = nullptr;
-    unsigned int* d_progress = nullptr;     // finished-tile counter of the running tensor launch (drift throttle)
     size_t d_coords_bytes = 0;
-    // pipelined host path: row chunks copied on copy_stream, each chunk's tiles launched as soon as it landed
-    cudaStream_t copy_stream = nullptr;
     std::vector<cudaEvent_t> chunk_ev;
-    long long chunk_N = -1;
-    int2* d_chunk_tiles = nullptr;
-    std::vector<int> chunk_off;         // chunk c owns tiles [chunk_off[c], chunk_off[c+1]) of d_chunk_tiles
-    std::vector<long long> chunk_row_end;
     // events around the latest timed linking kernel
     cudaEvent_t link_ev0 = nullptr, link_ev1 = nullptr;
     bool link_timed = false;
 };
-static State g;
+
+struct Global {
+    std::mutex mu;
+    int variant = CSG_VARIANT_AUTO;
+    int throttle = CSG_THROTTLE_AUTO;
+    bool timing = false;
+    int debug = 0;                      // ablation bits; only the -DCSG_ABLATE build can set it
+    long long launches = 0;
+    char cuda_msg[256] = "no CUDA error recorded";
+    void* encode_tiled = nullptr;       // cuTensorMapEncodeTiled
+    void* write_value32 = nullptr;      // cuStreamWriteValue32
+    bool write_value32_tried = false;
+    Device* dev[MAX_DEVICES] = {};
+};
+static Global g;
 
 static int cuda_fail(cudaError_t e, const char* what) {
     snprintf(g.cuda_msg, sizeof(g.cuda_msg), "%s: %s", what, cudaGetErrorString(e));
@@ -142,18 +169,28 @@ static int cuda_fail(cudaError_t e, const char* what) {
         if (e_ != cudaSuccess) return cuda_fail(e_, #call); \
     } while (0)
 
-static int ensure_device() {
-    if (g.sm_count > 0) return CSG_OK;
-    int dev = 0;
-    CSG_CUDA(cudaGetDevice(&dev));
-    cudaDeviceProp prop;
-    CSG_CUDA(cudaGetDeviceProperties(&prop, dev));
-    if (prop.major != 10) {
-        snprintf(g.cuda_msg, sizeof(g.cuda_msg), "device is sm_%d%d; libcsg is built for sm_100a only", prop.major,
-                 prop.minor);
+// State of the current CUDA device (created on first use).
+static int current_device(Device** out) {
+    int ord = 0;
+    CSG_CUDA(cudaGetDevice(&ord));
+    if (ord < 0 || ord >= MAX_DEVICES) {
+        snprintf(g.cuda_msg, sizeof(g.cuda_msg), "device ordinal %d out of range", ord);
         return CSG_E_CUDA;
     }
-    g.sm_count = prop.multiProcessorCount;
+    if (!g.dev[ord]) {
+        cudaDeviceProp prop;
+        CSG_CUDA(cudaGetDeviceProperties(&prop, ord));
+        if (prop.major != 10) {
+            snprintf(g.cuda_msg, sizeof(g.cuda_msg), "device is sm_%d%d; libcsg is built for sm_100a only", prop.major,
+                     prop.minor);
+            return CSG_E_CUDA;
+        }
+        Device* d = new Device;
+        d->ordinal = ord;
+        d->sm_count = prop.multiProcessorCount;
+        g.dev[ord] = d;
+    }
+    *out = g.dev[ord];
     return CSG_OK;
 }
 
@@ -222,33 +259,42 @@ static void build_tile_schedule(long long N, int shard, int nshards, std::vector
     }
 }
 
-static int ensure_tiles(long long N, int shard, int nshards, cudaStream_t stream) {
-    if (g.tiles_N == N && g.tiles_shard == shard && g.tiles_nshards == nshards && g.d_tiles) return CSG_OK;
-    build_tile_schedule(N, shard, nshards, g.h_tiles);
-    if (g.d_tiles) {
-        CSG_CUDA(cudaStreamSynchronize(stream));
-        CSG_CUDA(cudaFree(g.d_tiles));
-        g.d_tiles = nullptr;
-    }
-    g.ntiles = (int)g.h_tiles.size();
-    CSG_CUDA(cudaMalloc(&g.d_tiles, std::max<size_t>(1, g.h_tiles.size()) * sizeof(int2)));
-    CSG_CUDA(cudaMemcpyAsync(g.d_tiles, g.h_tiles.data(), g.h_tiles.size() * sizeof(int2), cudaMemcpyHostToDevice,
-                             stream));
-    g.tiles_N = N;
-    g.tiles_shard = shard;
-    g.tiles_nshards = nshards;
+// Device copy of a shard's tile list.  Built on the first call for that (N, shard, nshards) with one blocking copy;
+// afterwards a lookup.  Entries stay until csg_shutdown (at most 4 MiB each, N = 262144), so a captured CUDA graph or a
+// launch in flight on another stream never sees its tile list freed or overwritten.
+static int ensure_tiles(Device* D, long long N, int shard, int nshards, const TileList** out) {
+    for (const TileList& t : D->tiles)
+        if (t.N == N && t.shard == shard && t.nshards == nshards) {
+            *out = &t;
+            return CSG_OK;
+        }
+    std::vector<int2> h;
+    build_tile_schedule(N, shard, nshards, h);
+    TileList t{N, shard, nshards, nullptr, (int)h.size()};
+    CSG_CUDA(cudaMalloc(&t.d, std::max<size_t>(1, h.size()) * sizeof(int2)));
+    if (!h.empty()) CSG_CUDA(cudaMemcpy(t.d, h.data(), h.size() * sizeof(int2), cudaMemcpyHostToDevice));
+    D->tiles.push_back(t);
+    *out = &D->tiles.back();
     return CSG_OK;
 }
 
 // 2D byte view of the packed relation matrix for the TMA warp of the tensor variants: dim0 = stride*8 bytes of a
 // row, dim1 = N rows; box = 32 (int8) or 64 (fp4) bytes x 128 rows with the matching 32/64-byte swizzle
 // (conflict-free 16-byte reads by the producers); rows >= N and bytes beyond the row are zero-filled by the hardware.
+// The descriptor is a kernel parameter (copied at launch), so this cache is host memory only.
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+typedef CUresult (*WriteValue32Fn)(CUstream, CUdeviceptr, cuuint32_t, unsigned int);
+constexpr size_t MAPS_CACHED = 16;
 
-static int ensure_bits_map(int kind, const uint64_t* rel_bits, long long N, long long stride_words) {
-    if (g.map_ptr[kind] == rel_bits && g.map_N[kind] == N) return CSG_OK;
+static int ensure_bits_map(Device* D, int kind, const uint64_t* rel_bits, long long N, long long stride_words,
+                           const CUtensorMap** out) {
+    for (const BitsMap& m : D->maps)
+        if (m.ptr == rel_bits && m.N == N && m.kind == kind) {
+            *out = &m.map;
+            return CSG_OK;
+        }
     if (!g.encode_tiled) {
         cudaDriverEntryPointQueryResult qres;
         CSG_CUDA(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &g.encode_tiled, cudaEnableDefault, &qres));
@@ -258,22 +304,28 @@ static int ensure_bits_map(int kind, const uint64_t* rel_bits, long long N, long
             return CSG_E_CUDA;
         }
     }
+    BitsMap m{rel_bits, N, kind, {}};
     const int row_bytes = kind == KIND_FP4 ? TcTraits<KIND_FP4>::BITS_ROW_BYTES : TcTraits<KIND_I8>::BITS_ROW_BYTES;
     const cuuint64_t dims[2] = {(cuuint64_t)stride_words * 8, (cuuint64_t)N};
     const cuuint64_t strides[1] = {(cuuint64_t)stride_words * 8};
     const cuuint32_t box[2] = {(cuuint32_t)row_bytes, (cuuint32_t)TC_BITS_BOX_ROWS};
     const cuuint32_t estr[2] = {1, 1};
     CUresult r = reinterpret_cast<EncodeTiledFn>(g.encode_tiled)(
-        &g.bits_map[kind], CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<uint64_t*>(rel_bits), dims, strides, box, estr,
+        &m.map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<uint64_t*>(rel_bits), dims, strides, box, estr,
         CU_TENSOR_MAP_INTERLEAVE_NONE, kind == KIND_FP4 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_32B,
         CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
         snprintf(g.cuda_msg, sizeof(g.cuda_msg), "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
-        g.map_ptr[kind] = nullptr;
         return CSG_E_CUDA;
     }
-    g.map_ptr[kind] = rel_bits;
-    g.map_N[kind] = N;
+    if (D->maps.size() < MAPS_CACHED) {
+        D->maps.push_back(m);
+        *out = &D->maps.back().map;
+    } else {
+        D->maps[D->maps_next] = m;
+        *out = &D->maps[D->maps_next].map;
+        D->maps_next = (D->maps_next + 1) % MAPS_CACHED;
+    }
     return CSG_OK;
 }
 
@@ -288,97 +340,137 @@ static int validate(const void* rel_bits, long long N, int dim, double eps, int 
     return CSG_OK;
 }
 
-// Interval kernel over the tiles of one shard: counts (kmax+1 int64, overwritten) <- this shard's abundances.
-// TMA descriptor + dynamic shared memory opt-in of the tensor kernels.
-static int ensure_tensor_ready(int kind, const uint64_t* rel_bits, long long N, long long stride) {
-    int rc = ensure_bits_map(kind, rel_bits, N, stride);
-    if (rc) return rc;
-    if (!g.attr_set) {
-        const int s8 = TcTraits<KIND_I8>::SMEM_BYTES, s4 = TcTraits<KIND_FP4>::SMEM_BYTES;
-        CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_I8, 7>, cudaFuncAttributeMaxDynamicSharedMemorySize, s8));
-        CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_I8, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, s8));
-        CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_I8, 5>, cudaFuncAttributeMaxDynamicSharedMemorySize, s8));
-        CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_I8, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, s8));
-        CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_FP4, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, s4));
-        CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_FP4, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, s4));
-        CSG_CUDA(cudaFuncSetAttribute(tensor_action_kernel<KIND_FP4, 0, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, s4));
-        g.attr_set = true;
+#ifdef CSG_ABLATE
+constexpr int FP4_EXTRA = TCF_ABLATE;   // the ablation build's fp4 kernel carries the dbg switches (wrong counts when set)
+#else
+constexpr int FP4_EXTRA = 0;
+#endif
+
+// Dynamic shared memory opt-in of the tensor kernels and the occupancy of the instantiation that may wait.
+static int ensure_tensor_ready(Device* D) {
+    if (D->attr_set) return CSG_OK;
+    const int s8 = TcTraits<KIND_I8>::SMEM_BYTES, s4 = TcTraits<KIND_FP4>::SMEM_BYTES;
+#define CSG_OPT_IN(kernel, bytes) CSG_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes))
+    CSG_OPT_IN((tensor_action_kernel<KIND_I8, 7>), s8);
+    CSG_OPT_IN((tensor_action_kernel<KIND_I8, 6>), s8);
+    CSG_OPT_IN((tensor_action_kernel<KIND_I8, 5>), s8);
+    CSG_OPT_IN((tensor_action_kernel<KIND_I8, 4>), s8);
+    CSG_OPT_IN((tensor_action_kernel<KIND_I8, 7, TCF_DUMP>), s8);
+    CSG_OPT_IN((tensor_action_kernel<KIND_I8, 6, TCF_DUMP>), s8);
+    CSG_OPT_IN((tensor_action_kernel<KIND_I8, 5, TCF_DUMP>), s8);
+    CSG_OPT_IN((tensor_action_kernel<KIND_I8, 4, TCF_DUMP>), s8);
+    CSG_OPT_IN((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA>), s4);
+    CSG_OPT_IN((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA | TCF_WAIT>), s4);
+    CSG_OPT_IN((tensor_action_kernel<KIND_FP4, 0, TCF_DUMP>), s4);
+    CSG_OPT_IN((tensor_peak_kernel<KIND_FP4>), s4);
+    CSG_OPT_IN((tensor_peak_kernel<KIND_I8>), s8);
+#undef CSG_OPT_IN
+    // The drift throttle makes clusters wait for tiles finished by OTHER clusters, which is only safe when the whole
+    // grid is resident at once: ask the runtime how many CTA pairs of that instantiation fit on the device right now.
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(2 * (D->sm_count / 2));
+    cfg.blockDim = dim3(TC_THREADS);
+    cfg.dynamicSmemBytes = s4;
+    cudaLaunchAttribute attr;
+    attr.id = cudaLaunchAttributeClusterDimension;
+    attr.val.clusterDim.x = 2;
+    attr.val.clusterDim.y = 1;
+    attr.val.clusterDim.z = 1;
+    cfg.attrs = &attr;
+    cfg.numAttrs = 1;
+    int nclusters = 0;
+    if (cudaOccupancyMaxActiveClusters(&nclusters, tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA | TCF_WAIT>, &cfg) != cudaSuccess) {
+        cudaGetLastError();
+        nclusters = 0;
     }
+    D->wait_clusters = nclusters;
+    D->attr_set = true;
     return CSG_OK;
 }
 
-// One launch of the tensor kernel over a tile list (counts are added to, not zeroed).
-static int launch_tensor(int kind, const uint64_t* rel_bits, long long N, long long stride, int kmax, long long* counts,
-                         const int2* d_tiles, int ntiles, cudaStream_t stream) {
-    const int grid = 2 * std::max(1, std::min(ntiles, g.sm_count / 2));   // one CTA pair per SM pair
+// One launch of the tensor kernel over a tile list (counts are added to, not zeroed).  rows_ready: gate of the
+// host-matrix path (NULL when the matrix is resident); dump: csg_tile_interval_sizes (NULL otherwise).
+static int launch_tensor(Device* D, int kind, const uint64_t* rel_bits, long long N, long long stride, int kmax,
+                         long long* counts, const int2* d_tiles, int ntiles, const unsigned int* rows_ready, int* dump,
+                         cudaStream_t stream) {
+    int rc = ensure_tensor_ready(D);
+    if (rc) return rc;
+    const CUtensorMap* map = nullptr;
+    rc = ensure_bits_map(D, kind, rel_bits, N, stride, &map);
+    if (rc) return rc;
+    const int grid = 2 * std::max(1, std::min(ntiles, D->sm_count / 2));   // one CTA pair per SM pair
     // Drift throttle (tensor_kernel.cuh, TC_MAX_LEAD).  Measured: config 4 (N = 262144, full histogram) 1022 -> 929 ms,
     // DRAM reads 2.55 -> 0.67 TB per launch, SM clock under the power cap 1.67 -> 1.86 GHz; config 3 (kmax = 3)
-    // 106.6 -> 107.5 ms, the de Sitter workload (N = 131072, full histogram) 109.9 -> 111.4 ms.  So it is switched on
-    // only for matrices of more than 4 GiB, where a cluster walks through thousands of rounds.
+    // 106.6 -> 107.5 ms, the de Sitter workload (N = 131072, full histogram) 109.9 -> 111.4 ms.  So CSG_THROTTLE_AUTO
+    // switches it on only for matrices of more than 4 GiB, where a cluster walks through thousands of rounds -- and
+    // only if the runtime says that the whole grid can be resident at once (the wait is bounded in the kernel, too).
     unsigned int* progress = nullptr;
-    const bool drifts = kind == KIND_FP4 && N * stride * 8 > (4LL << 30);
-    if (drifts && ntiles > 16 * (grid / 2) && !getenv("CSG_NO_THROTTLE")) {
+    const bool big = N * stride * 8 > (4LL << 30) && ntiles > 16 * (grid / 2);
+    const bool want = g.throttle == CSG_THROTTLE_ON ? ntiles > grid / 2 : (g.throttle == CSG_THROTTLE_AUTO && big);
+    if (kind == KIND_FP4 && dump == nullptr && want && D->wait_clusters >= grid / 2) {
         // a ring of counters, one per launch, so that launches in flight on different streams do not share one
-        if (!g.d_progress) CSG_CUDA(cudaMalloc(&g.d_progress, 64 * sizeof(unsigned int)));
-        progress = g.d_progress + (g.launches & 63);
+        if (!D->d_progress) CSG_CUDA(cudaMalloc(&D->d_progress, PROGRESS_RING * sizeof(unsigned int)));
+        progress = D->d_progress + (g.launches % PROGRESS_RING);
         CSG_CUDA(cudaMemsetAsync(progress, 0, sizeof(unsigned int), stream));
     }
     unsigned long long* c64 = reinterpret_cast<unsigned long long*>(counts);
-    const char* dbg_env = getenv("CSG_DEBUG");
-    const int dbg = dbg_env ? atoi(dbg_env) : 0;
     const int s8 = TcTraits<KIND_I8>::SMEM_BYTES, s4 = TcTraits<KIND_FP4>::SMEM_BYTES;
+#define CSG_LAUNCH(KERNEL, SMEM) \
+    KERNEL<<<grid, TC_THREADS, SMEM, stream>>>(*map, rel_bits, N, stride, kmax, c64, d_tiles, ntiles, g.debug, progress, rows_ready, dump)
     // int8: operand bit TB: the accumulator holds n_ij << 2TB and n_ij <= N-2, so TB is the largest with
     // (N-2) << 2TB < 2^31; TB = 7 turns every unpack shift into a left shift (FMA pipe).
-    if (kind == KIND_FP4 && dbg != 0)   // timing ablations only (wrong counts)
-        tensor_action_kernel<KIND_FP4, 0, true><<<grid, TC_THREADS, s4, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, d_tiles, ntiles, dbg, progress);
-    else if (kind == KIND_FP4 && progress != nullptr)
-        tensor_action_kernel<KIND_FP4, 0, false, true><<<grid, TC_THREADS, s4, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, d_tiles, ntiles, dbg, progress);
-    else if (kind == KIND_FP4)
-        tensor_action_kernel<KIND_FP4, 0><<<grid, TC_THREADS, s4, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, d_tiles, ntiles, dbg, progress);
-    else if (N - 2 < (1LL << 17))
-        tensor_action_kernel<KIND_I8, 7><<<grid, TC_THREADS, s8, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, d_tiles, ntiles, dbg, progress);
-    else if (N - 2 < (1LL << 19))
-        tensor_action_kernel<KIND_I8, 6><<<grid, TC_THREADS, s8, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, d_tiles, ntiles, dbg, progress);
-    else if (N - 2 < (1LL << 21))
-        tensor_action_kernel<KIND_I8, 5><<<grid, TC_THREADS, s8, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, d_tiles, ntiles, dbg, progress);
-    else
-        tensor_action_kernel<KIND_I8, 4><<<grid, TC_THREADS, s8, stream>>>(g.bits_map[kind], rel_bits, N, stride, kmax, c64, d_tiles, ntiles, dbg, progress);
+    const int tb = N - 2 < (1LL << 17) ? 7 : N - 2 < (1LL << 19) ? 6 : N - 2 < (1LL << 21) ? 5 : 4;
+    if (kind == KIND_FP4) {
+        if (dump) CSG_LAUNCH((tensor_action_kernel<KIND_FP4, 0, TCF_DUMP>), s4);
+        else if (progress || rows_ready) CSG_LAUNCH((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA | TCF_WAIT>), s4);
+        else CSG_LAUNCH((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA>), s4);
+    } else if (dump) {
+        if (tb == 7) CSG_LAUNCH((tensor_action_kernel<KIND_I8, 7, TCF_DUMP>), s8);
+        else if (tb == 6) CSG_LAUNCH((tensor_action_kernel<KIND_I8, 6, TCF_DUMP>), s8);
+        else if (tb == 5) CSG_LAUNCH((tensor_action_kernel<KIND_I8, 5, TCF_DUMP>), s8);
+        else CSG_LAUNCH((tensor_action_kernel<KIND_I8, 4, TCF_DUMP>), s8);
+    } else {
+        if (tb == 7) CSG_LAUNCH((tensor_action_kernel<KIND_I8, 7>), s8);
+        else if (tb == 6) CSG_LAUNCH((tensor_action_kernel<KIND_I8, 6>), s8);
+        else if (tb == 5) CSG_LAUNCH((tensor_action_kernel<KIND_I8, 5>), s8);
+        else CSG_LAUNCH((tensor_action_kernel<KIND_I8, 4>), s8);
+    }
+#undef CSG_LAUNCH
     CSG_CUDA(cudaGetLastError());
     ++g.launches;
     return CSG_OK;
 }
 
-static int interval_device(const uint64_t* rel_bits, long long N, int kmax, int shard, int nshards,
+// Interval kernel over the tiles of one shard: counts (kmax+1 int64, overwritten) <- this shard's abundances.
+static int interval_device(Device* D, const uint64_t* rel_bits, long long N, int kmax, int shard, int nshards,
                            long long* counts, cudaStream_t stream) {
-    int rc = ensure_device();
-    if (rc) return rc;
     const long long stride = csg_row_stride_words(N);
     CSG_CUDA(cudaMemsetAsync(counts, 0, (size_t)(kmax + 1) * sizeof(long long), stream));
     const int variant = effective_variant(N);
     const bool tensor = variant == CSG_VARIANT_TENSOR || variant == CSG_VARIANT_TENSOR_FP4;
     const int kind = variant == CSG_VARIANT_TENSOR_FP4 ? KIND_FP4 : KIND_I8;
+    const TileList* tl = nullptr;
+    int rc;
     if (tensor) {
-        rc = ensure_tiles(N, shard, nshards, stream);
-        if (rc) return rc;
-        rc = ensure_tensor_ready(kind, rel_bits, N, stride);
+        rc = ensure_tiles(D, N, shard, nshards, &tl);
         if (rc) return rc;
     }
-    const int slot = (int)(g.timed_calls % TIMING_RING);
+    const int slot = (int)(D->timed_calls % TIMING_RING);
     if (g.timing) {
-        if (!g.ev0[slot]) {
-            CSG_CUDA(cudaEventCreate(&g.ev0[slot]));
-            CSG_CUDA(cudaEventCreate(&g.ev1[slot]));
+        if (!D->ev0[slot]) {
+            CSG_CUDA(cudaEventCreate(&D->ev0[slot]));
+            CSG_CUDA(cudaEventCreate(&D->ev1[slot]));
         }
-        CSG_CUDA(cudaEventRecord(g.ev0[slot], stream));
+        CSG_CUDA(cudaEventRecord(D->ev0[slot], stream));
     }
     if (tensor) {
-        rc = launch_tensor(kind, rel_bits, N, stride, kmax, counts, g.d_tiles, g.ntiles, stream);
+        rc = launch_tensor(D, kind, rel_bits, N, stride, kmax, counts, tl->d, tl->n, nullptr, nullptr, stream);
         if (rc) return rc;
     } else {
         const long long nb = (N + BS_T - 1) / BS_T;
         const long long ntiles = nb * (nb + 1) / 2;
         const long long mine = (ntiles - shard + nshards - 1) / nshards;   // tiles t = shard (mod nshards)
-        const int grid = (int)std::max<long long>(1, std::min<long long>(mine, (long long)g.sm_count * 2));
+        const int grid = (int)std::max<long long>(1, std::min<long long>(mine, (long long)D->sm_count * 2));
         bitset_action_kernel<<<grid, BS_THREADS, 0, stream>>>(reinterpret_cast<const uint32_t*>(rel_bits), N,
                                                                stride * 2, kmax,
                                                                reinterpret_cast<unsigned long long*>(counts), nb,
@@ -387,39 +479,46 @@ static int interval_device(const uint64_t* rel_bits, long long N, int kmax, int 
         ++g.launches;
     }
     if (g.timing) {
-        CSG_CUDA(cudaEventRecord(g.ev1[slot], stream));
-        ++g.timed_calls;
+        CSG_CUDA(cudaEventRecord(D->ev1[slot], stream));
+        ++D->timed_calls;
     }
     return CSG_OK;
 }
 
 static int finish_device(const long long* counts, long long N, int dim, double eps, int kmax, double* S,
                          cudaStream_t stream) {
-    int rc = ensure_device();
-    if (rc) return rc;
     finish_action_kernel<<<1, FIN_THREADS, 0, stream>>>(counts, N, dim, eps, kmax, S);
     CSG_CUDA(cudaGetLastError());
     ++g.launches;
     return CSG_OK;
 }
 
-static int action_device(const uint64_t* rel_bits, long long N, int dim, double eps, int kmax, long long* counts,
-                         double* S, cudaStream_t stream) {
-    int rc = interval_device(rel_bits, N, kmax, 0, 1, counts, stream);
+static int action_device(Device* D, const uint64_t* rel_bits, long long N, int dim, double eps, int kmax,
+                         long long* counts, double* S, cudaStream_t stream) {
+    int rc = interval_device(D, rel_bits, N, kmax, 0, 1, counts, stream);
     if (rc) return rc;
     return finish_device(counts, N, dim, eps, kmax, S, stream);
 }
 
-// Host matrix -> device in row chunks, the tiles whose LATER row block lies in a chunk launched as soon as that chunk
-// has landed (a tile (I, J) reads rows of blocks I <= J only).  The work of chunk c grows like (c+1)^2 - c^2, so the
-// copies of all but the first chunks hide behind the tiles of the chunks before them: the 2 GiB copy of N = 131072
-// (38 ms over PCIe) costs a few ms instead.  Tensor variants and large matrices only; counts must be zeroed by the
-// caller of this function on `stream` beforehand (done here).
+// Host matrix -> device in row chunks on a copy stream while the tiles already run (Sec. 2.2.5:
+// overlap of transfers with compute).  A tile (I, J) reads rows of blocks I <= J only, and the work of chunk c grows
+// like (c+1)^2 - c^2, so the copies of all but the first chunks hide behind the tiles of the chunks before them: the
+// 2 GiB copy of N = 131072 (38 ms over PCIe) costs a few ms instead.  The tile list is ordered by the chunk that holds
+// a tile's later row block (inside a chunk: deepest first, patch order).  Two ways to run it:
+//   gated (fp4 kind, when the driver offers cuStreamWriteValue32): ONE persistent launch; after every chunk the copy
+//     stream publishes the number of rows landed and the TMA thread of a cluster waits for the rows its next tile
+//     needs -- no launch tails between chunks;
+//   chunked launches (int8 kind, or no stream memory operations): one launch per chunk behind an event.
+// Tensor variants and large matrices only.
 constexpr int HOST_CHUNKS = 32;
 constexpr long long HOST_PIPELINE_MIN_BYTES = 32LL << 20;
 
-static int ensure_chunk_tiles(long long N, cudaStream_t stream) {
-    if (g.chunk_N == N && g.d_chunk_tiles) return CSG_OK;
+static int ensure_chunk_tiles(Device* D, long long N, const ChunkTiles** out) {
+    for (const ChunkTiles* c : D->chunk_tiles)
+        if (c->N == N) {
+            *out = c;
+            return CSG_OK;
+        }
     const int nB = (int)((N + TC_T - 1) / TC_T);
     const int blocks_per_chunk = (nB + HOST_CHUNKS - 1) / HOST_CHUNKS;
     const int nchunks = (nB + blocks_per_chunk - 1) / blocks_per_chunk;
@@ -428,54 +527,91 @@ static int ensure_chunk_tiles(long long N, cudaStream_t stream) {
     std::vector<std::vector<int2>> per(nchunks);
     for (const int2& t : all) per[t.y / blocks_per_chunk].push_back(t);   // keeps the deepest-first, patch order
     std::vector<int2> flat;
-    g.chunk_off.assign(1, 0);
-    g.chunk_row_end.clear();
-    for (int c = 0; c < nchunks; ++c) {
-        flat.insert(flat.end(), per[c].begin(), per[c].end());
-        g.chunk_off.push_back((int)flat.size());
-        g.chunk_row_end.push_back(std::min<long long>(N, (long long)(c + 1) * blocks_per_chunk * TC_T));
+    ChunkTiles* c = new ChunkTiles;
+    c->N = N;
+    c->d = nullptr;
+    c->off.assign(1, 0);
+    for (int k = 0; k < nchunks; ++k) {
+        flat.insert(flat.end(), per[k].begin(), per[k].end());
+        c->off.push_back((int)flat.size());
+        c->row_end.push_back(std::min<long long>(N, (long long)(k + 1) * blocks_per_chunk * TC_T));
     }
-    if (g.d_chunk_tiles) {
-        CSG_CUDA(cudaStreamSynchronize(stream));
-        CSG_CUDA(cudaFree(g.d_chunk_tiles));
-        g.d_chunk_tiles = nullptr;
+    c->n = (int)flat.size();
+    cudaError_t e = cudaMalloc(&c->d, flat.size() * sizeof(int2));
+    if (e == cudaSuccess) e = cudaMemcpy(c->d, flat.data(), flat.size() * sizeof(int2), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) {
+        if (c->d) cudaFree(c->d);
+        delete c;
+        return cuda_fail(e, "tile list of the host pipeline");
     }
-    CSG_CUDA(cudaMalloc(&g.d_chunk_tiles, flat.size() * sizeof(int2)));
-    CSG_CUDA(cudaMemcpyAsync(g.d_chunk_tiles, flat.data(), flat.size() * sizeof(int2), cudaMemcpyHostToDevice, stream));
-    CSG_CUDA(cudaStreamSynchronize(stream));   // `flat` is a local
-    while ((int)g.chunk_ev.size() < nchunks + 1) {
-        cudaEvent_t e;
-        CSG_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
-        g.chunk_ev.push_back(e);
+    while ((int)D->chunk_ev.size() < nchunks + 2) {
+        cudaEvent_t ev;
+        CSG_CUDA(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+        D->chunk_ev.push_back(ev);
     }
-    g.chunk_N = N;
+    D->chunk_tiles.push_back(c);
+    *out = c;
     return CSG_OK;
 }
 
-static int interval_host_pipelined(const uint64_t* rel_bits_host, uint64_t* d_bits, long long N, int kmax, int kind,
-                                   long long* counts, cudaStream_t stream) {
+static WriteValue32Fn stream_write_value32() {
+    if (!g.write_value32_tried) {
+        g.write_value32_tried = true;
+        cudaDriverEntryPointQueryResult qres;
+        void* fn = nullptr;
+        if (cudaGetDriverEntryPoint("cuStreamWriteValue32", &fn, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            g.write_value32 = fn;
+        else
+            cudaGetLastError();
+    }
+    return reinterpret_cast<WriteValue32Fn>(g.write_value32);
+}
+
+static int interval_host_pipelined(Device* D, const uint64_t* rel_bits_host, uint64_t* d_bits, long long N, int kmax,
+                                   int kind, long long* counts, cudaStream_t stream) {
     const long long stride = csg_row_stride_words(N);
-    int rc = ensure_chunk_tiles(N, stream);
+    const ChunkTiles* ct = nullptr;
+    int rc = ensure_chunk_tiles(D, N, &ct);
     if (rc) return rc;
-    rc = ensure_tensor_ready(kind, d_bits, N, stride);
-    if (rc) return rc;
-    if (!g.copy_stream) CSG_CUDA(cudaStreamCreateWithFlags(&g.copy_stream, cudaStreamNonBlocking));
+    if (!D->copy_stream) CSG_CUDA(cudaStreamCreateWithFlags(&D->copy_stream, cudaStreamNonBlocking));
     CSG_CUDA(cudaMemsetAsync(counts, 0, (size_t)(kmax + 1) * sizeof(long long), stream));
+    const int nchunks = (int)ct->row_end.size();
+    cudaEvent_t ev_prev = D->chunk_ev[nchunks], ev_reset = D->chunk_ev[nchunks + 1];
     // the copies must not overtake work of an earlier call that still reads d_bits on `stream`
-    CSG_CUDA(cudaEventRecord(g.chunk_ev.back(), stream));
-    CSG_CUDA(cudaStreamWaitEvent(g.copy_stream, g.chunk_ev.back(), 0));
-    const int nchunks = (int)g.chunk_row_end.size();
+    CSG_CUDA(cudaEventRecord(ev_prev, stream));
+    CSG_CUDA(cudaStreamWaitEvent(D->copy_stream, ev_prev, 0));
+    WriteValue32Fn write32 = kind == KIND_FP4 ? stream_write_value32() : nullptr;
+    if (write32) {
+        if (!D->d_rows_ready) CSG_CUDA(cudaMalloc(&D->d_rows_ready, sizeof(unsigned int)));
+        // reset the gate, then ONE launch that starts at once and follows the copies
+        if (write32(D->copy_stream, (CUdeviceptr)D->d_rows_ready, 0u, 0) != CUDA_SUCCESS) {
+            write32 = nullptr;                                 // no stream memory operations here: chunked launches
+        } else {
+            CSG_CUDA(cudaEventRecord(ev_reset, D->copy_stream));
+            CSG_CUDA(cudaStreamWaitEvent(stream, ev_reset, 0));
+            rc = launch_tensor(D, kind, d_bits, N, stride, kmax, counts, ct->d, ct->n, D->d_rows_ready, nullptr, stream);
+            if (rc) return rc;
+        }
+    }
     long long row0 = 0;
     for (int c = 0; c < nchunks; ++c) {
-        const long long row1 = g.chunk_row_end[c];
+        const long long row1 = ct->row_end[c];
         CSG_CUDA(cudaMemcpyAsync(d_bits + row0 * stride, rel_bits_host + row0 * stride,
-                                 (size_t)(row1 - row0) * stride * sizeof(uint64_t), cudaMemcpyHostToDevice, g.copy_stream));
-        CSG_CUDA(cudaEventRecord(g.chunk_ev[c], g.copy_stream));
-        CSG_CUDA(cudaStreamWaitEvent(stream, g.chunk_ev[c], 0));
-        const int nt = g.chunk_off[c + 1] - g.chunk_off[c];
-        if (nt > 0) {
-            rc = launch_tensor(kind, d_bits, N, stride, kmax, counts, g.d_chunk_tiles + g.chunk_off[c], nt, stream);
-            if (rc) return rc;
+                                 (size_t)(row1 - row0) * stride * sizeof(uint64_t), cudaMemcpyHostToDevice, D->copy_stream));
+        if (write32) {
+            if (write32(D->copy_stream, (CUdeviceptr)D->d_rows_ready, (cuuint32_t)row1, 0) != CUDA_SUCCESS) {
+                snprintf(g.cuda_msg, sizeof(g.cuda_msg), "cuStreamWriteValue32 failed while a gated launch is waiting");
+                return CSG_E_CUDA;
+            }
+        } else {
+            CSG_CUDA(cudaEventRecord(D->chunk_ev[c], D->copy_stream));
+            CSG_CUDA(cudaStreamWaitEvent(stream, D->chunk_ev[c], 0));
+            const int nt = ct->off[c + 1] - ct->off[c];
+            if (nt > 0) {
+                rc = launch_tensor(D, kind, d_bits, N, stride, kmax, counts, ct->d + ct->off[c], nt, nullptr, nullptr, stream);
+                if (rc) return rc;
+            }
         }
         row0 = row1;
     }
@@ -485,18 +621,17 @@ static int interval_host_pipelined(const uint64_t* rel_bits_host, uint64_t* d_bi
 static int geometry_dim(int geometry) { return geometry == CSG_GEOM_MINKOWSKI_4D ? 4 : 2; }
 
 // Linking kernel on `stream`: every word of rel_bits (N rows x stride) is overwritten.
-static int link_device(const double* coords, long long N, int geometry, uint64_t* rel_bits, cudaStream_t stream) {
-    int rc = ensure_device();
-    if (rc) return rc;
+static int link_device(Device* D, const double* coords, long long N, int geometry, uint64_t* rel_bits,
+                       cudaStream_t stream) {
     const long long stride = csg_row_stride_words(N);
     const int nB = (int)((N + LK_T - 1) / LK_T);
     const long long ntiles = (long long)nB * (nB + 1) / 2;
     if (g.timing) {
-        if (!g.link_ev0) {
-            CSG_CUDA(cudaEventCreate(&g.link_ev0));
-            CSG_CUDA(cudaEventCreate(&g.link_ev1));
+        if (!D->link_ev0) {
+            CSG_CUDA(cudaEventCreate(&D->link_ev0));
+            CSG_CUDA(cudaEventCreate(&D->link_ev1));
         }
-        CSG_CUDA(cudaEventRecord(g.link_ev0, stream));
+        CSG_CUDA(cudaEventRecord(D->link_ev0, stream));
     }
     if (geometry == CSG_GEOM_MINKOWSKI_2D)
         link_kernel<GEOM_M2><<<(unsigned)ntiles, LK_THREADS, 0, stream>>>(coords, N, stride, rel_bits, nB);
@@ -507,12 +642,14 @@ static int link_device(const double* coords, long long N, int geometry, uint64_t
     CSG_CUDA(cudaGetLastError());
     ++g.launches;
     if (g.timing) {
-        CSG_CUDA(cudaEventRecord(g.link_ev1, stream));
-        g.link_timed = true;
+        CSG_CUDA(cudaEventRecord(D->link_ev1, stream));
+        D->link_timed = true;
     }
     return CSG_OK;
 }
 
+// Library-owned device buffer of the host entry points; grows, never shrinks.  Growing frees the old buffer, which
+// is safe here because those entry points synchronise their stream before they return.
 static int ensure_buffer(void** ptr, size_t* have, size_t want) {
     if (*have >= want) return CSG_OK;
     if (*ptr) CSG_CUDA(cudaFree(*ptr));
@@ -521,6 +658,30 @@ static int ensure_buffer(void** ptr, size_t* have, size_t want) {
     CSG_CUDA(cudaMalloc(ptr, want));
     *have = want;
     return CSG_OK;
+}
+
+static void release_device(Device* D) {
+    for (TileList& t : D->tiles) cudaFree(t.d);
+    for (ChunkTiles* c : D->chunk_tiles) {
+        cudaFree(c->d);
+        delete c;
+    }
+    if (D->d_bits) cudaFree(D->d_bits);
+    if (D->d_counts) cudaFree(D->d_counts);
+    if (D->d_S) cudaFree(D->d_S);
+    if (D->d_coords) cudaFree(D->d_coords);
+    if (D->d_progress) cudaFree(D->d_progress);
+    if (D->d_rows_ready) cudaFree(D->d_rows_ready);
+    for (cudaEvent_t e : D->chunk_ev) cudaEventDestroy(e);
+    if (D->copy_stream) cudaStreamDestroy(D->copy_stream);
+    if (D->host_stream) cudaStreamDestroy(D->host_stream);
+    if (D->link_ev0) cudaEventDestroy(D->link_ev0);
+    if (D->link_ev1) cudaEventDestroy(D->link_ev1);
+    for (int k = 0; k < TIMING_RING; ++k) {
+        if (D->ev0[k]) cudaEventDestroy(D->ev0[k]);
+        if (D->ev1[k]) cudaEventDestroy(D->ev1[k]);
+    }
+    delete D;
 }
 
 }  // namespace csg
@@ -539,7 +700,9 @@ int csg_action(const uint64_t* rel_bits, int64_t N, int dim, double eps, int kma
     if ((reinterpret_cast<uintptr_t>(rel_bits) & 15) || (reinterpret_cast<uintptr_t>(counts) & 7) ||
         (reinterpret_cast<uintptr_t>(S) & 7))
         return CSG_E_ALIGN;
-    return action_device(rel_bits, N, dim, eps, kmax, reinterpret_cast<long long*>(counts), S, stream);
+    Device* D = nullptr;
+    if ((rc = current_device(&D))) return rc;
+    return action_device(D, rel_bits, N, dim, eps, kmax, reinterpret_cast<long long*>(counts), S, stream);
 }
 
 int csg_action_partial(const uint64_t* rel_bits, int64_t N, int kmax, int shard, int nshards, int64_t* counts,
@@ -550,7 +713,10 @@ int csg_action_partial(const uint64_t* rel_bits, int64_t N, int kmax, int shard,
     if (kmax < 0 || kmax > CSG_MAX_KMAX) return CSG_E_KMAX;
     if (nshards < 1 || shard < 0 || shard >= nshards) return CSG_E_SHARD;
     if ((reinterpret_cast<uintptr_t>(rel_bits) & 15) || (reinterpret_cast<uintptr_t>(counts) & 7)) return CSG_E_ALIGN;
-    return interval_device(rel_bits, N, kmax, shard, nshards, reinterpret_cast<long long*>(counts), stream);
+    Device* D = nullptr;
+    int rc = current_device(&D);
+    if (rc) return rc;
+    return interval_device(D, rel_bits, N, kmax, shard, nshards, reinterpret_cast<long long*>(counts), stream);
 }
 
 int csg_action_finish(const int64_t* counts, int64_t N, int dim, double eps, int kmax, double* S,
@@ -559,6 +725,8 @@ int csg_action_finish(const int64_t* counts, int64_t N, int dim, double eps, int
     int rc = validate(counts, N, dim, eps, kmax, counts, S);
     if (rc) return rc;
     if ((reinterpret_cast<uintptr_t>(counts) & 7) || (reinterpret_cast<uintptr_t>(S) & 7)) return CSG_E_ALIGN;
+    Device* D = nullptr;
+    if ((rc = current_device(&D))) return rc;
     return finish_device(reinterpret_cast<const long long*>(counts), N, dim, eps, kmax, S, stream);
 }
 
@@ -571,8 +739,8 @@ int csg_action_batch(const uint64_t* rel_bits, int64_t N, int64_t batch, int dim
     if ((reinterpret_cast<uintptr_t>(rel_bits) & 15) || (reinterpret_cast<uintptr_t>(counts) & 7) ||
         (reinterpret_cast<uintptr_t>(S) & 7))
         return CSG_E_ALIGN;
-    rc = ensure_device();
-    if (rc) return rc;
+    Device* D = nullptr;
+    if ((rc = current_device(&D))) return rc;
     const long long stride = csg_row_stride_words(N);
     const long long set_words = N * stride;
     long long* c = reinterpret_cast<long long*>(counts);
@@ -583,7 +751,7 @@ int csg_action_batch(const uint64_t* rel_bits, int64_t N, int64_t batch, int dim
         CSG_CUDA(cudaMemsetAsync(c, 0, (size_t)batch * (kmax + 1) * sizeof(long long), stream));
         const long long nb = (N + BS_T - 1) / BS_T;
         const long long ntiles = nb * (nb + 1) / 2;
-        const long long per_set = std::max<long long>(1, (2LL * g.sm_count + batch - 1) / batch);
+        const long long per_set = std::max<long long>(1, (2LL * D->sm_count + batch - 1) / batch);
         const dim3 grid((unsigned)std::min<long long>(ntiles, per_set), (unsigned)batch);
         bitset_action_kernel<<<grid, BS_THREADS, 0, stream>>>(reinterpret_cast<const uint32_t*>(rel_bits), N, stride * 2,
                                                                kmax, reinterpret_cast<unsigned long long*>(c), nb, ntiles,
@@ -593,7 +761,7 @@ int csg_action_batch(const uint64_t* rel_bits, int64_t N, int64_t batch, int dim
     } else {
         // large sets fill the machine on their own: one tensor launch per set, back to back on the stream
         for (int64_t b = 0; b < batch; ++b) {
-            rc = interval_device(rel_bits + b * set_words, N, kmax, 0, 1, c + b * (kmax + 1), stream);
+            rc = interval_device(D, rel_bits + b * set_words, N, kmax, 0, 1, c + b * (kmax + 1), stream);
             if (rc) return rc;
         }
     }
@@ -621,40 +789,32 @@ int csg_action_host(const uint64_t* rel_bits_host, int64_t N, int dim, double ep
     std::lock_guard<std::mutex> lock(g.mu);
     int rc = validate(rel_bits_host, N, dim, eps, kmax, counts_host, S_host);
     if (rc) return rc;
-    rc = ensure_device();
-    if (rc) return rc;
-    if (!g.host_stream) CSG_CUDA(cudaStreamCreateWithFlags(&g.host_stream, cudaStreamNonBlocking));
+    Device* D = nullptr;
+    if ((rc = current_device(&D))) return rc;
+    if (!D->host_stream) CSG_CUDA(cudaStreamCreateWithFlags(&D->host_stream, cudaStreamNonBlocking));
     const size_t bits_bytes = (size_t)N * (size_t)csg_row_stride_words(N) * sizeof(uint64_t);
     const size_t counts_bytes = (size_t)(kmax + 1) * sizeof(long long);
-    if (g.d_bits_bytes < bits_bytes) {
-        if (g.d_bits) CSG_CUDA(cudaFree(g.d_bits));
-        g.d_bits = nullptr;
-        g.d_bits_bytes = 0;
-        CSG_CUDA(cudaMalloc(&g.d_bits, bits_bytes));
-        g.d_bits_bytes = bits_bytes;
-    }
-    if (g.d_counts_bytes < counts_bytes) {
-        if (g.d_counts) CSG_CUDA(cudaFree(g.d_counts));
-        g.d_counts = nullptr;
-        g.d_counts_bytes = 0;
-        CSG_CUDA(cudaMalloc(&g.d_counts, counts_bytes));
-        g.d_counts_bytes = counts_bytes;
-    }
-    if (!g.d_S) CSG_CUDA(cudaMalloc(&g.d_S, sizeof(double)));
+    if ((rc = ensure_buffer(reinterpret_cast<void**>(&D->d_bits), &D->d_bits_bytes, bits_bytes))) return rc;
+    if ((rc = ensure_buffer(reinterpret_cast<void**>(&D->d_counts), &D->d_counts_bytes, counts_bytes))) return rc;
+    if (!D->d_S) CSG_CUDA(cudaMalloc(&D->d_S, sizeof(double)));
     const int variant = effective_variant(N);
     if (variant != CSG_VARIANT_BITSET && bits_bytes >= (size_t)HOST_PIPELINE_MIN_BYTES) {
-        rc = interval_host_pipelined(rel_bits_host, g.d_bits, N, kmax, variant == CSG_VARIANT_TENSOR_FP4 ? KIND_FP4 : KIND_I8,
-                                     g.d_counts, g.host_stream);
-        if (rc) return rc;
-        rc = finish_device(g.d_counts, N, dim, eps, kmax, g.d_S, g.host_stream);
+        rc = interval_host_pipelined(D, rel_bits_host, D->d_bits, N, kmax,
+                                     variant == CSG_VARIANT_TENSOR_FP4 ? KIND_FP4 : KIND_I8, D->d_counts, D->host_stream);
+        if (rc) {
+            cudaStreamSynchronize(D->host_stream);     // never leave a gated launch or a copy behind an error return
+            cudaStreamSynchronize(D->copy_stream);
+            return rc;
+        }
+        rc = finish_device(D->d_counts, N, dim, eps, kmax, D->d_S, D->host_stream);
     } else {
-        CSG_CUDA(cudaMemcpyAsync(g.d_bits, rel_bits_host, bits_bytes, cudaMemcpyHostToDevice, g.host_stream));
-        rc = action_device(g.d_bits, N, dim, eps, kmax, g.d_counts, g.d_S, g.host_stream);
+        CSG_CUDA(cudaMemcpyAsync(D->d_bits, rel_bits_host, bits_bytes, cudaMemcpyHostToDevice, D->host_stream));
+        rc = action_device(D, D->d_bits, N, dim, eps, kmax, D->d_counts, D->d_S, D->host_stream);
     }
     if (rc) return rc;
-    CSG_CUDA(cudaMemcpyAsync(counts_host, g.d_counts, counts_bytes, cudaMemcpyDeviceToHost, g.host_stream));
-    CSG_CUDA(cudaMemcpyAsync(S_host, g.d_S, sizeof(double), cudaMemcpyDeviceToHost, g.host_stream));
-    CSG_CUDA(cudaStreamSynchronize(g.host_stream));
+    CSG_CUDA(cudaMemcpyAsync(counts_host, D->d_counts, counts_bytes, cudaMemcpyDeviceToHost, D->host_stream));
+    CSG_CUDA(cudaMemcpyAsync(S_host, D->d_S, sizeof(double), cudaMemcpyDeviceToHost, D->host_stream));
+    CSG_CUDA(cudaStreamSynchronize(D->host_stream));
     return CSG_OK;
 }
 
@@ -664,7 +824,10 @@ int csg_link(const double* coords, int64_t N, int geometry, uint64_t* rel_bits, 
     if (N < 1 || N > CSG_MAX_N) return CSG_E_SIZE;
     if (geometry < CSG_GEOM_MINKOWSKI_2D || geometry > CSG_GEOM_DESITTER_2D) return CSG_E_GEOMETRY;
     if ((reinterpret_cast<uintptr_t>(rel_bits) & 15) || (reinterpret_cast<uintptr_t>(coords) & 7)) return CSG_E_ALIGN;
-    return link_device(coords, N, geometry, rel_bits, stream);
+    Device* D = nullptr;
+    int rc = current_device(&D);
+    if (rc) return rc;
+    return link_device(D, coords, N, geometry, rel_bits, stream);
 }
 
 int csg_causet_action_host(const double* coords_host, int64_t N, int geometry, double eps, int kmax,
@@ -674,36 +837,39 @@ int csg_causet_action_host(const double* coords_host, int64_t N, int geometry, d
     const int dim = geometry_dim(geometry);
     int rc = validate(coords_host, N, dim, eps, kmax, counts_host, S_host);
     if (rc) return rc;
-    rc = ensure_device();
-    if (rc) return rc;
-    if (!g.host_stream) CSG_CUDA(cudaStreamCreateWithFlags(&g.host_stream, cudaStreamNonBlocking));
+    Device* D = nullptr;
+    if ((rc = current_device(&D))) return rc;
+    if (!D->host_stream) CSG_CUDA(cudaStreamCreateWithFlags(&D->host_stream, cudaStreamNonBlocking));
     const size_t coords_bytes = (size_t)N * dim * sizeof(double);
     const size_t bits_bytes = (size_t)N * (size_t)csg_row_stride_words(N) * sizeof(uint64_t);
     const size_t counts_bytes = (size_t)(kmax + 1) * sizeof(long long);
-    if ((rc = ensure_buffer(reinterpret_cast<void**>(&g.d_coords), &g.d_coords_bytes, coords_bytes))) return rc;
-    if ((rc = ensure_buffer(reinterpret_cast<void**>(&g.d_bits), &g.d_bits_bytes, bits_bytes))) return rc;
-    if ((rc = ensure_buffer(reinterpret_cast<void**>(&g.d_counts), &g.d_counts_bytes, counts_bytes))) return rc;
-    if (!g.d_S) CSG_CUDA(cudaMalloc(&g.d_S, sizeof(double)));
-    CSG_CUDA(cudaMemcpyAsync(g.d_coords, coords_host, coords_bytes, cudaMemcpyHostToDevice, g.host_stream));
-    rc = link_device(g.d_coords, N, geometry, g.d_bits, g.host_stream);
+    if ((rc = ensure_buffer(reinterpret_cast<void**>(&D->d_coords), &D->d_coords_bytes, coords_bytes))) return rc;
+    if ((rc = ensure_buffer(reinterpret_cast<void**>(&D->d_bits), &D->d_bits_bytes, bits_bytes))) return rc;
+    if ((rc = ensure_buffer(reinterpret_cast<void**>(&D->d_counts), &D->d_counts_bytes, counts_bytes))) return rc;
+    if (!D->d_S) CSG_CUDA(cudaMalloc(&D->d_S, sizeof(double)));
+    CSG_CUDA(cudaMemcpyAsync(D->d_coords, coords_host, coords_bytes, cudaMemcpyHostToDevice, D->host_stream));
+    rc = link_device(D, D->d_coords, N, geometry, D->d_bits, D->host_stream);
     if (rc) return rc;
-    rc = action_device(g.d_bits, N, dim, eps, kmax, g.d_counts, g.d_S, g.host_stream);
+    rc = action_device(D, D->d_bits, N, dim, eps, kmax, D->d_counts, D->d_S, D->host_stream);
     if (rc) return rc;
-    CSG_CUDA(cudaMemcpyAsync(counts_host, g.d_counts, counts_bytes, cudaMemcpyDeviceToHost, g.host_stream));
-    CSG_CUDA(cudaMemcpyAsync(S_host, g.d_S, sizeof(double), cudaMemcpyDeviceToHost, g.host_stream));
-    CSG_CUDA(cudaStreamSynchronize(g.host_stream));
+    CSG_CUDA(cudaMemcpyAsync(counts_host, D->d_counts, counts_bytes, cudaMemcpyDeviceToHost, D->host_stream));
+    CSG_CUDA(cudaMemcpyAsync(S_host, D->d_S, sizeof(double), cudaMemcpyDeviceToHost, D->host_stream));
+    CSG_CUDA(cudaStreamSynchronize(D->host_stream));
     return CSG_OK;
 }
 
 int csg_last_link_ms(float* ms) {
     std::lock_guard<std::mutex> lock(g.mu);
     if (!ms) return CSG_E_NULL;
-    if (!g.link_timed) {
+    Device* D = nullptr;
+    int rc = current_device(&D);
+    if (rc) return rc;
+    if (!D->link_timed) {
         snprintf(g.cuda_msg, sizeof(g.cuda_msg), "kernel timing: no timed csg_link call so far");
         return CSG_E_CUDA;
     }
-    CSG_CUDA(cudaEventSynchronize(g.link_ev1));
-    CSG_CUDA(cudaEventElapsedTime(ms, g.link_ev0, g.link_ev1));
+    CSG_CUDA(cudaEventSynchronize(D->link_ev1));
+    CSG_CUDA(cudaEventElapsedTime(ms, D->link_ev0, D->link_ev1));
     return CSG_OK;
 }
 
@@ -713,7 +879,8 @@ int csg_interval_sizes(const uint64_t* rel_bits, int64_t N, const int64_t* pairs
     if (!rel_bits || (npairs > 0 && (!pairs_ij || !n_out))) return CSG_E_NULL;
     if (N < 1 || N > CSG_MAX_N || npairs < 0) return CSG_E_SIZE;
     if (reinterpret_cast<uintptr_t>(rel_bits) & 15) return CSG_E_ALIGN;
-    int rc = ensure_device();
+    Device* D = nullptr;
+    int rc = current_device(&D);
     if (rc) return rc;
     if (npairs == 0) return CSG_OK;
     const int warps_per_block = 8;
@@ -724,6 +891,36 @@ int csg_interval_sizes(const uint64_t* rel_bits, int64_t N, const int64_t* pairs
     CSG_CUDA(cudaGetLastError());
     ++g.launches;
     return CSG_OK;
+}
+
+int csg_tile_interval_sizes(const uint64_t* rel_bits, int64_t N, const int32_t* tiles_ij_host, int64_t ntiles,
+                            int32_t* n_out, cudaStream_t stream) {
+    std::lock_guard<std::mutex> lock(g.mu);
+    if (!rel_bits || (ntiles > 0 && (!tiles_ij_host || !n_out))) return CSG_E_NULL;
+    if (N < 1 || N > CSG_MAX_N || ntiles < 0 || ntiles > (1 << 15)) return CSG_E_SIZE;
+    if ((reinterpret_cast<uintptr_t>(rel_bits) & 15) || (reinterpret_cast<uintptr_t>(n_out) & 3)) return CSG_E_ALIGN;
+    const int nB = (int)((N + TC_T - 1) / TC_T);
+    for (int64_t t = 0; t < ntiles; ++t)
+        if (tiles_ij_host[2 * t] < 0 || tiles_ij_host[2 * t] > tiles_ij_host[2 * t + 1] || tiles_ij_host[2 * t + 1] >= nB)
+            return CSG_E_SIZE;
+    const int variant = effective_variant(N);
+    if (variant == CSG_VARIANT_BITSET) return CSG_E_UNSUPPORTED;
+    Device* D = nullptr;
+    int rc = current_device(&D);
+    if (rc) return rc;
+    if (ntiles == 0) return CSG_OK;
+    // a test hook: temporary tile list, synchronous
+    int2* d_tiles = nullptr;
+    CSG_CUDA(cudaMalloc(&d_tiles, (size_t)ntiles * sizeof(int2)));
+    cudaError_t e = cudaMemcpy(d_tiles, tiles_ij_host, (size_t)ntiles * sizeof(int2), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        rc = launch_tensor(D, variant == CSG_VARIANT_TENSOR_FP4 ? KIND_FP4 : KIND_I8, rel_bits, N, csg_row_stride_words(N),
+                           0, nullptr, d_tiles, (int)ntiles, nullptr, n_out, stream);
+        e = cudaStreamSynchronize(stream);
+    }
+    cudaFree(d_tiles);
+    if (e != cudaSuccess) return cuda_fail(e, "csg_tile_interval_sizes");
+    return rc;
 }
 
 int csg_set_variant(int variant) {
@@ -739,25 +936,45 @@ int csg_effective_variant(int64_t N) {
     return effective_variant(N);
 }
 
+int csg_set_throttle(int mode) {
+    std::lock_guard<std::mutex> lock(g.mu);
+    if (mode < CSG_THROTTLE_AUTO || mode > CSG_THROTTLE_OFF) return CSG_E_VARIANT;
+    g.throttle = mode;
+    return CSG_OK;
+}
+
+#ifdef CSG_ABLATE
+int csg_set_debug(int bits) {
+    std::lock_guard<std::mutex> lock(g.mu);
+    g.debug = bits;
+    return CSG_OK;
+}
+#endif
+
 int csg_set_kernel_timing(int enable) {
     std::lock_guard<std::mutex> lock(g.mu);
     g.timing = enable != 0;
-    if (!g.timing) g.timed_calls = 0;
+    if (!g.timing)
+        for (Device* D : g.dev)
+            if (D) D->timed_calls = 0;
     return CSG_OK;
 }
 
 static int kernel_ms_history(float* ms, int n) {
     if (!ms) return CSG_E_NULL;
     if (n < 1 || n > TIMING_RING) return CSG_E_SIZE;
-    if (g.timed_calls < n) {
+    Device* D = nullptr;
+    int rc = current_device(&D);
+    if (rc) return rc;
+    if (D->timed_calls < n) {
         snprintf(g.cuda_msg, sizeof(g.cuda_msg), "kernel timing: only %lld timed csg_action calls so far, %d asked",
-                 g.timed_calls, n);
+                 D->timed_calls, n);
         return CSG_E_CUDA;
     }
     for (int k = 0; k < n; ++k) {
-        const int slot = (int)((g.timed_calls - n + k) % TIMING_RING);
-        CSG_CUDA(cudaEventSynchronize(g.ev1[slot]));
-        CSG_CUDA(cudaEventElapsedTime(&ms[k], g.ev0[slot], g.ev1[slot]));
+        const int slot = (int)((D->timed_calls - n + k) % TIMING_RING);
+        CSG_CUDA(cudaEventSynchronize(D->ev1[slot]));
+        CSG_CUDA(cudaEventElapsedTime(&ms[k], D->ev0[slot], D->ev1[slot]));
     }
     return CSG_OK;
 }
@@ -777,18 +994,58 @@ int64_t csg_launch_count(void) {
     return g.launches;
 }
 
+int csg_measure_peak(int what, int iters, float* ms, double* units) {
+    std::lock_guard<std::mutex> lock(g.mu);
+    if (!ms || !units) return CSG_E_NULL;
+    if (iters < 1 || what < CSG_PEAK_MMA_MXF4 || what > CSG_PEAK_ALU_LOP3) return CSG_E_SIZE;
+    Device* D = nullptr;
+    int rc = current_device(&D);
+    if (rc) return rc;
+    if ((rc = ensure_tensor_ready(D))) return rc;
+    cudaEvent_t e0, e1;
+    CSG_CUDA(cudaEventCreate(&e0));
+    CSG_CUDA(cudaEventCreate(&e1));
+    unsigned int* sink = nullptr;
+    CSG_CUDA(cudaMalloc(&sink, sizeof(unsigned int)));
+    const int clusters = D->sm_count / 2;
+    cudaEventRecord(e0, 0);
+    if (what == CSG_PEAK_MMA_MXF4) {
+        tensor_peak_kernel<KIND_FP4><<<2 * clusters, TC_THREADS, TcTraits<KIND_FP4>::SMEM_BYTES>>>(iters, sink);
+        *units = (double)clusters * iters * 4.0 * 256.0 * 256.0 * 64.0;          // MACs
+    } else if (what == CSG_PEAK_MMA_I8) {
+        tensor_peak_kernel<KIND_I8><<<2 * clusters, TC_THREADS, TcTraits<KIND_I8>::SMEM_BYTES>>>(iters, sink);
+        *units = (double)clusters * iters * 4.0 * 256.0 * 256.0 * 32.0;
+    } else {
+        const int grid = D->sm_count * 8;
+        if (what == CSG_PEAK_ALU_MIX) alu_peak_kernel<0><<<grid, ALU_PEAK_THREADS>>>(iters, sink);
+        else if (what == CSG_PEAK_ALU_POPC) alu_peak_kernel<1><<<grid, ALU_PEAK_THREADS>>>(iters, sink);
+        else alu_peak_kernel<2><<<grid, ALU_PEAK_THREADS>>>(iters, sink);
+        *units = (double)grid * ALU_PEAK_THREADS * iters * 8.0;                   // lane-steps (MIX: 1 AND + 1 POPC + 1 ADD each)
+    }
+    cudaError_t e = cudaGetLastError();
+    cudaEventRecord(e1, 0);
+    if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(ms, e0, e1);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(sink);
+    ++g.launches;
+    if (e != cudaSuccess) return cuda_fail(e, "csg_measure_peak");
+    return CSG_OK;
+}
+
 const char* csg_strerror(int code) {
     switch (code) {
         case CSG_OK: return "success";
         case CSG_E_NULL: return "null pointer";
-        case CSG_E_SIZE: return "N or npairs out of range";
+        case CSG_E_SIZE: return "N, npairs, ntiles or a tile index out of range";
         case CSG_E_ALIGN: return "misaligned buffer (rel_bits needs 16 bytes, counts and S 8 bytes)";
         case CSG_E_DIM: return "dim must be 2 or 4";
         case CSG_E_EPS: return "eps must be in (0, 1]";
         case CSG_E_KMAX: return "kmax out of range (local action needs kmax >= 2 in 2D, >= 3 in 4D)";
         case CSG_E_UNSUPPORTED: return "unsupported combination of arguments";
         case CSG_E_CUDA: return g.cuda_msg;
-        case CSG_E_VARIANT: return "unknown variant";
+        case CSG_E_VARIANT: return "unknown variant or mode";
         case CSG_E_GEOMETRY: return "geometry must be CSG_GEOM_MINKOWSKI_2D, _MINKOWSKI_4D or _DESITTER_2D";
         case CSG_E_SHARD: return "shard must satisfy 0 <= shard < nshards";
         default: return "unknown error code";
@@ -797,42 +1054,11 @@ const char* csg_strerror(int code) {
 
 int csg_shutdown(void) {
     std::lock_guard<std::mutex> lock(g.mu);
-    if (g.d_tiles) cudaFree(g.d_tiles);
-    if (g.d_bits) cudaFree(g.d_bits);
-    if (g.d_counts) cudaFree(g.d_counts);
-    if (g.d_S) cudaFree(g.d_S);
-    if (g.d_coords) cudaFree(g.d_coords);
-    if (g.d_progress) cudaFree(g.d_progress);
-    g.d_progress = nullptr;
-    if (g.d_chunk_tiles) cudaFree(g.d_chunk_tiles);
-    g.d_chunk_tiles = nullptr;
-    g.chunk_N = -1;
-    for (cudaEvent_t e : g.chunk_ev) cudaEventDestroy(e);
-    g.chunk_ev.clear();
-    if (g.copy_stream) cudaStreamDestroy(g.copy_stream);
-    g.copy_stream = nullptr;
-    if (g.link_ev0) cudaEventDestroy(g.link_ev0);
-    if (g.link_ev1) cudaEventDestroy(g.link_ev1);
-    g.link_ev0 = g.link_ev1 = nullptr;
-    g.link_timed = false;
-    g.d_coords = nullptr;
-    g.d_coords_bytes = 0;
-    for (int k = 0; k < TIMING_RING; ++k) {
-        if (g.ev0[k]) cudaEventDestroy(g.ev0[k]);
-        if (g.ev1[k]) cudaEventDestroy(g.ev1[k]);
-        g.ev0[k] = g.ev1[k] = nullptr;
-    }
-    if (g.host_stream) cudaStreamDestroy(g.host_stream);
-    g.d_tiles = nullptr;
-    g.d_bits = nullptr;
-    g.d_counts = nullptr;
-    g.d_S = nullptr;
-    g.host_stream = nullptr;
-    g.tiles_N = -1;
-    g.map_ptr[0] = g.map_ptr[1] = nullptr;
-    g.map_N[0] = g.map_N[1] = -1;
-    g.d_bits_bytes = g.d_counts_bytes = 0;
-    g.timed_calls = 0;
+    for (int d = 0; d < MAX_DEVICES; ++d)
+        if (g.dev[d]) {
+            release_device(g.dev[d]);
+            g.dev[d] = nullptr;
+        }
     cudaGetLastError();
     return CSG_OK;
 }

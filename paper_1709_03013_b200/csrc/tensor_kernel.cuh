@@ -32,8 +32,12 @@
 //     smeared action only).  The first two groups of the NEXT tile are expanded before the epilogue of a tile, so
 //     the tensor cores restart as soon as the accumulators are drained.  No N x N count matrix ever reaches HBM.
 //
-// `dbg` (env CSG_DEBUG, default 0; a separate ABLATE instantiation of the fp4 kernel, see
-// paper_1709_03013_b200/ablate.py) switches parts of the kernel off for timing ablations (1: no MMA issue, 2: no
+// Template FLAGS select what else is compiled in: TCF_WAIT (the TMA thread may wait on two global words before it
+// starts a tile: the drift throttle and the host-copy gate, see below), TCF_DUMP (test hook csg_tile_interval_sizes:
+// the epilogue writes every n_ij of the listed tiles instead of bucketing it), TCF_ABLATE (only in the separate
+// -DCSG_ABLATE build of paper_1709_03013_b200/ablate.py, never in libcsg.so).
+// `dbg` (csg_set_debug of the ABLATE build; 0 and compiled out everywhere else) switches parts of the kernel off
+// for timing ablations (1: no MMA issue, 2: no
 // expansion arithmetic, 4: no operand stores, 8: no epilogue work, 16: no fence before publishing a stage, 32: no
 // packed-bit ring, 64: producers free-running with no MMA thread and no epilogue, 128: no prefill of the next tile
 // before an epilogue, 256: no open-range masks); any non-zero value gives wrong counts.
@@ -65,17 +69,24 @@ constexpr int TC_THREADS = TC_PRODUCERS + 64;  // + the MMA warp + the TMA warp
 #ifndef CSG_WHOLE_GROUP
 #define CSG_WHOLE_GROUP 1
 #endif
+#ifndef CSG_SCALE_CLASSES
+#define CSG_SCALE_CLASSES 1                // fp4 operands: position classes keep their nibble bit, block scales undo it (unpack_group_fp4)
+#endif
 constexpr bool TC_WHOLE_GROUP = CSG_WHOLE_GROUP != 0;   // a producer set expands both stages of every second group
 constexpr int TC_MAX_LEAD = 1;                 // rounds a cluster may run ahead of the average (L2 sharing inside a patch)
+constexpr int TC_THROTTLE_MAX_POLLS = 1 << 15; // polls of >= 200 ns in ONE wait before a cluster stops throttling for good (see the TMA warp)
+constexpr int TCF_ABLATE = 1, TCF_WAIT = 2, TCF_DUMP = 4;   // template FLAGS of tensor_action_kernel
 constexpr int TC_PREFILL_GROUPS = 2;           // groups (2 stages each) of the next tile expanded before a tile's epilogue
 constexpr int TC_HIST = 2048;              // privatised low bins per CTA
 
 // The two operand encodings of the kernel.
 //   KIND_I8 : one relation bit -> one u8 (0 or 1 << TB); tcgen05.mma kind::i8, K = 32 per instruction, s32
 //             accumulators; a stage row of 128 bytes covers 128 columns.
-//   KIND_FP4: one relation bit -> one e2m1 nibble (0 or 2.0 = 0b0100), two per byte; tcgen05.mma kind::mxf4 with
-//             all block scales 1.0 (UE8M0 0x7F), K = 64 per instruction, f32 accumulators holding 4 n_ij (exact
-//             below 2^24); a stage row of 128 bytes covers 256 columns, at twice the int8 MAC rate.
+//   KIND_FP4: one relation bit -> one e2m1 nibble, two per byte; tcgen05.mma kind::mxf4 (block32 UE8M0 scales),
+//             K = 64 per instruction, f32 accumulators holding 4 n_ij (exact below 2^24); a stage row of 128 bytes
+//             covers 256 columns, at twice the int8 MAC rate.  The nibble of a set bit is 0.5, 1.0, 2.0 or 2.0
+//             depending on the bit's position class inside its 32-bit word, and the block scales (4, 2, 1, 1) undo
+//             that, so every product of two set bits is 4 (see unpack_group_fp4).
 constexpr int KIND_I8 = 0, KIND_FP4 = 1;
 template <int KIND>
 struct TcTraits {
@@ -121,6 +132,17 @@ __device__ __forceinline__ uint32_t cluster_ctarank() {
     uint32_t r;
     asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
     return r;
+}
+// True in exactly one lane of a converged warp.  ptxas knows that a branch on this predicate has a single active
+// thread, so the tcgen05 / TMA instructions inside it are issued directly; inside `if (lane == 0)` it wraps every
+// one of them in an ELECT / BRA.U.ANY loop over the "possibly several" active lanes (5 extra instructions each).
+__device__ __forceinline__ bool elect_one() {
+    uint32_t is_elected;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "elect.sync _|p, 0xffffffff;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}" : "=r"(is_elected));
+    return is_elected != 0;
 }
 __device__ __forceinline__ void cluster_sync_all() {
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
@@ -251,6 +273,9 @@ __device__ __forceinline__ void umma_mxf4_2cta(uint32_t tmem_d, uint64_t adesc, 
 // Instruction descriptor, kind::mxf4 block scaled: A = B = e2m1 (1), scales UE8M0 (1), K-major, N = 256, M = 256,
 // scale-factor ids 0, K = 64.
 constexpr uint32_t TC_IDESC_FP4 = (1u << 7) | (1u << 10) | ((256u >> 3) << 17) | (1u << 23) | ((256u >> 4) << 24);
+// the same with scale-factor ids 2 for both operands (bits 4-5: B, bits 29-30: A): the two scales of the
+// instruction's two 32-k blocks are bytes 2, 3 of the 32-bit scale cell instead of bytes 0, 1
+constexpr uint32_t TC_IDESC_FP4_ODD = TC_IDESC_FP4 | (CSG_SCALE_CLASSES ? ((2u << 4) | (2u << 29)) : 0u);
 // 32 lanes x 32 columns store of one value (fills the scale-factor region of TMEM).
 __device__ __forceinline__ void tmem_fill_32x32(uint32_t taddr, uint32_t v) {
     asm volatile(
@@ -312,15 +337,30 @@ __device__ __forceinline__ void unpack_word(uint32_t x, uint4& lo, uint4& hi) {
     hi.x = unpack_class<TB>(x, 4); hi.y = unpack_class<TB>(x, 5);
     hi.z = unpack_class<TB>(x, 6); hi.w = unpack_class<TB>(x, 7);
 }
-// KIND_FP4.  One 32-bit word (32 k's) -> 32 e2m1 nibbles (one 16-byte chunk), each 0 or 0b0100 (= 2.0).
-// Class q = bits q, q+4, ..., q+28 goes to bit 2 of the eight nibbles of one 32-bit lane.
-__device__ __forceinline__ uint4 unpack_word_fp4(uint32_t x) {
-    uint4 o;
-    o.x = (x << 2) & 0x44444444u;
-    o.y = (x << 1) & 0x44444444u;
-    o.z = x & 0x44444444u;
-    o.w = (x >> 1) & 0x44444444u;
-    return o;
+// KIND_FP4.  Four 32-bit words (128 k's) -> four 16-byte chunks of 32 e2m1 nibbles each.  Class q of a word =
+// its bits q, q+4, ..., q+28 = bit q of its eight nibbles.  Chunk q of the group holds class q of all four words,
+// and a chunk is exactly one block of 32 k's with one UE8M0 scale, so a class may stay where it is:
+//     class 0: x & 0x11111111 -> nibbles 0b0001 = 0.5,  block scale 4      class 2: x & 0x44444444 -> 0b0100 = 2.0, scale 1
+//     class 1: x & 0x22222222 -> nibbles 0b0010 = 1.0,  block scale 2      class 3: (x >> 1) & 0x44444444 -> 2.0, scale 1
+// (bit 3 of a nibble is the sign, so class 3 alone is shifted).  Both operands use the same encoding and the same
+// scales, so every product of two set bits is (0.5*4)^2 = (1*2)^2 = (2*1)^2 = 4: the f32 accumulator holds 4 n_ij
+// exactly.  5 ALU operations per word instead of the 7 of "every class shifted to bit 2, all scales 1".
+// The MMA with even kk reads chunks 0, 1 (scale bytes 0, 1 of the TMEM cell), the one with odd kk chunks 2, 3
+// (scale bytes 2, 3): TC_SF_CELL and the scale-factor ids of TC_IDESC_FP4_ODD.
+constexpr uint32_t TC_SF_CELL = CSG_SCALE_CLASSES ? 0x7F7F8081u : 0x7F7F7F7Fu;   // UE8M0 bytes: 4, 2, 1, 1 (or all 1)
+__device__ __forceinline__ void unpack_group_fp4(const uint32_t* w, uint4* o) {
+#if CSG_SCALE_CLASSES
+    o[0] = make_uint4(w[0] & 0x11111111u, w[1] & 0x11111111u, w[2] & 0x11111111u, w[3] & 0x11111111u);
+    o[1] = make_uint4(w[0] & 0x22222222u, w[1] & 0x22222222u, w[2] & 0x22222222u, w[3] & 0x22222222u);
+    o[2] = make_uint4(w[0] & 0x44444444u, w[1] & 0x44444444u, w[2] & 0x44444444u, w[3] & 0x44444444u);
+    o[3] = make_uint4((w[0] >> 1) & 0x44444444u, (w[1] >> 1) & 0x44444444u, (w[2] >> 1) & 0x44444444u,
+                      (w[3] >> 1) & 0x44444444u);
+#else
+#pragma unroll
+    for (int m = 0; m < 4; ++m)
+        o[m] = make_uint4((w[m] << 2) & 0x44444444u, (w[m] << 1) & 0x44444444u, w[m] & 0x44444444u,
+                          (w[m] >> 1) & 0x44444444u);
+#endif
 }
 
 // Word m (bits 32m..32m+31) of a stage: keep local bit positions p with p > r (operand U in the stages that
@@ -351,14 +391,20 @@ __device__ __forceinline__ void tile_k_range(int I, int J, int& kb_begin, int& k
 // 4^TB, the accumulator holds n_ij << 2TB; the host picks the largest TB with (N-2) << 2TB < 2^31 (exact in s32).
 // KIND_FP4: TB unused (pass 0); the f32 accumulator holds 4 n_ij, exact for n_ij < 2^22.
 // tiles[t] = {I, J}: 256-row blocks, I <= J.  Grid = 2 x (number of SM pairs), cluster (2,1,1).
-template <int KIND, int TB, bool ABLATE = false, bool THROTTLE = false>
+// progress (TCF_WAIT, may be NULL): zeroed counter of finished tiles, the drift throttle.  rows_ready (TCF_WAIT, may
+// be NULL): number of matrix rows that have landed in `rel` so far, written by the host-copy stream; a tile (I, J)
+// starts once rows < 256 (J+1) are there.  dump (TCF_DUMP): ntiles x 256 x 256 int32, n_ij or -1.
+template <int KIND, int TB, int FLAGS = 0>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(TC_THREADS, 1)
 tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_t* __restrict__ rel, long long N,
                      long long stride_words, int kmax, unsigned long long* __restrict__ counts,
-                     const int2* __restrict__ tiles, int ntiles, int dbg_arg, unsigned int* __restrict__ progress_arg) {
-    unsigned int* const progress = THROTTLE ? progress_arg : nullptr;   // compiled out of the instantiations that do not throttle
+                     const int2* __restrict__ tiles, int ntiles, int dbg_arg, unsigned int* __restrict__ progress_arg,
+                     const unsigned int* __restrict__ rows_ready_arg, int* __restrict__ dump) {
+    constexpr bool ABLATE = (FLAGS & TCF_ABLATE) != 0, WAITS = (FLAGS & TCF_WAIT) != 0, DUMP = (FLAGS & TCF_DUMP) != 0;
+    unsigned int* const progress = WAITS ? progress_arg : nullptr;      // compiled out of the instantiations that never wait
+    const unsigned int* const rows_ready = WAITS ? rows_ready_arg : nullptr;
     using T = TcTraits<KIND>;
-    const int dbg = ABLATE ? dbg_arg : 0;             // compiled out of the production instantiation
+    const int dbg = ABLATE ? dbg_arg : 0;             // compiled out of every instantiation of libcsg.so
     constexpr int COLS = T::STAGE_COLS, WORDS = T::WORDS;
     extern __shared__ uint8_t smem_raw[];
     // the dynamic shared window starts at the same offset in both CTAs, so this rounding is identical in both
@@ -398,8 +444,9 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
     if (KIND == KIND_FP4 && warp < 4) {
-        // every block scale = 1.0: fill TMEM columns 256..287 of all 128 lanes with UE8M0 0x7F bytes
-        tmem_fill_32x32(tmem_base + ((uint32_t)(32 * warp) << 16) + T::TMEM_SF, 0x7F7F7F7Fu);
+        // block scales: every 32-bit cell of TMEM columns 256..287 (all 128 lanes) holds the same four UE8M0 bytes,
+        // so the row a cell belongs to does not matter: byte b scales the b-th chunk of a 64-byte operand group
+        tmem_fill_32x32(tmem_base + ((uint32_t)(32 * warp) << 16) + T::TMEM_SF, TC_SF_CELL);
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
         tc_fence_before();
     }
@@ -441,7 +488,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
         const int q4 = warp & 3;                      // TMEM lane quarter this warp may read
         const int cq = warp >> 2;                     // which 64 accumulator columns it drains
         uint32_t tphase = 0;                          // parity of tmem_full
-        int epi_I = -1, epi_J = -1;                   // tile whose accumulators still wait for their epilogue
+        int epi_I = -1, epi_J = -1, epi_t = -1;       // tile whose accumulators still wait for their epilogue
 
         // Publish this set's stage that is written but not yet visible to the MMA thread.
         auto publish_pending = [&]() {
@@ -457,7 +504,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
             pending = -1;
         };
         // Fused epilogue of tile (eI, eJ): TMEM -> registers -> mask by R[i][j], i<j -> histogram.
-        auto epilogue = [&](int eI, int eJ) {
+        auto epilogue = [&](int eI, int eJ, int et) {
             if (dbg & 64) return;
             const long long i0 = (long long)eI * TC_T, j0 = (long long)eJ * TC_T;
             const long long i = i0 + 128 * (int)rank + 32 * q4 + lane;
@@ -483,7 +530,10 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
 #pragma unroll
                 for (int x = 0; x < 32; ++x) {
                     const int n = KIND == KIND_FP4 ? (int)(__uint_as_float(v[x]) * 0.25f) : (int)(v[x] >> (2 * TB));
-                    if (((rw >> x) & 1u) && n <= kmax) {
+                    if (DUMP) {                       // test hook: every n_ij of the tile, -1 where i, j are not a related pair
+                        dump[((size_t)et * TC_T + (size_t)(128 * (int)rank + 32 * q4 + lane)) * TC_T + 32 * (2 * cq + e) + x] =
+                            ((rw >> x) & 1u) ? n : -1;
+                    } else if (((rw >> x) & 1u) && n <= kmax) {
                         if (n < TC_HIST) atomicAdd(&hist[n], 1u);
                         else atomicAdd(&counts[n], 1ULL);
                     }
@@ -515,7 +565,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
             const int prefill = (ABLATE && (dbg & 128)) ? 0 : TC_PREFILL_GROUPS;    // dbg 128: epilogue before any next stage
             if (prefill == 0 && epi_I >= 0) {
                 publish_pending();
-                epilogue(epi_I, epi_J);
+                epilogue(epi_I, epi_J, epi_t);
                 epi_I = -1;
             }
             const int epi_at = kb_begin + TC_GROUP * (min(prefill, (kb_end - kb_begin) / TC_GROUP) - 1);
@@ -539,8 +589,8 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
 #pragma unroll
                     for (int m = 0; m < 8; ++m) o[m] = make_uint4(w[m % WORDS], w[(m + 1) % WORDS], w[(m + 2) % WORDS], w[(m + 3) % WORDS]);
                 } else if (KIND == KIND_FP4) {
-#pragma unroll
-                    for (int m = 0; m < 8; ++m) o[m] = unpack_word_fp4(w[m % WORDS]);
+                    unpack_group_fp4(&w[0], &o[0]);
+                    unpack_group_fp4(&w[WORDS - 4], &o[4]);
                 } else {
 #pragma unroll
                     for (int m = 0; m < 4; ++m) unpack_word<TB>(w[m], o[2 * m], o[2 * m + 1]);
@@ -636,20 +686,29 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 }
                 if (epi_I >= 0 && kb0 == epi_at) {             // the previous tile's epilogue, after the prefill
                     publish_pending();
-                    epilogue(epi_I, epi_J);
+                    epilogue(epi_I, epi_J, epi_t);
                     epi_I = -1;
                 }
             }
             epi_I = I;
             epi_J = J;
+            epi_t = t;
         }
         publish_pending();                                     // last stage of the last tile
-        if (epi_I >= 0) epilogue(epi_I, epi_J);
+        if (epi_I >= 0) epilogue(epi_I, epi_J, epi_t);
     } else if (warp == TC_MMA_WARP) {
-        // ================================================================== MMA issuer (leader CTA, lane 0 issues)
+        // ================================================================== MMA issuer (leader CTA, one elected lane issues)
+        // The whole warp walks the loop converged (the barrier waits and the ring bookkeeping are warp-uniform, so they
+        // stay on the uniform datapath); only the tcgen05 instructions sit under the elected lane's predicate.  This
+        // one warp paces the tensor cores of two SMs: at ~88 instructions per stage (lane-0 branch, per-instruction
+        // ELECT loops, descriptors rebuilt and moved to uniform registers every stage) it needed ~700 clk per stage
+        // and was the bottleneck of the kernel (ncu source view: the warp never waited on `full`, it was busy issuing).
         if (rank == 0 && !(dbg & 64)) {
+            const bool issuer = elect_one();
             uint32_t stage = 0, sphase = 0, ephase = 0;
             int done_tiles = 0;
+            const uint32_t tmem_sfa = tmem_base + T::TMEM_SF, tmem_sfb = tmem_base + T::TMEM_SFB;
+            const uint64_t adesc0 = make_kmajor_sw128_desc(smem0), bdesc0 = make_kmajor_sw128_desc(smem0 + T::OFF_B);
             for (int rd = 0; rd < rounds; ++rd) {
                 const int t = rd * G + ((rd & 1) ? (G - 1 - cl) : cl);
                 if (t >= ntiles) continue;
@@ -661,30 +720,30 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                     ephase ^= 1;
                 }
                 tc_fence_after();
+                uint32_t fresh = 1;                         // the tile's first MMA overwrites the accumulators
                 for (int kb = kb_begin; kb < kb_end; ++kb) {
                     mbar_wait(full0 + 8 * stage, sphase);
                     tc_fence_after();
-                    if (lane == 0) {
-                        const uint32_t a_addr = smem0 + stage * T::STAGE_BYTES;
-                        const uint64_t adesc = make_kmajor_sw128_desc(a_addr);
-                        const uint64_t bdesc = make_kmajor_sw128_desc(a_addr + T::OFF_B);
+                    if (issuer) {
+                        const uint64_t soff = (uint64_t)(stage * (T::STAGE_BYTES >> 4));   // descriptor address unit: 16 bytes
+                        const uint64_t adesc = adesc0 + soff, bdesc = bdesc0 + soff;
+                        const uint32_t a_tmem = tmem_base + T::TMEM_A + 32u * stage;
 #pragma unroll
                         for (int kk = 0; kk < TC_ROW_BYTES / 32; ++kk) {   // 32 bytes of K per instruction: +2 in 16-byte units
-                            const uint32_t acc = (kb > kb_begin || kk > 0) ? 1u : 0u;
+                            const uint32_t acc = kk > 0 ? 1u : (fresh ^ 1u);
                             if (dbg & 1) continue;                          // ablation: no MMA issue
+                            const uint32_t idesc4 = (kk & 1) ? TC_IDESC_FP4_ODD : TC_IDESC_FP4;   // which two scale bytes
                             if (KIND == KIND_FP4 && T::A_TMEM)
-                                umma_mxf4_2cta_ts(tmem_base, tmem_base + T::TMEM_A + 32u * stage + 8u * kk, bdesc + 2 * kk,
-                                                  TC_IDESC_FP4, acc, tmem_base + T::TMEM_SF, tmem_base + T::TMEM_SFB);
+                                umma_mxf4_2cta_ts(tmem_base, a_tmem + 8u * kk, bdesc + 2 * kk, idesc4, acc, tmem_sfa, tmem_sfb);
                             else if (KIND == KIND_FP4)
-                                umma_mxf4_2cta(tmem_base, adesc + 2 * kk, bdesc + 2 * kk, TC_IDESC_FP4, acc,
-                                               tmem_base + T::TMEM_SF, tmem_base + T::TMEM_SFB);
+                                umma_mxf4_2cta(tmem_base, adesc + 2 * kk, bdesc + 2 * kk, idesc4, acc, tmem_sfa, tmem_sfb);
                             else
                                 umma_i8_2cta(tmem_base, adesc + 2 * kk, bdesc + 2 * kk, TC_IDESC, acc);
                         }
                         umma_commit_2cta(empty0 + 8 * stage);
                         if (kb == kb_end - 1) umma_commit_2cta(tmem_full);
                     }
-                    __syncwarp();
+                    fresh = 0;
                     if (++stage == T::STAGES) { stage = 0; sphase ^= 1; }
                 }
                 ++done_tiles;
@@ -694,6 +753,8 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
         // ================================================================== TMA warp: packed bits -> shared ring
         if (lane == 0) {
             uint32_t bb = 0, bphase = 0;
+            bool throttling = true;
+            unsigned int rows_seen = 0;
             for (int rd = 0; rd < rounds; ++rd) {
                 const int t = rd * G + ((rd & 1) ? (G - 1 - cl) : cl);
                 if (t >= ntiles) continue;
@@ -707,9 +768,33 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 // 38 %).  A cluster starts round rd only when (rd - TC_MAX_LEAD) * G tiles are finished in total; the
                 // slowest cluster never waits (everybody else has finished at least as many), so no deadlock, and the
                 // makespan of the static deal is unchanged.  Only the TMA thread polls; everything downstream starves.
-                if (progress != nullptr && rd > TC_MAX_LEAD) {
+                // The wait is bounded: it relies on all clusters of the grid being resident together (the host clamps the
+                // grid to cudaOccupancyMaxActiveClusters), and if that ever fails -- SMs held by another kernel or an MPS
+                // limit -- a cluster that has polled TC_THROTTLE_MAX_POLLS times in one wait (> 6.5 ms; a tile takes well
+                // under 1 ms) stops throttling for the rest of the launch: the failure costs L2 reuse, not a hang.
+                if (WAITS && progress != nullptr && rd > TC_MAX_LEAD && throttling) {
                     const unsigned int need = (unsigned int)(rd - TC_MAX_LEAD) * (unsigned int)G;
-                    while (*reinterpret_cast<volatile unsigned int*>(progress) < need) __nanosleep(200);
+                    int polls = 0;
+                    while (*reinterpret_cast<volatile unsigned int*>(progress) < need) {
+                        if (++polls >= TC_THROTTLE_MAX_POLLS) { throttling = false; break; }
+                        __nanosleep(200);
+                    }
+                }
+                // Host-copy gate (csg_action_host): the matrix arrives in row chunks on a copy stream, which publishes the
+                // number of rows landed after each chunk; tile (I, J) reads rows below 256 (J+1) only.  The wait depends
+                // on the copy engine alone, never on another CTA.
+                if (WAITS && rows_ready != nullptr) {
+                    const unsigned int need_rows = (unsigned int)min((long long)(tile.y + 1) * TC_T, N);
+                    if (rows_seen < need_rows) {
+                        unsigned int got;
+                        while (true) {
+                            asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(got) : "l"(rows_ready) : "memory");
+                            if (got >= need_rows) break;
+                            __nanosleep(500);
+                        }
+                        rows_seen = got;
+                        asm volatile("fence.proxy.async.global;" ::: "memory");   // the bytes are read by the async proxy (TMA)
+                    }
                 }
                 for (int kb0 = kb_begin; kb0 < ((dbg & 32) ? kb_begin : kb_end); kb0 += TC_GROUP) {
                     mbar_wait(bits_empty0 + 8 * bb, bphase ^ 1);

@@ -31,6 +31,26 @@ def test_exports_match_header(lib):
         assert getattr(lib, n) is not None
 
 
+def test_no_environment_switches_in_the_product_library(lib):
+    """The timing-ablation switches (wrong counts when set) live only in the -DCSG_ABLATE build: libcsg.so reads no
+    environment variable and exports no csg_set_debug."""
+    import subprocess
+    syms = subprocess.run(["nm", "-D", csg.LIB_PATH], capture_output=True, text=True, check=True).stdout
+    assert "csg_set_debug" not in syms               # (getenv itself is imported by the static CUDA runtime)
+    blob = open(csg.LIB_PATH, "rb").read()
+    assert b"CSG_DEBUG" not in blob and b"CSG_NO_THROTTLE" not in blob and b"CSG_" + b"ABLATE" not in blob
+    for src in ("csg.cu", "tensor_kernel.cuh", "bitset_kernel.cuh", "link_kernel.cuh", "peak_kernels.cuh"):
+        assert "getenv" not in open(os.path.join(ROOT, "paper_1709_03013_b200", "csrc", src)).read(), src
+
+
+def test_throttle_setter(lib):
+    for mode in (csg.THROTTLE_ON, csg.THROTTLE_OFF, csg.THROTTLE_AUTO):
+        csg.csg_set_throttle(mode)
+    with pytest.raises(csg.CsgError) as e:
+        csg.csg_set_throttle(3)
+    assert e.value.code == -9
+
+
 def test_row_stride(lib):
     assert [csg.csg_row_stride_words(n) for n in (1, 255, 256, 257, 1024, 131072)] == [4, 4, 4, 8, 16, 2048]
     assert csg.csg_row_stride_words(0) == 0

@@ -283,7 +283,7 @@ def golden_histogram(name):
 
 def check_config(csg, cfg, full_reference):
     N, dim = cfg["N"], cfg["dim"]
-    _, bits = csg_inputs.make_causet(dim, N, cfg["seed"])
+    coords, bits = csg_inputs.make_causet(dim, N, cfg["seed"])
     d = csg.to_device(bits)
     csg.csg_set_variant(csg.VARIANT_AUTO)
     # (1) the configuration as benchmarked
@@ -297,16 +297,46 @@ def check_config(csg, cfg, full_reference):
     assert (full[:cfg["kmax"] + 1] == counts).all()
     nrel, chains = degree_invariants(bits, N)
     assert full.sum() == nrel                                         # I1
+    if dim == 2:
+        assert full.sum() == oracle.dominance2d_relations(coords)     # P5: C(N,2) - inversions, from the coordinates
     assert int((np.arange(N - 1, dtype=object) * full.astype(object)).sum()) == chains   # I2 = I3
     # (2b) the tile shards of the multi-GPU path (patch schedule at these sizes) add up to the same histogram
     parts = sum(csg.csg_action_partial(d, N, cfg["kmax"], s, 3) for s in range(3))
     torch.cuda.synchronize()
     assert (parts.cpu().numpy() == counts).all()
-    # (3) sampled outputs the oracle computes one by one
+    # (3) sampled outputs the oracle computes one by one, taken from the tensor kernel ITSELF: whole
+    #     256 x 256 tiles dumped by csg_tile_interval_sizes (same sweep, masks and accumulators as csg_action), at the
+    #     places where the open-range masks and the ragged edges live: on the diagonal, next to it, the far corner, the
+    #     last row/column block, and a few in between.  From them >= 10^4 RELATED pairs, half of them on rows/columns
+    #     0, 1, 127, 128, 254, 255 of their tile, compared with the bit-by-bit oracle; all unrelated entries must be -1.
     rng = np.random.default_rng(cfg["seed"])
-    pairs = np.sort(rng.integers(0, N, size=(300, 2)), axis=1).astype(np.int64)
+    nB = (N + 255) // 256
+    tiles = [(0, 0), (0, 1), (0, nB - 1), (nB - 1, nB - 1), (nB - 2, nB - 1), (nB // 2, nB // 2), (nB // 2, nB // 2 + 1),
+             (nB // 3, 2 * nB // 3), (1, nB - 2), (nB // 5, nB // 5 + 7)]
+    tiles = [(min(a, nB - 1), min(max(a, b), nB - 1)) for a, b in tiles]
+    for variant in ((csg.VARIANT_TENSOR_FP4, csg.VARIANT_TENSOR) if N <= 131072 else (csg.VARIANT_TENSOR_FP4,)):
+        csg.csg_set_variant(variant)
+        dump = csg.csg_tile_interval_sizes(d, N, tiles).cpu().numpy()
+        checked = 0
+        for t, (I, J) in enumerate(tiles):
+            tile = dump[t]
+            rr, cc = np.nonzero(tile >= 0)
+            edge = np.isin(rr, (0, 1, 127, 128, 254, 255)) | np.isin(cc, (0, 1, 127, 128, 254, 255))
+            pick = np.concatenate([rng.permutation(np.nonzero(edge)[0])[:600], rng.permutation(np.nonzero(~edge)[0])[:600]])
+            for k in pick:
+                i, j = 256 * I + int(rr[k]), 256 * J + int(cc[k])
+                assert tile[rr[k], cc[k]] == oracle.pair_interval(bits, N, i, j), (variant, I, J, i, j)
+            checked += len(pick)
+            ur, uc = np.nonzero(tile < 0)
+            for k in rng.permutation(len(ur))[:200]:
+                i, j = 256 * I + int(ur[k]), 256 * J + int(uc[k])
+                assert i >= j or j >= N or oracle.pair_interval(bits, N, i, j) == -1, (variant, I, J, i, j)
+        assert checked >= (10000 if dim == 2 else 3000), checked      # 4D: near-diagonal tiles hold few related pairs
+    csg.csg_set_variant(csg.VARIANT_AUTO)
+    # ... and the one-warp-per-pair hook on uniformly drawn pairs (mostly unrelated in 4D)
+    pairs = np.sort(rng.integers(0, N, size=(2000, 2)), axis=1).astype(np.int64)
     got = csg.csg_interval_sizes(d, N, torch.from_numpy(pairs).cuda()).cpu().numpy()
-    for (i, j), n in zip(pairs[:60], got[:60]):
+    for (i, j), n in zip(pairs, got):
         assert n == oracle.pair_interval(bits, N, i, j)
     # (4) the WHOLE histogram against the oracle's stored one (Algorithm 5 over the full config, minutes of CPU, run
     #     once by tests/golden/make_config_goldens.py); the bitset hash ties the stored line to this very input
@@ -315,7 +345,12 @@ def check_config(csg, cfg, full_reference):
         import hashlib
         assert gold["N"] == N and csg_inputs.bits_hash(bits) == gold["bits_hash"]
         assert int(full.sum()) == gold["total"] and [int(x) for x in full[:8]] == gold["head"]
-        assert hashlib.sha256(np.ascontiguousarray(full, dtype="<i8").tobytes()).hexdigest() == gold["sha256"]
+        if hashlib.sha256(np.ascontiguousarray(full, dtype="<i8").tobytes()).hexdigest() != gold["sha256"]:
+            # say WHICH bins differ: recompute the oracle histogram (2D: minutes, from the coordinates)
+            want = oracle.dominance2d_counts(coords, N - 2) if dim == 2 else oracle.alg5_counts(bits, N, N - 2)
+            bad = np.nonzero(want != full)[0]
+            raise AssertionError("histogram differs from the oracle in %d bins, first %s: got %s want %s"
+                                 % (len(bad), bad[:8], full[bad[:8]], want[bad[:8]]))
         if cfg["eps"] == 1.0:
             assert float(S.item()) == oracle.action_local(dim, N, full[:4])
     # (5) else the reference histogram computed now, where Algorithm 5 finishes in reasonable time
@@ -360,7 +395,123 @@ def test_config3_headline(csg):
 
 @pytest.mark.slow
 def test_config4_smeared(csg):
+    """All 262143 bins and S against the oracle's stored histogram (tests/golden/config_histograms.txt, written from
+    oracle/dominance2d.c); this is the configuration that runs the throttled instantiation of the fp4 kernel."""
+    assert golden_histogram(csg_inputs.CONFIGS[4]["name"]) is not None
     check_config(csg, csg_inputs.CONFIGS[4], full_reference=False)
+
+
+# --------------------------------------------------------------------------- the tensor kernel's own n_ij, pair by pair
+@pytest.mark.parametrize("variant", [2, 3])
+@pytest.mark.parametrize("dim,N,seed", [(2, 700, 1), (4, 1300, 2), (2, 2049, 3)])
+def test_tile_dump_equals_oracle_pair_by_pair(csg, variant, dim, N, seed):
+    """csg_tile_interval_sizes: every entry of every tile against the definition (U @ U on the expanded matrix)."""
+    _, bits = csg_inputs.make_causet(dim, N, seed)
+    U = np.triu(oracle.expand(bits, N), 1).astype(np.int64)
+    want = np.where(U == 1, U @ U, -1)
+    nB = (N + 255) // 256
+    tiles = [(I, J) for I in range(nB) for J in range(I, nB)]
+    csg.csg_set_variant(variant)
+    dump = csg.csg_tile_interval_sizes(csg.to_device(bits), N, tiles).cpu().numpy()
+    csg.csg_set_variant(csg.VARIANT_AUTO)
+    padded = np.full((256 * nB, 256 * nB), -1, dtype=np.int64)
+    padded[:N, :N] = want
+    for t, (I, J) in enumerate(tiles):
+        assert (dump[t] == padded[256 * I:256 * I + 256, 256 * J:256 * J + 256]).all(), (I, J)
+
+
+# --------------------------------------------------------------------------- the throttled instantiation under a live oracle
+@pytest.mark.parametrize("dim,N,kmax", [(2, 16384, 16382), (4, 9001, 3), (2, 5000, 4998)])
+def test_throttled_instantiation_equals_oracle(csg, dim, N, kmax):
+    """CSG_THROTTLE_ON selects the instantiation of the fp4 kernel that BASELINE.json configs[4] runs (TMA threads wait
+    on the finished-tile counter) at sizes where Algorithm 5 finishes in seconds; results must not depend on it."""
+    _, bits = csg_inputs.make_causet(dim, N, 31 + N)
+    want = oracle.alg5_counts(bits, N, kmax)
+    d = csg.to_device(bits)
+    csg.csg_set_variant(csg.VARIANT_TENSOR_FP4)
+    try:
+        for mode in (csg.THROTTLE_ON, csg.THROTTLE_OFF, csg.THROTTLE_ON):
+            csg.csg_set_throttle(mode)
+            for _ in range(3):
+                c, S = csg.csg_action(d, N, dim, 1.0, kmax)
+                torch.cuda.synchronize()
+                assert (c.cpu().numpy() == want).all(), mode
+                assert float(S.item()) == oracle.action_local(dim, N, want)
+    finally:
+        csg.csg_set_throttle(csg.THROTTLE_AUTO)
+        csg.csg_set_variant(csg.VARIANT_AUTO)
+
+
+# --------------------------------------------------------------------------- cached state: sizes, shards, streams, graphs
+def test_alternating_sizes_shards_and_streams_without_sync(csg):
+    """After one warm-up call per (N, shard) csg_action / csg_action_partial only enqueue: alternating two sizes and
+    three shards on two streams never synchronises (the call returns while its stream is still busy) and every
+    result is bit-exact."""
+    csg.csg_set_variant(csg.VARIANT_AUTO)
+    sizes = [(4, 2600), (2, 1900)]
+    sets = {N: csg_inputs.make_causet(dim, N, 50 + N)[1] for dim, N in sizes}
+    want = {N: oracle.alg5_counts(sets[N], N, 3) for _, N in sizes}
+    dev = {N: csg.to_device(sets[N]) for _, N in sizes}
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    for dim, N in sizes:                                              # warm-up: builds the cached tile schedules
+        csg.csg_action(dev[N], N, dim, 1.0, 3)
+        for s in range(3):
+            csg.csg_action_partial(dev[N], N, 3, s, 3)
+    torch.cuda.synchronize()
+    results = []
+    busy_seen = 0
+    for it in range(12):
+        dim, N = sizes[it % 2]
+        st = streams[(it // 2) % 2]
+        with torch.cuda.stream(st):
+            torch.cuda._sleep(40_000_000)                             # ~20 ms of busy stream ahead of the call
+            c, S = csg.csg_action(dev[N], N, dim, 1.0, 3, stream=st)
+            parts = [csg.csg_action_partial(dev[N], N, 3, s, 3, stream=st) for s in range(3)]
+            busy_seen += not st.query()                               # had the call synchronised, the stream would be idle
+        results.append((N, dim, c, S, parts))
+    torch.cuda.synchronize()
+    assert busy_seen >= 10, busy_seen
+    for N, dim, c, S, parts in results:
+        assert (c.cpu().numpy() == want[N]).all()
+        assert (sum(parts).cpu().numpy() == want[N]).all()
+        assert float(S.item()) == oracle.action_local(dim, N, want[N])
+
+
+def test_graph_survives_other_sizes(csg):
+    """A captured csg_action keeps working after calls with other sizes (cached tile lists are never freed or
+    overwritten before csg_shutdown)."""
+    csg.csg_set_variant(csg.VARIANT_AUTO)
+    N1, N2, N3 = 3000, 1700, 5200
+    b1, b2, b3 = (csg_inputs.make_causet(4, N, 60 + N)[1] for N in (N1, N2, N3))
+    d1, d2, d3 = csg.to_device(b1), csg.to_device(b2), csg.to_device(b3)
+    c1 = torch.zeros(4, dtype=torch.int64, device="cuda")
+    S1 = torch.zeros(1, dtype=torch.float64, device="cuda")
+    csg.csg_action(d1, N1, 4, 1.0, 3, c1, S1)
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        csg.csg_action(d1, N1, 4, 1.0, 3, c1, S1)
+    want1 = oracle.alg5_counts(b1, N1, 3)
+    for other_d, other_N, other_b in ((d2, N2, b2), (d3, N3, b3), (d2, N2, b2)):
+        c, _ = csg.csg_action(other_d, other_N, 4, 1.0, 3)
+        for s in range(2):
+            csg.csg_action_partial(other_d, other_N, 3, s, 2)
+        torch.cuda.synchronize()
+        assert (c.cpu().numpy() == oracle.alg5_counts(other_b, other_N, 3)).all()
+        c1.fill_(-1)
+        graph.replay()
+        torch.cuda.synchronize()
+        assert (c1.cpu().numpy() == want1).all()
+        assert float(S1.item()) == oracle.action_local(4, N1, want1)
+
+
+def test_measure_peak_runs(csg):
+    for what in (csg.PEAK_MMA_MXF4, csg.PEAK_MMA_I8, csg.PEAK_ALU_MIX, csg.PEAK_ALU_POPC, csg.PEAK_ALU_LOP3):
+        ms, units = csg.csg_measure_peak(what, 2000)
+        assert ms > 0 and units > 0
+    ms, units = csg.csg_measure_peak(csg.PEAK_MMA_MXF4, 20000)
+    rate = units / (ms * 1e-3)                                        # MAC/s over the device
+    assert 1.5e15 < rate < 6e15, rate                                 # nominal dense fp4: 4.5e15 MAC/s
 
 
 @pytest.mark.parametrize("N,dim", [(1000, 2), (3000, 4)])

@@ -23,18 +23,26 @@ def csg():
     return m
 
 
+@pytest.mark.parametrize("throttle", [0, 1])
 @pytest.mark.parametrize("dim,N,reps", [(2, 16384, 12), (4, 16384, 8), (2, 9000, 12)])
-def test_repeated_full_histograms(csg, dim, N, reps):
+def test_repeated_full_histograms(csg, dim, N, reps, throttle):
+    """throttle = 1 (CSG_THROTTLE_ON): the instantiation of the fp4 kernel whose TMA threads wait on the finished-tile
+    counter -- the one BASELINE.json configs[4] runs -- on the device-resident call, and together with the copy gate
+    on the host call."""
     _, bits = csg_inputs.make_causet(dim, N, 777 + N)
     want = oracle.alg5_counts(bits, N, N - 2)
     d = csg.to_device(bits)
     pinned = torch.from_numpy(bits.view(np.int64)).pin_memory()
-    for r in range(reps):
-        c, _ = csg.csg_action(d, N, dim, 1.0, N - 2)
-        torch.cuda.synchronize()
-        assert (c.cpu().numpy() == want).all(), ("device", r)
-        ch, _ = csg.csg_action_host(pinned, N, dim, 1.0, N - 2)
-        assert (ch == want).all(), ("host", r)
+    csg.csg_set_throttle(throttle)
+    try:
+        for r in range(reps):
+            c, _ = csg.csg_action(d, N, dim, 1.0, N - 2)
+            torch.cuda.synchronize()
+            assert (c.cpu().numpy() == want).all(), ("device", r)
+            ch, _ = csg.csg_action_host(pinned, N, dim, 1.0, N - 2)
+            assert (ch == want).all(), ("host", r)
+    finally:
+        csg.csg_set_throttle(0)
 
 
 @pytest.mark.slow
