@@ -50,12 +50,66 @@ def read_peaks():
     return dict(bf16=1590.0, bf16_sustained=1400.0, hbm=6650.0, source="fallback (B200_PROFILING.md)")
 
 
-def read_traffic(kernel):
-    """dram bytes per launch of the dominant kernel from the committed ncu --set full summary, or None."""
+def kernel_source_hash():
+    """sha256 over the CUDA sources: profiles/dram_traffic.json records the hash its captures were taken at."""
+    import hashlib
+    h = hashlib.sha256()
+    csrc = os.path.join(ROOT, "paper_1709_03013_b200", "csrc")
+    for name in sorted(os.listdir(csrc)):
+        if name.endswith((".cu", ".cuh")):
+            h.update(open(os.path.join(csrc, name), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def read_traffic(kernel, workload_index):
+    """(dram bytes per launch, provenance) of a kernel from the committed ncu --set full summaries
+    (profiles/dram_traffic.json), or (None, why): the capture must be of THIS workload and of the present sources."""
     path = os.path.join(ROOT, "profiles", "dram_traffic.json")
     if not os.path.exists(path):
-        return None
-    return json.load(open(path)).get(kernel)
+        return None, "no capture committed"
+    entry = json.load(open(path)).get(kernel)
+    if not isinstance(entry, dict):
+        return None, "no capture committed for this kernel"
+    if entry.get("config") != workload_index:
+        return None, "the committed capture (%s) is of configs[%s], not of this workload" % (entry.get("capture"), entry.get("config"))
+    if entry.get("csrc_sha256_16") != kernel_source_hash():
+        return None, "stale: the kernel sources changed after the committed capture (%s)" % entry.get("capture")
+    return entry["dram_bytes_per_launch"], "ncu --set full, %s" % entry.get("capture")
+
+
+def config_dict(cfg, N, dim, eps, kmax):
+    """The `config` object of the JSON line: the same keys and values from both arms (ours / reference)."""
+    stride = 4 * ((N + 255) // 256)
+    nbytes = N * stride * 8
+    return {"workload": workload_name(cfg), "N": N, "dim": dim, "eps": eps, "kmax": kmax, "seed": cfg["seed"],
+            "bitset_bytes": nbytes,
+            "l2": "input (%.0f MiB) %s L2 (126 MB)" % (nbytes / 2**20, "larger than" if nbytes > 126e6 else "fits in")}
+
+
+def useful_work_ratio(bits, N):
+    """sum over related pairs i<j of (j-i-1), divided by C(N,3): the share of the ordered-triple tests that the paper's
+    own method executes (Algorithm 5 skips unrelated pairs, PAPER.md:407 l.4-5); the dense tile formulation does all
+    C(N,3).  Host side, O(N^2/64): sum_j j over the set bits of the upper triangle from word popcounts."""
+    import numpy as np
+    W = bits.shape[1]
+    masks = [np.uint64(sum(1 << p for p in range(64) if (p >> b) & 1)) for b in range(6)]
+    total = 0
+    cols = np.arange(W, dtype=np.int64)
+    for r0 in range(0, N, 2048):
+        blk = bits[r0:min(N, r0 + 2048)].copy()
+        rows = np.arange(r0, r0 + blk.shape[0], dtype=np.int64)
+        wi = rows // 64
+        blk[cols[None, :] < wi[:, None]] = 0                                   # words wholly left of the diagonal
+        own = np.arange(blk.shape[0])
+        keep = ~((np.uint64(2) << (rows % 64).astype(np.uint64)) - np.uint64(1)) if True else None
+        keep = np.where(rows % 64 == 63, np.uint64(0), keep)                    # bit 63: nothing right of it in the word
+        blk[own, wi] &= keep                                                    # keep columns j > i only
+        pc = np.bitwise_count(blk).astype(np.int64)
+        sum_j = (pc * (64 * cols)[None, :]).sum(1)
+        for b in range(6):
+            sum_j += (np.bitwise_count(blk & masks[b]).astype(np.int64).sum(1)) << b
+        total += int((sum_j - (rows + 1) * pc.sum(1)).sum())
+    return total / comb3(N) if N >= 3 else 0.0
 
 
 # ------------------------------------------------------------------------------------------- clocks sampler
@@ -180,9 +234,10 @@ def run_reference(args, cfg, rank, world):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * secs_total / max(args.steps, 1), "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "u64 bit ops (host)", "data": "synthetic",
-        "config": {"workload": workload_name(cfg), "N": N, "dim": dim, "eps": cfg["eps"], "kmax": kmax,
-                   "seed": cfg["seed"], "note": "each step is a bounded sample of the workload"},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "config": config_dict(cfg, N, dim, cfg["eps"], kmax),
+        "note": "each step is a bounded sample of the workload",
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample,
+                         "full_config_s_extrapolated": comb3(N) / value},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -265,12 +320,15 @@ def run_ours(args, cfg, rank, local_rank, world):
     result_S = float(S.item())
 
     # ---- end-to-end leg: HOST buffers through csg_action_host (H2D of the bitset + D2H of counts, S inside)
-    e2e_steps = max(1, min(args.steps, 3))
+    e2e_steps = max(1, min(args.steps, 5))
     csg.csg_action_host(host, N, dim, eps, kmax)   # warm-up (allocates the library's device buffers)
     barrier()
+    e2e_each = []
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
+        t1 = time.perf_counter()
         c_host, S_host = csg.csg_action_host(host, N, dim, eps, kmax)
+        e2e_each.append(1e3 * (time.perf_counter() - t1))
     e2e_s = time.perf_counter() - t0
     checks = {"e2e_equals_device": bool((c_host == result_counts).all() and S_host == result_S)}
 
@@ -297,6 +355,11 @@ def run_ours(args, cfg, rank, local_rank, world):
         c2_host, S2_host = csg.csg_causet_action_host(coords_pinned, N, geom, eps, kmax)
     e2e_coords_s = time.perf_counter() - t0
     checks["coords_in_equals_device"] = bool((c2_host == result_counts).all() and S2_host == result_S)
+    if tiles_mode:
+        # the all-reduced histogram of the sharded run must equal the one this GPU computes alone (same seed)
+        c_single, S_single = csg.csg_action(d_bits, N, dim, eps, kmax)
+        torch.cuda.synchronize()
+        checks["sharded_equals_single"] = bool((c_single.cpu().numpy() == result_counts).all() and float(S_single.item()) == result_S)
     for name, ok in checks.items():
         if not ok:
             print("bench.py: CHECK FAILED: %s" % name, file=sys.stderr, flush=True)
@@ -346,26 +409,47 @@ def run_ours(args, cfg, rank, local_rank, world):
     k_ms = sum(kernel_ms) / len(kernel_ms)
     kernel_triples = triples / world if tiles_mode else triples     # what one launch of rank 0 covers
     peaks = read_peaks()
+    sm_clock_mhz = (clocks or {}).get("sm_mhz") or 1965.0
+    traffic, traffic_src = read_traffic(kernel_name, cfg["index"])
     if variant in (csg.VARIANT_TENSOR, csg.VARIANT_TENSOR_FP4):
-        # dense binary contraction on tcgen05: 1 triple test = 1 MAC = 2 ops.  peak = measured bf16 dense peak x the
-        # nominal ratio of the operand type on B200 (B200_PROFILING.md table: int8/fp8 2x, fp4 4x bf16).
-        ratio = 4.0 if variant == csg.VARIANT_TENSOR_FP4 else 2.0
+        # dense binary contraction on tcgen05: 1 triple test = 1 MAC = 2 ops.  peak = what the tensor cores of THIS device
+        # sustain on the kernel's own instruction (csg_measure_peak: bare tcgen05.mma.cta_group::2 loop, same kind, shape
+        # and operand sources, no producers), measured in this run for ~110 ms, i.e. a kernel timed alone.
+        fp4 = variant == csg.VARIANT_TENSOR_FP4
+        what = csg.PEAK_MMA_MXF4 if fp4 else csg.PEAK_MMA_I8
+        csg.csg_measure_peak(what, 20000)
+        p_ms, p_units = csg.csg_measure_peak(what, 400000)
+        peak = 2.0 * p_units / (p_ms * 1e-3) / 1e12
         achieved = 2.0 * kernel_triples / (k_ms * 1e-3) / 1e12
-        roofline = {"bound": "tensor", "kernel": kernel_name, "achieved": achieved, "peak": ratio * peaks["bf16"],
-                    "unit": "TOP/s (%s)" % ("fp4 e2m1, kind::mxf4" if ratio == 4.0 else "int8, kind::i8"),
-                    "frac": achieved / (ratio * peaks["bf16"]),
-                    "peak_sustained": ratio * peaks["bf16_sustained"],
-                    "frac_of_sustained": achieved / (ratio * peaks["bf16_sustained"]),
-                    "peak_source": "%g x bf16 " % ratio + peaks["source"], "kernel_ms": k_ms,
-                    "traffic": read_traffic(kernel_name)}
+        hw = 2.0 * (16384 if fp4 else 8192) * 148 * sm_clock_mhz * 1e6 / 1e12      # MAC/clk/SM x SMs x sampled clock
+        ratio = 4.0 if fp4 else 2.0
+        roofline = {"bound": "tensor", "kernel": kernel_name, "achieved": achieved, "peak": peak,
+                    "unit": "TOP/s (%s)" % ("fp4 e2m1, kind::mxf4" if fp4 else "int8, kind::i8"),
+                    "frac": achieved / peak,
+                    "peak_source": "measured in this run: csg_measure_peak, bare tcgen05.mma.cta_group::2.kind::%s loop "
+                                   "(M=N=256, %s), 400000 groups of 4 per SM pair, %.1f ms" % (
+                                       "mxf4.block_scale" if fp4 else "i8", "K=64, A in TMEM" if fp4 else "K=32", p_ms),
+                    "frac_of_hw": achieved / hw,
+                    "hw_rate": "%d MAC/clk/SM x 148 SMs x %.0f MHz (sampled) = %.0f TOP/s" % (16384 if fp4 else 8192, sm_clock_mhz, hw),
+                    "frac_of_scaled_bf16": achieved / (ratio * peaks["bf16"]),
+                    "scaled_bf16": "%g x bf16 %s = %.0f TOP/s (power-capped cuBLAS figure; context only)" % (ratio, peaks["source"], ratio * peaks["bf16"]),
+                    "kernel_ms": k_ms, "traffic": traffic, "traffic_source": traffic_src}
     else:
-        # LOP3+POPC+IADD per 32 triple tests; POPC pipe 16 lanes/clk/SM x 148 SMs x 1.965 GHz
-        peak = 16 * 148 * 1.965e9 * 32 / 1e12
+        # LOP3 AND + POPC + IADD per 32 triple tests: peak = measured issue rate of exactly that mix (csg_measure_peak)
+        csg.csg_measure_peak(csg.PEAK_ALU_MIX, 2000)
+        p_ms, p_units = csg.csg_measure_peak(csg.PEAK_ALU_MIX, 20000)
+        peak = 32.0 * p_units / (p_ms * 1e-3) / 1e12
         achieved = kernel_triples / (k_ms * 1e-3) / 1e12
         roofline = {"bound": "alu", "kernel": kernel_name, "achieved": achieved, "peak": peak,
-                    "unit": "T bit-tests/s", "frac": achieved / peak, "peak_source": "derived: POPC 16/clk/SM",
-                    "kernel_ms": k_ms, "traffic": read_traffic(kernel_name)}
+                    "unit": "T bit-tests/s", "frac": achieved / peak,
+                    "peak_source": "measured in this run: csg_measure_peak, AND+POPC+ADD mix on 32-bit words, all SMs "
+                                   "(%.1f lane-steps/clk/SM at %.0f MHz: the POPC pipe)" % (p_units / (p_ms * 1e-3) / 148 / (sm_clock_mhz * 1e6), sm_clock_mhz),
+                    "kernel_ms": k_ms, "traffic": traffic, "traffic_source": traffic_src}
     roofline["hbm_gbs_algorithmic"] = (N * csg.csg_row_stride_words(N) * 8) / (k_ms * 1e-3) / 1e9
+    # what the paper's method would execute of these tests (it skips unrelated pairs, PAPER.md:407 l.4-5)
+    roofline["useful_work_ratio"] = useful_work_ratio(bits, N)
+    roofline["useful_work_note"] = ("sum over related pairs of (j-i-1) / C(N,3): Algorithm 5 executes only this share of the "
+                                    "ordered-triple tests; the dense tiles execute all C(N,3), which is what `achieved` counts")
 
     cpu_baseline = None
     extra = {}
@@ -374,7 +458,8 @@ def run_ours(args, cfg, rank, local_rank, world):
         cpu_baseline = {"value": tests / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
                         "sample": "Algorithm 5 restated (oracle/alg5_packed.c, OpenMP) on %d rows in 16 evenly spaced "
                                   "row blocks of the same causal set, %.1f s; tests = sum over visited pairs of (j-i-1)"
-                                  % (rows, dt)}
+                                  % (rows, dt),
+                        "full_config_s_extrapolated": comb3(N) / (tests / dt)}
         ptests, pdt, pn = plain_oracle_sample(bits, N, kmax)
         extra["cpu_baseline_plain"] = {"value": ptests / pdt, "unit": UNIT, "cores": 1, "kind": "oracle",
                                        "sample": "plain triple loop (oracle/csg_oracle.c) on the first %d elements "
@@ -387,19 +472,19 @@ def run_ours(args, cfg, rank, local_rank, world):
                   csg.VARIANT_TENSOR_FP4: "e2m1 x e2m1 -> f32, exact integers (tcgen05 kind::mxf4, unit scales)",
                   csg.VARIANT_BITSET: "u32 and/popc"}[variant],
         "data": "synthetic",
-        "config": {"workload": workload_name(cfg), "N": N, "dim": dim, "eps": eps, "kmax": kmax, "seed": cfg["seed"],
-                   "variant": {1: "bitset", 2: "tensor_i8", 3: "tensor_fp4"}[variant], "bitset_bytes": N * csg.csg_row_stride_words(N) * 8,
-                   "l2": "input (%.0f MiB) %s L2 (126 MB)" % (N * csg.csg_row_stride_words(N) * 8 / 2**20,
-                                                            "larger than" if N * csg.csg_row_stride_words(N) * 8 > 126e6
-                                                            else "fits in"),
-                   "parallelism": ("1 causal set, tiles sharded over %d GPUs, one int64 all-reduce" % world) if tiles_mode
-                   else "1 causal set per GPU, no collectives", "host_generation_s": gen_s},
+        "config": config_dict(cfg, N, dim, eps, kmax),
+        "variant": {1: "bitset", 2: "tensor_i8", 3: "tensor_fp4"}[variant],
+        "parallelism": ("1 causal set, tiles sharded over %d GPUs, one int64 all-reduce" % world) if tiles_mode
+        else "1 causal set per GPU, no collectives",
+        "host_generation_s": gen_s,
         "action_time_s": ms_total / args.steps * 1e-3,
         "kernel_ms_per_step": kernel_ms,
         "result": {"counts_head": [int(x) for x in result_counts[:4]], "S": result_S},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": N * csg.csg_row_stride_words(N) * 8,
-                "d2h_bytes_per_step": (kmax + 1) * 8 + 8, "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps},
+                "d2h_bytes_per_step": (kmax + 1) * 8 + 8, "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps,
+                "ms_median": sorted(e2e_each)[len(e2e_each) // 2], "ms_best": min(e2e_each),
+                "what": "csg_action_host: pinned host matrix -> H2D in 32 row chunks + one gated launch + D2H of counts and S"},
         "gpu_launches": launches,
         "checks": checks,   # the legs of this run agree with each other (parity with the oracle is the tests' job)
         "roofline": roofline,
@@ -415,7 +500,7 @@ def run_ours(args, cfg, rank, local_rank, world):
         "roofline": {"bound": "alu", "achieved": pairs * fp64_ops / (l_ms * 1e-3) / 1e12, "peak": fp64_peak / 1e12,
                      "unit": "T fp64 instr/s", "frac": pairs * fp64_ops / (l_ms * 1e-3) / fp64_peak,
                      "peak_source": "derived: 64 FP64 lanes/clk/SM x 148 SMs x 1.965 GHz (DESIGN.md)",
-                     "traffic": read_traffic("link_kernel<%s>" % {0: "GEOM_M2", 1: "GEOM_M4", 2: "GEOM_DS2"}[geom])},
+                     "traffic": read_traffic("link_kernel<%s>" % {0: "GEOM_M2", 1: "GEOM_M4", 2: "GEOM_DS2"}[geom], cfg["index"])[0]},
         "e2e_from_coords": {"value": multigpu.whole_job_rate(world * triples, e2e_steps, e2e_coords_ms), "unit": UNIT,
                             "ms_per_step": e2e_coords_ms / e2e_steps, "h2d_bytes_per_step": N * dim * 8,
                             "d2h_bytes_per_step": (kmax + 1) * 8 + 8,
@@ -427,7 +512,7 @@ def run_ours(args, cfg, rank, local_rank, world):
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
-    return 0
+    return 0 if all(checks.values()) else 3          # the line is printed either way; a failed cross-check fails the run
 
 
 def main():

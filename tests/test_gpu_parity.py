@@ -312,7 +312,7 @@ def check_config(csg, cfg, full_reference):
     rng = np.random.default_rng(cfg["seed"])
     nB = (N + 255) // 256
     tiles = [(0, 0), (0, 1), (0, nB - 1), (nB - 1, nB - 1), (nB - 2, nB - 1), (nB // 2, nB // 2), (nB // 2, nB // 2 + 1),
-             (nB // 3, 2 * nB // 3), (1, nB - 2), (nB // 5, nB // 5 + 7)]
+             (nB // 3, 2 * nB // 3), (1, nB - 2), (nB // 5, nB // 5 + 7), (nB // 7, nB - 3), (2 * nB // 3, nB - 1)]
     tiles = [(min(a, nB - 1), min(max(a, b), nB - 1)) for a, b in tiles]
     for variant in ((csg.VARIANT_TENSOR_FP4, csg.VARIANT_TENSOR) if N <= 131072 else (csg.VARIANT_TENSOR_FP4,)):
         csg.csg_set_variant(variant)
@@ -322,7 +322,7 @@ def check_config(csg, cfg, full_reference):
             tile = dump[t]
             rr, cc = np.nonzero(tile >= 0)
             edge = np.isin(rr, (0, 1, 127, 128, 254, 255)) | np.isin(cc, (0, 1, 127, 128, 254, 255))
-            pick = np.concatenate([rng.permutation(np.nonzero(edge)[0])[:600], rng.permutation(np.nonzero(~edge)[0])[:600]])
+            pick = np.concatenate([rng.permutation(np.nonzero(edge)[0])[:800], rng.permutation(np.nonzero(~edge)[0])[:800]])
             for k in pick:
                 i, j = 256 * I + int(rr[k]), 256 * J + int(cc[k])
                 assert tile[rr[k], cc[k]] == oracle.pair_interval(bits, N, i, j), (variant, I, J, i, j)
