@@ -484,7 +484,7 @@ def run_ours(args, cfg, rank, local_rank, world):
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": N * csg.csg_row_stride_words(N) * 8,
                 "d2h_bytes_per_step": (kmax + 1) * 8 + 8, "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps,
                 "ms_median": sorted(e2e_each)[len(e2e_each) // 2], "ms_best": min(e2e_each),
-                "what": "csg_action_host: pinned host matrix -> H2D in 32 row chunks + one gated launch + D2H of counts and S"},
+                "what": "csg_action_host: pinned host matrix -> H2D in 64 row chunks (outside-in) + one gated launch + D2H of counts and S"},
         "gpu_launches": launches,
         "checks": checks,   # the legs of this run agree with each other (parity with the oracle is the tests' job)
         "roofline": roofline,

@@ -140,10 +140,10 @@ int64_t csg_tile_schedule(int64_t N, int shard, int nshards, int32_t *tiles_ij, 
  * Same computation with HOST buffers (the end-to-end call): copies rel_bits to the device (pinned or
  * pageable host memory), runs csg_action on an internal stream, copies counts and S back and
  * synchronises.  rel_bits_host: N*stride words; counts_host: kmax+1 int64; S_host: 1 double.
- * Matrices of 32 MiB and more go over in 32 row chunks on a copy stream while ONE persistent launch of the
- * interval kernel already runs: after each chunk the copy stream publishes the number of rows landed
- * (cuStreamWriteValue32) and a tile starts when the rows it reads are there (overlap of the
- * transfer with the computation).
+ * Matrices of 32 MiB and more go over in 64 row chunks, outermost chunks first, on a copy stream while ONE
+ * persistent launch of the interval kernel already runs: after each chunk the copy stream publishes how many have
+ * been delivered (cuStreamWriteValue32) and a tile starts when the two row blocks it reads are there
+ * (overlap of the transfer with the computation).
  */
 int csg_action_host(const uint64_t *rel_bits_host, int64_t N, int dim, double eps, int kmax,
                     int64_t *counts_host, double *S_host);

@@ -100,12 +100,13 @@ struct TileList {                       // tile schedule of one (N, shard, nshar
     int2* d;
     int n;
 };
-struct ChunkTiles {                     // the same tiles grouped by the row chunk of the host-matrix pipeline
+struct ChunkTiles {                     // the same tiles ordered by when the host-matrix pipeline makes them runnable
     long long N;
-    int2* d;
+    int2* d;                            // tiles, sorted by need (stable: deepest first / patch order inside a step)
+    int* d_need;                        // per tile: copy steps that must have completed before it may start
     int n;
-    std::vector<int> off;               // chunk c owns tiles [off[c], off[c+1])
-    std::vector<long long> row_end;
+    std::vector<int> off;               // tiles [off[s], off[s+1]) become runnable when copy step s completes
+    std::vector<long long> row_begin, row_end;   // rows copied by step s
 };
 struct BitsMap {                        // TMA descriptor of a relation matrix (passed to the kernel by value)
     const void* ptr;
@@ -127,7 +128,7 @@ struct Device {
     cudaEvent_t ev0[TIMING_RING] = {}, ev1[TIMING_RING] = {};
     long long timed_calls = 0;
     unsigned int* d_progress = nullptr; // PROGRESS_RING finished-tile counters, one per launch in flight (drift throttle)
-    unsigned int* d_rows_ready = nullptr;   // rows of the host matrix landed so far (gate of csg_action_host)
+    unsigned int* d_landed = nullptr;   // chunks of the host matrix delivered so far (gate of csg_action_host)
     // end-to-end (host buffer) path
     cudaStream_t host_stream = nullptr, copy_stream = nullptr;
     uint64_t* d_bits = nullptr;
@@ -388,11 +389,11 @@ static int ensure_tensor_ready(Device* D) {
     return CSG_OK;
 }
 
-// One launch of the tensor kernel over a tile list (counts are added to, not zeroed).  rows_ready: gate of the
-// host-matrix path (NULL when the matrix is resident); dump: csg_tile_interval_sizes (NULL otherwise).
+// One launch of the tensor kernel over a tile list (counts are added to, not zeroed).  landed / tile_need: gate of
+// the host-matrix path (NULL when the matrix is resident); dump: csg_tile_interval_sizes (NULL otherwise).
 static int launch_tensor(Device* D, int kind, const uint64_t* rel_bits, long long N, long long stride, int kmax,
-                         long long* counts, const int2* d_tiles, int ntiles, const unsigned int* rows_ready, int* dump,
-                         cudaStream_t stream) {
+                         long long* counts, const int2* d_tiles, int ntiles, const unsigned int* landed,
+                         const int* tile_need, int* dump, cudaStream_t stream) {
     int rc = ensure_tensor_ready(D);
     if (rc) return rc;
     const CUtensorMap* map = nullptr;
@@ -416,13 +417,13 @@ static int launch_tensor(Device* D, int kind, const uint64_t* rel_bits, long lon
     unsigned long long* c64 = reinterpret_cast<unsigned long long*>(counts);
     const int s8 = TcTraits<KIND_I8>::SMEM_BYTES, s4 = TcTraits<KIND_FP4>::SMEM_BYTES;
 #define CSG_LAUNCH(KERNEL, SMEM) \
-    KERNEL<<<grid, TC_THREADS, SMEM, stream>>>(*map, rel_bits, N, stride, kmax, c64, d_tiles, ntiles, g.debug, progress, rows_ready, dump)
+    KERNEL<<<grid, TC_THREADS, SMEM, stream>>>(*map, rel_bits, N, stride, kmax, c64, d_tiles, ntiles, g.debug, progress, landed, tile_need, dump)
     // int8: operand bit TB: the accumulator holds n_ij << 2TB and n_ij <= N-2, so TB is the largest with
     // (N-2) << 2TB < 2^31; TB = 7 turns every unpack shift into a left shift (FMA pipe).
     const int tb = N - 2 < (1LL << 17) ? 7 : N - 2 < (1LL << 19) ? 6 : N - 2 < (1LL << 21) ? 5 : 4;
     if (kind == KIND_FP4) {
         if (dump) CSG_LAUNCH((tensor_action_kernel<KIND_FP4, 0, TCF_DUMP>), s4);
-        else if (progress || rows_ready) CSG_LAUNCH((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA | TCF_WAIT>), s4);
+        else if (progress || landed) CSG_LAUNCH((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA | TCF_WAIT>), s4);
         else CSG_LAUNCH((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA>), s4);
     } else if (dump) {
         if (tb == 7) CSG_LAUNCH((tensor_action_kernel<KIND_I8, 7, TCF_DUMP>), s8);
@@ -464,7 +465,7 @@ static int interval_device(Device* D, const uint64_t* rel_bits, long long N, int
         CSG_CUDA(cudaEventRecord(D->ev0[slot], stream));
     }
     if (tensor) {
-        rc = launch_tensor(D, kind, rel_bits, N, stride, kmax, counts, tl->d, tl->n, nullptr, nullptr, stream);
+        rc = launch_tensor(D, kind, rel_bits, N, stride, kmax, counts, tl->d, tl->n, nullptr, nullptr, nullptr, stream);
         if (rc) return rc;
     } else {
         const long long nb = (N + BS_T - 1) / BS_T;
@@ -501,16 +502,20 @@ static int action_device(Device* D, const uint64_t* rel_bits, long long N, int d
 }
 
 // Host matrix -> device in row chunks on a copy stream while the tiles already run (Sec. 2.2.5:
-// overlap of transfers with compute).  A tile (I, J) reads rows of blocks I <= J only, and the work of chunk c grows
-// like (c+1)^2 - c^2, so the copies of all but the first chunks hide behind the tiles of the chunks before them: the
-// 2 GiB copy of N = 131072 (38 ms over PCIe) costs a few ms instead.  The tile list is ordered by the chunk that holds
-// a tile's later row block (inside a chunk: deepest first, patch order).  Two ways to run it:
+// overlap of transfers with compute).  A tile (I, J) reads the rows of blocks I and J only, so it is runnable as soon
+// as the chunks holding those two blocks have landed.  The chunks are copied OUTSIDE-IN (first, last, second, ...):
+// the first two chunks already make the deepest tiles of the triangle runnable, and after a fraction f of the copy
+// 1.5 f^2 - 0.5 f^3 of the work is available instead of the f^3 of a front-to-back copy.  With the copy taking T_c and
+// the kernel T_k the transfer then costs max_f [T_c f - T_k (1.5 f^2 - 0.5 f^3)]: about 3 ms at N = 131072 (41 ms of
+// PCIe copy, 91 ms of kernel) against 10.6 ms front to back (measured 10.9) and 41 ms without overlap.
+// The tile list is sorted by the copy step that makes a tile runnable (stable, so inside a step the schedule's
+// deepest-first patch order survives).  Two ways to run it:
 //   gated (fp4 kind, when the driver offers cuStreamWriteValue32): ONE persistent launch; after every chunk the copy
-//     stream publishes the number of rows landed and the TMA thread of a cluster waits for the rows its next tile
-//     needs -- no launch tails between chunks;
-//   chunked launches (int8 kind, or no stream memory operations): one launch per chunk behind an event.
+//     stream publishes the number of chunks delivered and the TMA thread of a cluster waits for the count its next
+//     tile needs -- no launch tails between chunks;
+//   chunked launches (int8 kind, or no stream memory operations): one launch per copy step behind an event.
 // Tensor variants and large matrices only.
-constexpr int HOST_CHUNKS = 32;
+constexpr int HOST_CHUNKS = 64;
 constexpr long long HOST_PIPELINE_MIN_BYTES = 32LL << 20;
 
 static int ensure_chunk_tiles(Device* D, long long N, const ChunkTiles** out) {
@@ -522,25 +527,39 @@ static int ensure_chunk_tiles(Device* D, long long N, const ChunkTiles** out) {
     const int nB = (int)((N + TC_T - 1) / TC_T);
     const int blocks_per_chunk = (nB + HOST_CHUNKS - 1) / HOST_CHUNKS;
     const int nchunks = (nB + blocks_per_chunk - 1) / blocks_per_chunk;
-    std::vector<int2> all;
-    build_tile_schedule(N, 0, 1, all);
-    std::vector<std::vector<int2>> per(nchunks);
-    for (const int2& t : all) per[t.y / blocks_per_chunk].push_back(t);   // keeps the deepest-first, patch order
-    std::vector<int2> flat;
+    // copy order outside-in: chunk 0, nchunks-1, 1, nchunks-2, ...; step_of[c] = position of chunk c in that order
+    std::vector<int> step_of(nchunks);
     ChunkTiles* c = new ChunkTiles;
     c->N = N;
     c->d = nullptr;
+    c->d_need = nullptr;
+    for (int s = 0, lo = 0, hi = nchunks - 1; s < nchunks; ++s) {
+        const int chunk = (s & 1) ? hi-- : lo++;
+        step_of[chunk] = s;
+        c->row_begin.push_back((long long)chunk * blocks_per_chunk * TC_T);
+        c->row_end.push_back(std::min<long long>(N, (long long)(chunk + 1) * blocks_per_chunk * TC_T));
+    }
+    std::vector<int2> all;
+    build_tile_schedule(N, 0, 1, all);
+    std::vector<std::vector<int2>> per(nchunks);
+    for (const int2& t : all)       // runnable after the later of its two chunks; keeps the schedule's order inside a step
+        per[std::max(step_of[t.x / blocks_per_chunk], step_of[t.y / blocks_per_chunk])].push_back(t);
+    std::vector<int2> flat;
+    std::vector<int> need;
     c->off.assign(1, 0);
-    for (int k = 0; k < nchunks; ++k) {
-        flat.insert(flat.end(), per[k].begin(), per[k].end());
+    for (int s = 0; s < nchunks; ++s) {
+        flat.insert(flat.end(), per[s].begin(), per[s].end());
+        need.insert(need.end(), per[s].size(), s + 1);
         c->off.push_back((int)flat.size());
-        c->row_end.push_back(std::min<long long>(N, (long long)(k + 1) * blocks_per_chunk * TC_T));
     }
     c->n = (int)flat.size();
     cudaError_t e = cudaMalloc(&c->d, flat.size() * sizeof(int2));
+    if (e == cudaSuccess) e = cudaMalloc(&c->d_need, need.size() * sizeof(int));
     if (e == cudaSuccess) e = cudaMemcpy(c->d, flat.data(), flat.size() * sizeof(int2), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(c->d_need, need.data(), need.size() * sizeof(int), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) {
         if (c->d) cudaFree(c->d);
+        if (c->d_need) cudaFree(c->d_need);
         delete c;
         return cuda_fail(e, "tile list of the host pipeline");
     }
@@ -576,31 +595,30 @@ static int interval_host_pipelined(Device* D, const uint64_t* rel_bits_host, uin
     if (rc) return rc;
     if (!D->copy_stream) CSG_CUDA(cudaStreamCreateWithFlags(&D->copy_stream, cudaStreamNonBlocking));
     CSG_CUDA(cudaMemsetAsync(counts, 0, (size_t)(kmax + 1) * sizeof(long long), stream));
-    const int nchunks = (int)ct->row_end.size();
+    const int nchunks = (int)ct->row_end.size();       // = copy steps
     cudaEvent_t ev_prev = D->chunk_ev[nchunks], ev_reset = D->chunk_ev[nchunks + 1];
     // the copies must not overtake work of an earlier call that still reads d_bits on `stream`
     CSG_CUDA(cudaEventRecord(ev_prev, stream));
     CSG_CUDA(cudaStreamWaitEvent(D->copy_stream, ev_prev, 0));
     WriteValue32Fn write32 = kind == KIND_FP4 ? stream_write_value32() : nullptr;
     if (write32) {
-        if (!D->d_rows_ready) CSG_CUDA(cudaMalloc(&D->d_rows_ready, sizeof(unsigned int)));
+        if (!D->d_landed) CSG_CUDA(cudaMalloc(&D->d_landed, sizeof(unsigned int)));
         // reset the gate, then ONE launch that starts at once and follows the copies
-        if (write32(D->copy_stream, (CUdeviceptr)D->d_rows_ready, 0u, 0) != CUDA_SUCCESS) {
+        if (write32(D->copy_stream, (CUdeviceptr)D->d_landed, 0u, 0) != CUDA_SUCCESS) {
             write32 = nullptr;                                 // no stream memory operations here: chunked launches
         } else {
             CSG_CUDA(cudaEventRecord(ev_reset, D->copy_stream));
             CSG_CUDA(cudaStreamWaitEvent(stream, ev_reset, 0));
-            rc = launch_tensor(D, kind, d_bits, N, stride, kmax, counts, ct->d, ct->n, D->d_rows_ready, nullptr, stream);
+            rc = launch_tensor(D, kind, d_bits, N, stride, kmax, counts, ct->d, ct->n, D->d_landed, ct->d_need, nullptr, stream);
             if (rc) return rc;
         }
     }
-    long long row0 = 0;
     for (int c = 0; c < nchunks; ++c) {
-        const long long row1 = ct->row_end[c];
+        const long long row0 = ct->row_begin[c], row1 = ct->row_end[c];
         CSG_CUDA(cudaMemcpyAsync(d_bits + row0 * stride, rel_bits_host + row0 * stride,
                                  (size_t)(row1 - row0) * stride * sizeof(uint64_t), cudaMemcpyHostToDevice, D->copy_stream));
         if (write32) {
-            if (write32(D->copy_stream, (CUdeviceptr)D->d_rows_ready, (cuuint32_t)row1, 0) != CUDA_SUCCESS) {
+            if (write32(D->copy_stream, (CUdeviceptr)D->d_landed, (cuuint32_t)(c + 1), 0) != CUDA_SUCCESS) {
                 snprintf(g.cuda_msg, sizeof(g.cuda_msg), "cuStreamWriteValue32 failed while a gated launch is waiting");
                 return CSG_E_CUDA;
             }
@@ -609,11 +627,10 @@ static int interval_host_pipelined(Device* D, const uint64_t* rel_bits_host, uin
             CSG_CUDA(cudaStreamWaitEvent(stream, D->chunk_ev[c], 0));
             const int nt = ct->off[c + 1] - ct->off[c];
             if (nt > 0) {
-                rc = launch_tensor(D, kind, d_bits, N, stride, kmax, counts, ct->d + ct->off[c], nt, nullptr, nullptr, stream);
+                rc = launch_tensor(D, kind, d_bits, N, stride, kmax, counts, ct->d + ct->off[c], nt, nullptr, nullptr, nullptr, stream);
                 if (rc) return rc;
             }
         }
-        row0 = row1;
     }
     return CSG_OK;
 }
@@ -664,6 +681,7 @@ static void release_device(Device* D) {
     for (TileList& t : D->tiles) cudaFree(t.d);
     for (ChunkTiles* c : D->chunk_tiles) {
         cudaFree(c->d);
+        cudaFree(c->d_need);
         delete c;
     }
     if (D->d_bits) cudaFree(D->d_bits);
@@ -671,7 +689,7 @@ static void release_device(Device* D) {
     if (D->d_S) cudaFree(D->d_S);
     if (D->d_coords) cudaFree(D->d_coords);
     if (D->d_progress) cudaFree(D->d_progress);
-    if (D->d_rows_ready) cudaFree(D->d_rows_ready);
+    if (D->d_landed) cudaFree(D->d_landed);
     for (cudaEvent_t e : D->chunk_ev) cudaEventDestroy(e);
     if (D->copy_stream) cudaStreamDestroy(D->copy_stream);
     if (D->host_stream) cudaStreamDestroy(D->host_stream);
@@ -915,7 +933,7 @@ int csg_tile_interval_sizes(const uint64_t* rel_bits, int64_t N, const int32_t* 
     cudaError_t e = cudaMemcpy(d_tiles, tiles_ij_host, (size_t)ntiles * sizeof(int2), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) {
         rc = launch_tensor(D, variant == CSG_VARIANT_TENSOR_FP4 ? KIND_FP4 : KIND_I8, rel_bits, N, csg_row_stride_words(N),
-                           0, nullptr, d_tiles, (int)ntiles, nullptr, n_out, stream);
+                           0, nullptr, d_tiles, (int)ntiles, nullptr, nullptr, n_out, stream);
         e = cudaStreamSynchronize(stream);
     }
     cudaFree(d_tiles);

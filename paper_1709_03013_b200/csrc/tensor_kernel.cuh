@@ -391,18 +391,19 @@ __device__ __forceinline__ void tile_k_range(int I, int J, int& kb_begin, int& k
 // 4^TB, the accumulator holds n_ij << 2TB; the host picks the largest TB with (N-2) << 2TB < 2^31 (exact in s32).
 // KIND_FP4: TB unused (pass 0); the f32 accumulator holds 4 n_ij, exact for n_ij < 2^22.
 // tiles[t] = {I, J}: 256-row blocks, I <= J.  Grid = 2 x (number of SM pairs), cluster (2,1,1).
-// progress (TCF_WAIT, may be NULL): zeroed counter of finished tiles, the drift throttle.  rows_ready (TCF_WAIT, may
-// be NULL): number of matrix rows that have landed in `rel` so far, written by the host-copy stream; a tile (I, J)
-// starts once rows < 256 (J+1) are there.  dump (TCF_DUMP): ntiles x 256 x 256 int32, n_ij or -1.
+// progress (TCF_WAIT, may be NULL): zeroed counter of finished tiles, the drift throttle.  landed / tile_need (TCF_WAIT,
+// may be NULL): the host-copy gate -- *landed = number of row chunks of `rel` the copy stream has delivered so far,
+// tile_need[t] = how many must be there before tile t may start.  dump (TCF_DUMP): ntiles x 256 x 256 int32, n_ij or -1.
 template <int KIND, int TB, int FLAGS = 0>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(TC_THREADS, 1)
 tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_t* __restrict__ rel, long long N,
                      long long stride_words, int kmax, unsigned long long* __restrict__ counts,
                      const int2* __restrict__ tiles, int ntiles, int dbg_arg, unsigned int* __restrict__ progress_arg,
-                     const unsigned int* __restrict__ rows_ready_arg, int* __restrict__ dump) {
+                     const unsigned int* __restrict__ landed_arg, const int* __restrict__ tile_need,
+                     int* __restrict__ dump) {
     constexpr bool ABLATE = (FLAGS & TCF_ABLATE) != 0, WAITS = (FLAGS & TCF_WAIT) != 0, DUMP = (FLAGS & TCF_DUMP) != 0;
     unsigned int* const progress = WAITS ? progress_arg : nullptr;      // compiled out of the instantiations that never wait
-    const unsigned int* const rows_ready = WAITS ? rows_ready_arg : nullptr;
+    const unsigned int* const landed = WAITS ? landed_arg : nullptr;
     using T = TcTraits<KIND>;
     const int dbg = ABLATE ? dbg_arg : 0;             // compiled out of every instantiation of libcsg.so
     constexpr int COLS = T::STAGE_COLS, WORDS = T::WORDS;
@@ -521,27 +522,44 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
             mbar_wait(tmem_full, tphase);
             tphase ^= 1;
             tc_fence_after();
+            // Both 32-column chunks of this thread go to registers first; the accumulators are then handed back to the MMA
+            // thread (tmem_empty) BEFORE the values are looked at, so the next tile's MMAs -- their first stages are already
+            // in the ring -- run while this tile is bucketed.  The accumulator encodes n_ij monotonically (fp4: the f32 bit
+            // pattern of 4 n, int8: n << 2TB), so "n <= kmax" is one unsigned compare against vmax with no conversion
+            // (F2I runs at a quarter of the ALU rate and made the epilogue the longest part of a tile boundary); only the
+            // values that pass are decoded.
+            const int kcap = (int)min((long long)kmax, N - 2 < 0 ? 0LL : N - 2);       // n_ij never exceeds N-2
+            const uint32_t vmax = KIND == KIND_FP4 ? __float_as_uint(4.0f * (float)kcap) : ((uint32_t)kcap << (2 * TB));
+            uint32_t v0[32], v1[32];
+            if (!(dbg & 8)) {
+                tmem_ld_32x32(tmem_base + ((uint32_t)(32 * q4) << 16) + (uint32_t)(32 * (2 * cq)), v0);
+                tmem_ld_32x32(tmem_base + ((uint32_t)(32 * q4) << 16) + (uint32_t)(32 * (2 * cq + 1)), v1);
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(tmem_empty_leader);
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
                 if (dbg & 8) break;                   // ablation: no epilogue work
-                uint32_t v[32];
-                tmem_ld_32x32(tmem_base + ((uint32_t)(32 * q4) << 16) + (uint32_t)(32 * (2 * cq + e)), v);
                 const uint32_t rw = relw[e];
+                if (!DUMP && rw == 0u) continue;      // no related pair among these 32 columns
 #pragma unroll
                 for (int x = 0; x < 32; ++x) {
-                    const int n = KIND == KIND_FP4 ? (int)(__uint_as_float(v[x]) * 0.25f) : (int)(v[x] >> (2 * TB));
+                    const uint32_t v = e == 0 ? v0[x] : v1[x];
                     if (DUMP) {                       // test hook: every n_ij of the tile, -1 where i, j are not a related pair
+                        const int n = KIND == KIND_FP4 ? (int)(__uint_as_float(v) * 0.25f) : (int)(v >> (2 * TB));
                         dump[((size_t)et * TC_T + (size_t)(128 * (int)rank + 32 * q4 + lane)) * TC_T + 32 * (2 * cq + e) + x] =
                             ((rw >> x) & 1u) ? n : -1;
-                    } else if (((rw >> x) & 1u) && n <= kmax) {
+                    } else if ((rw & (1u << x)) && v <= vmax) {
+                        // fp4: 4 n < 2^24 is an exact f32; n = low 23 bits of (4n * 0.25 + 2^23)
+                        const int n = KIND == KIND_FP4
+                                          ? (int)(__float_as_uint(fmaf(__uint_as_float(v), 0.25f, 8388608.0f)) & 0x7FFFFFu)
+                                          : (int)(v >> (2 * TB));
                         if (n < TC_HIST) atomicAdd(&hist[n], 1u);
                         else atomicAdd(&counts[n], 1ULL);
                     }
                 }
             }
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(tmem_empty_leader);
             // one count per finished tile of this cluster (throttle of the TMA threads, see below)
             if (progress != nullptr && rank == 0 && tid == 0) atomicAdd(progress, 1u);
         };
@@ -754,7 +772,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
         if (lane == 0) {
             uint32_t bb = 0, bphase = 0;
             bool throttling = true;
-            unsigned int rows_seen = 0;
+            unsigned int chunks_seen = 0;
             for (int rd = 0; rd < rounds; ++rd) {
                 const int t = rd * G + ((rd & 1) ? (G - 1 - cl) : cl);
                 if (t >= ntiles) continue;
@@ -781,18 +799,19 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                     }
                 }
                 // Host-copy gate (csg_action_host): the matrix arrives in row chunks on a copy stream, which publishes the
-                // number of rows landed after each chunk; tile (I, J) reads rows below 256 (J+1) only.  The wait depends
-                // on the copy engine alone, never on another CTA.
-                if (WAITS && rows_ready != nullptr) {
-                    const unsigned int need_rows = (unsigned int)min((long long)(tile.y + 1) * TC_T, N);
-                    if (rows_seen < need_rows) {
+                // number of chunks delivered after each one; tile (I, J) reads the rows of blocks I and J only, and the
+                // host has worked out how many chunks that takes in its copy order.  The wait depends on the copy engine
+                // alone, never on another CTA.
+                if (WAITS && landed != nullptr) {
+                    const unsigned int need = (unsigned int)tile_need[t];
+                    if (chunks_seen < need) {
                         unsigned int got;
                         while (true) {
-                            asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(got) : "l"(rows_ready) : "memory");
-                            if (got >= need_rows) break;
+                            asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(got) : "l"(landed) : "memory");
+                            if (got >= need) break;
                             __nanosleep(500);
                         }
-                        rows_seen = got;
+                        chunks_seen = got;
                         asm volatile("fence.proxy.async.global;" ::: "memory");   // the bytes are read by the async proxy (TMA)
                     }
                 }
