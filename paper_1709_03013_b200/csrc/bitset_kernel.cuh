@@ -8,8 +8,15 @@
 // 64 times.  The open range i<k<j is applied when a row segment is staged: row i keeps only columns > i
 // (operand "U"), row j keeps only columns < j (operand "L"), so n_ij = sum_k U[i][k] & L[j][k] with no
 // per-pair masking in the inner loop.
+//
+// Small sets are launch-bound (N = 1024: ~14 us of kernel), so for them the memset before and the finishing kernel
+// after are folded into this launch (`fused` != NULL): CTAs add their histograms into a zeroed library workspace, the
+// last CTA to finish (a ticket) moves the sums to `counts`, re-zeroes the workspace for the next launch on the same
+// stream and computes S (finish.cuh).
 #pragma once
 #include <cstdint>
+
+#include "finish.cuh"
 
 namespace csg {
 
@@ -18,6 +25,13 @@ constexpr int BS_KW = 32;        // 32-bit words per K-chunk
 constexpr int BS_LD = 36;        // shared row stride in words (32 + 4 pad: conflict-free 128-bit reads)
 constexpr int BS_THREADS = 256;
 constexpr int BS_HIST = 2048;    // privatised low bins per CTA
+constexpr int BS_FUSED_BINS = 1024;   // fused single-launch path: kmax + 1 <= this (N <= 1024 under CSG_VARIANT_AUTO)
+
+// Workspace of the fused path, one per stream (launches on one stream run one after the other): all zero between launches.
+struct BitsetFusedWs {
+    unsigned long long acc[BS_FUSED_BINS];
+    unsigned int ticket;
+};
 
 // Bits of 32-bit word kw (columns 32kw..32kw+31) with column index > i.
 __device__ __forceinline__ uint32_t mask_cols_gt(long long i, long long kw) {
@@ -47,7 +61,8 @@ __device__ __forceinline__ void bitset_tile_from_index(long long t, long long nb
 __global__ void __launch_bounds__(BS_THREADS, 2)
 bitset_action_kernel(const uint32_t* __restrict__ rel, long long N, long long stride32, int kmax,
                      unsigned long long* __restrict__ counts, long long nb, long long ntiles, int shard,
-                     int nshards, long long set_stride32, long long counts_stride) {
+                     int nshards, long long set_stride32, long long counts_stride, BitsetFusedWs* __restrict__ fused,
+                     int dim, double eps, double* __restrict__ S) {
     // blockIdx.y = causal set of a batch (csg_action_batch): same N, matrices set_stride32 words apart
     rel += (long long)blockIdx.y * set_stride32;
     counts += (long long)blockIdx.y * counts_stride;
@@ -142,8 +157,28 @@ bitset_action_kernel(const uint32_t* __restrict__ rel, long long N, long long st
     }
 
     __syncthreads();
+    unsigned long long* const target = fused ? fused->acc : counts;
     for (int b = tid; b < BS_HIST && b <= kmax; b += BS_THREADS)
-        if (hist[b]) atomicAdd(&counts[b], (unsigned long long)hist[b]);
+        if (hist[b]) atomicAdd(&target[b], (unsigned long long)hist[b]);
+    if (fused == nullptr) return;
+    // ---- fused tail (single set, kmax < BS_FUSED_BINS): the last CTA publishes counts and S
+    __shared__ unsigned int is_last;
+    __threadfence();                                  // this CTA's sums are visible before its ticket is
+    __syncthreads();
+    if (tid == 0) is_last = atomicAdd(&fused->ticket, 1u) == gridDim.x - 1 ? 1u : 0u;
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    long long* sums = reinterpret_cast<long long*>(sB);          // 9216 bytes >= BS_FUSED_BINS x 8
+    double* red = reinterpret_cast<double*>(sA);                 // 9216 bytes >= FIN_LANES x 8
+    for (int b = tid; b < BS_FUSED_BINS; b += BS_THREADS) {
+        const unsigned long long v = b <= kmax ? atomicExch(&fused->acc[b], 0ULL) : 0ULL;   // read and re-zero
+        sums[b] = (long long)v;
+        if (b <= kmax) counts[b] = v;
+    }
+    if (tid == 0) fused->ticket = 0u;
+    __syncthreads();
+    finish_block(sums, N, dim, eps, kmax, S, red);
 }
 
 // Test hook (csg_interval_sizes): one warp per listed pair, straight AND+POPC over the open range.

@@ -9,10 +9,12 @@
 #include <cstdio>
 #include <cstring>
 #include <cstdlib>
+#include <map>
 #include <mutex>
 #include <vector>
 
 #include "../../include/csg.h"
+#include "finish.cuh"
 #include "bitset_kernel.cuh"
 #include "link_kernel.cuh"
 #include "tensor_kernel.cuh"
@@ -21,67 +23,14 @@
 namespace csg {
 
 // ---------------------------------------------------------------------------------------------- finishing
-// counts -> S.  One CTA.
-//   eps == 1, dim 2: Eq. 4 with n_i = counts[i-1]:  S = 2 (N - 2 N_0 + 4 N_1 - 2 N_2)
-//   eps == 1, dim 4: S = (4/sqrt 6)(N - N_0 + 9 N_1 - 16 N_2 + 8 N_3)   (not in the paper; A8)
-//   eps <  1, dim 2: Eq. 5: S = 2 eps [N - 2 eps sum_k N_k f_2(k, eps)],
-//                    f_2(k,e) = (1-e)^k - 2 e k (1-e)^(k-1) + e^2 k(k-1)/2 (1-e)^(k-2)   (bracket multiplied out)
-//   eps <  1, dim 4: S = (4/sqrt 6) sqrt(eps) [N - eps sum_k N_k f_4(k, eps)]   (not in the paper; A9),
-//                    f_4(k,e) = (1-e)^k - 9 e k (1-e)^(k-1) + 8 e^2 k(k-1) (1-e)^(k-2) - (4/3) e^3 k(k-1)(k-2) (1-e)^(k-3)
-// The integer combinations are exact in int64 and below 2^53, so the local S is one exact product.
-// The smeared sum is a fixed-order (thread-strided, compensated, then tree) double reduction: deterministic.
+// counts -> S (csrc/finish.cuh).  One CTA per causal set of a batch.
 constexpr int FIN_THREADS = 1024;
 
 __global__ void __launch_bounds__(FIN_THREADS, 1)
 finish_action_kernel(const long long* __restrict__ counts, long long N, int dim, double eps, int kmax,
                      double* __restrict__ S) {
-    __shared__ double red[FIN_THREADS];
-    counts += (long long)blockIdx.x * (kmax + 1);     // one CTA per causal set of a batch
-    S += blockIdx.x;
-    const int tid = threadIdx.x;
-    if (eps == 1.0) {
-        if (tid == 0) {
-            if (dim == 2) {
-                const long long I2 = N - 2 * counts[0] + 4 * counts[1] - 2 * counts[2];
-                *S = 2.0 * (double)I2;
-            } else {
-                const long long I4 = N - counts[0] + 9 * counts[1] - 16 * counts[2] + 8 * counts[3];
-                *S = (4.0 / sqrt(6.0)) * (double)I4;
-            }
-        }
-        return;
-    }
-    const double x = 1.0 - eps;
-    double sum = 0.0, comp = 0.0;
-    for (long long k = tid; k <= kmax; k += FIN_THREADS) {
-        const long long c = counts[k];
-        if (c == 0) continue;
-        const double dk = (double)k;
-        double w = pow(x, dk);
-        if (dim == 2) {
-            if (k >= 1) w -= 2.0 * eps * dk * pow(x, dk - 1.0);
-            if (k >= 2) w += 0.5 * eps * eps * dk * (dk - 1.0) * pow(x, dk - 2.0);
-        } else {
-            if (k >= 1) w -= 9.0 * eps * dk * pow(x, dk - 1.0);
-            if (k >= 2) w += 8.0 * eps * eps * dk * (dk - 1.0) * pow(x, dk - 2.0);
-            if (k >= 3) w -= (4.0 / 3.0) * eps * eps * eps * dk * (dk - 1.0) * (dk - 2.0) * pow(x, dk - 3.0);
-        }
-        const double term = (double)c * w;
-        const double y = term - comp;
-        const double t = sum + y;
-        comp = (t - sum) - y;
-        sum = t;
-    }
-    red[tid] = sum;
-    __syncthreads();
-    for (int s = FIN_THREADS / 2; s > 0; s >>= 1) {
-        if (tid < s) red[tid] += red[tid + s];
-        __syncthreads();
-    }
-    if (tid == 0) {
-        if (dim == 2) *S = 2.0 * eps * ((double)N - 2.0 * eps * red[0]);
-        else *S = (4.0 / sqrt(6.0)) * sqrt(eps) * ((double)N - eps * red[0]);
-    }
+    __shared__ double red[FIN_LANES];
+    finish_block(counts + (long long)blockIdx.x * (kmax + 1), N, dim, eps, kmax, S + blockIdx.x, red);
 }
 
 // ---------------------------------------------------------------------------------------------- host state
@@ -128,6 +77,7 @@ struct Device {
     cudaEvent_t ev0[TIMING_RING] = {}, ev1[TIMING_RING] = {};
     long long timed_calls = 0;
     unsigned int* d_progress = nullptr; // PROGRESS_RING finished-tile counters, one per launch in flight (drift throttle)
+    std::map<cudaStream_t, BitsetFusedWs*> fused_ws;   // fused small-N launch: one zeroed workspace per stream
     unsigned int* d_landed = nullptr;   // chunks of the host matrix delivered so far (gate of csg_action_host)
     // end-to-end (host buffer) path
     cudaStream_t host_stream = nullptr, copy_stream = nullptr;
@@ -475,7 +425,7 @@ static int interval_device(Device* D, const uint64_t* rel_bits, long long N, int
         bitset_action_kernel<<<grid, BS_THREADS, 0, stream>>>(reinterpret_cast<const uint32_t*>(rel_bits), N,
                                                                stride * 2, kmax,
                                                                reinterpret_cast<unsigned long long*>(counts), nb,
-                                                               ntiles, shard, nshards, 0, 0);
+                                                               ntiles, shard, nshards, 0, 0, nullptr, 0, 1.0, nullptr);
         CSG_CUDA(cudaGetLastError());
         ++g.launches;
     }
@@ -494,8 +444,54 @@ static int finish_device(const long long* counts, long long N, int dim, double e
     return CSG_OK;
 }
 
+// Small sets on the bitset variant: memset, interval kernel and finishing kernel in ONE launch (bitset_kernel.cuh).
+// The workspace is per stream, so launches that share it run one after the other; a stream that is being captured
+// (the graph may later run next to eager launches of its source stream) and the per-thread default stream (one
+// handle, many streams) take the three-node path instead.
+static bool fused_small_ok(long long N, int kmax, cudaStream_t stream) {
+    if (effective_variant(N) != CSG_VARIANT_BITSET || kmax >= BS_FUSED_BINS || stream == cudaStreamPerThread) return false;
+    cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(stream, &st) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    return st == cudaStreamCaptureStatusNone;
+}
+
+static int action_fused_small(Device* D, const uint64_t* rel_bits, long long N, int dim, double eps, int kmax,
+                              long long* counts, double* S, cudaStream_t stream) {
+    BitsetFusedWs*& ws = D->fused_ws[stream];
+    if (!ws) {
+        CSG_CUDA(cudaMalloc(&ws, sizeof(BitsetFusedWs)));
+        CSG_CUDA(cudaMemset(ws, 0, sizeof(BitsetFusedWs)));
+    }
+    const long long stride = csg_row_stride_words(N);
+    const long long nb = (N + BS_T - 1) / BS_T;
+    const long long ntiles = nb * (nb + 1) / 2;
+    const int grid = (int)std::max<long long>(1, std::min<long long>(ntiles, (long long)D->sm_count * 2));
+    const int slot = (int)(D->timed_calls % TIMING_RING);
+    if (g.timing) {
+        if (!D->ev0[slot]) {
+            CSG_CUDA(cudaEventCreate(&D->ev0[slot]));
+            CSG_CUDA(cudaEventCreate(&D->ev1[slot]));
+        }
+        CSG_CUDA(cudaEventRecord(D->ev0[slot], stream));
+    }
+    bitset_action_kernel<<<grid, BS_THREADS, 0, stream>>>(reinterpret_cast<const uint32_t*>(rel_bits), N, stride * 2, kmax,
+                                                           reinterpret_cast<unsigned long long*>(counts), nb, ntiles, 0, 1, 0,
+                                                           0, ws, dim, eps, S);
+    CSG_CUDA(cudaGetLastError());
+    ++g.launches;
+    if (g.timing) {
+        CSG_CUDA(cudaEventRecord(D->ev1[slot], stream));
+        ++D->timed_calls;
+    }
+    return CSG_OK;
+}
+
 static int action_device(Device* D, const uint64_t* rel_bits, long long N, int dim, double eps, int kmax,
                          long long* counts, double* S, cudaStream_t stream) {
+    if (fused_small_ok(N, kmax, stream)) return action_fused_small(D, rel_bits, N, dim, eps, kmax, counts, S, stream);
     int rc = interval_device(D, rel_bits, N, kmax, 0, 1, counts, stream);
     if (rc) return rc;
     return finish_device(counts, N, dim, eps, kmax, S, stream);
@@ -690,6 +686,7 @@ static void release_device(Device* D) {
     if (D->d_coords) cudaFree(D->d_coords);
     if (D->d_progress) cudaFree(D->d_progress);
     if (D->d_landed) cudaFree(D->d_landed);
+    for (auto& kv : D->fused_ws) cudaFree(kv.second);
     for (cudaEvent_t e : D->chunk_ev) cudaEventDestroy(e);
     if (D->copy_stream) cudaStreamDestroy(D->copy_stream);
     if (D->host_stream) cudaStreamDestroy(D->host_stream);
@@ -773,7 +770,7 @@ int csg_action_batch(const uint64_t* rel_bits, int64_t N, int64_t batch, int dim
         const dim3 grid((unsigned)std::min<long long>(ntiles, per_set), (unsigned)batch);
         bitset_action_kernel<<<grid, BS_THREADS, 0, stream>>>(reinterpret_cast<const uint32_t*>(rel_bits), N, stride * 2,
                                                                kmax, reinterpret_cast<unsigned long long*>(c), nb, ntiles,
-                                                               0, 1, set_words * 2, kmax + 1);
+                                                               0, 1, set_words * 2, kmax + 1, nullptr, 0, 1.0, nullptr);
         CSG_CUDA(cudaGetLastError());
         ++g.launches;
     } else {

@@ -505,6 +505,50 @@ def test_graph_survives_other_sizes(csg):
         assert float(S1.item()) == oracle.action_local(4, N1, want1)
 
 
+def test_fused_small_sets_on_streams_and_in_graphs(csg):
+    """N <= 1024 (bitset variant): eager calls take the fused single launch (one kernel per action, per-stream
+    workspace), captured calls the three-node path; both bit-exact, interleaved on two streams, local and smeared."""
+    csg.csg_set_variant(csg.VARIANT_AUTO)
+    cases = [(2, 1024, 1.0, 3), (4, 700, 1.0, 3), (2, 513, 0.1, 511), (2, 64, 1.0, 62), (2, 3, 1.0, 2)]
+    data = []
+    for dim, N, eps, kmax in cases:
+        _, bits = csg_inputs.make_causet(dim, N, 800 + N)
+        want = oracle.counts_from_bits(bits, N, kmax)
+        data.append((dim, N, eps, kmax, csg.to_device(bits), want))
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    torch.cuda.synchronize()
+    l0 = csg.csg_launch_count()
+    out = []
+    for rep in range(6):
+        for k, (dim, N, eps, kmax, d, want) in enumerate(data):
+            st = streams[(rep + k) % 2]
+            with torch.cuda.stream(st):
+                out.append((k, csg.csg_action(d, N, dim, eps, kmax, stream=st)))
+    torch.cuda.synchronize()
+    assert csg.csg_launch_count() - l0 == 6 * len(cases)              # ONE kernel per action
+    for k, (c, S) in out:
+        dim, N, eps, kmax, d, want = data[k]
+        assert (c.cpu().numpy() == want).all(), (N, eps)
+        if eps == 1.0:
+            assert float(S.item()) == oracle.action_local(dim, N, np.concatenate([want, np.zeros(4, np.int64)]))
+        else:
+            s_want, scale = oracle.action_smeared_2d(N, want, eps)
+            assert abs(float(S.item()) - s_want) <= 1e-12 * scale
+    # same S bits from the fused launch, the three-node path (inside a graph) and the batch call
+    dim, N, eps, kmax, d, want = data[2]
+    c_e, S_e = csg.csg_action(d, N, dim, eps, kmax)
+    c_g = torch.zeros(kmax + 1, dtype=torch.int64, device="cuda")
+    S_g = torch.zeros(1, dtype=torch.float64, device="cuda")
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        csg.csg_action(d, N, dim, eps, kmax, c_g, S_g)
+    graph.replay()
+    c_b, S_b = csg.csg_action_batch(d, N, 1, dim, eps, kmax)
+    torch.cuda.synchronize()
+    assert torch.equal(c_e, c_g) and torch.equal(c_e, c_b[0])
+    assert float(S_e.item()) == float(S_g.item()) == float(S_b[0].item())
+
+
 def test_measure_peak_runs(csg):
     for what in (csg.PEAK_MMA_MXF4, csg.PEAK_MMA_I8, csg.PEAK_ALU_MIX, csg.PEAK_ALU_POPC, csg.PEAK_ALU_LOP3):
         ms, units = csg.csg_measure_peak(what, 2000)
