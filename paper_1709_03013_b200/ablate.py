@@ -5,7 +5,7 @@
 The script builds and loads libcsg_ablate.so -- the library's sources compiled with -DCSG_ABLATE, which adds the
 ablation switches to the fp4 instantiation of tensor_action_kernel and exports csg_set_debug -- INSTEAD of libcsg.so
 (the product library has neither).  For every value of --debug it calls csg_set_debug (bits: 1 no MMA issue, 2 no expansion arithmetic, 4 no
-operand stores, 8 no epilogue work, 16 no fence before publishing a stage, 32 no packed-bit ring, 64 free-running
+operand stores, 8 no bucketing in the epilogue, 16 no fence before publishing a stage, 32 no packed-bit ring, 64 free-running
 producers, 128 no prefill before the epilogue, 256 no open-range masks; any non-zero value gives WRONG counts), and the
 CUDA-event time of the interval kernel (csg_last_kernel_ms) of four calls is printed.  Needs a B200.
 """
