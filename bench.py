@@ -50,14 +50,18 @@ def read_peaks():
     return dict(bf16=1590.0, bf16_sustained=1400.0, hbm=6650.0, source="fallback (B200_PROFILING.md)")
 
 
-def kernel_source_hash():
-    """sha256 over the CUDA sources: profiles/dram_traffic.json records the hash its captures were taken at."""
+KERNEL_SOURCES = {"tensor_action_kernel": ["tensor_kernel.cuh"], "bitset_action_kernel": ["bitset_kernel.cuh", "finish.cuh"],
+                  "link_kernel": ["link_kernel.cuh"]}
+
+
+def kernel_source_hash(kernel):
+    """sha256 (16 hex digits) over the source files of a kernel: profiles/dram_traffic.json records the hash its
+    capture was taken at, so a capture of older code is recognised as stale."""
     import hashlib
     h = hashlib.sha256()
     csrc = os.path.join(ROOT, "paper_1709_03013_b200", "csrc")
-    for name in sorted(os.listdir(csrc)):
-        if name.endswith((".cu", ".cuh")):
-            h.update(open(os.path.join(csrc, name), "rb").read())
+    for name in KERNEL_SOURCES[kernel.split("<")[0]]:
+        h.update(open(os.path.join(csrc, name), "rb").read())
     return h.hexdigest()[:16]
 
 
@@ -72,7 +76,7 @@ def read_traffic(kernel, workload_index):
         return None, "no capture committed for this kernel"
     if entry.get("config") != workload_index:
         return None, "the committed capture (%s) is of configs[%s], not of this workload" % (entry.get("capture"), entry.get("config"))
-    if entry.get("csrc_sha256_16") != kernel_source_hash():
+    if entry.get("csrc_sha256_16") != kernel_source_hash(kernel):
         return None, "stale: the kernel sources changed after the committed capture (%s)" % entry.get("capture")
     return entry["dram_bytes_per_launch"], "ncu --set full, %s" % entry.get("capture")
 
