@@ -81,6 +81,40 @@ def read_traffic(kernel, workload_index):
     return entry["dram_bytes_per_launch"], "ncu --set full, %s" % entry.get("capture")
 
 
+def library_gemm_context(torch):
+    """Plain library GEMMs of the same box, for context beside the roofline: int8 (torch._int_mm, cuBLASLt) and
+    fp8 e4m3 (torch._scaled_mm), 8192^3, best of 10 after 3 warm-ups, CUDA events.  The stack exposes no fp4 GEMM."""
+    out = {}
+    M = 8192
+
+    def best_tops(fn):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        best = float("inf")
+        for _ in range(10):
+            e0.record(); fn(); e1.record()
+            torch.cuda.synchronize()
+            best = min(best, e0.elapsed_time(e1))
+        return 2.0 * M ** 3 / (best * 1e-3) / 1e12
+    try:
+        a = torch.randint(-3, 3, (M, M), dtype=torch.int8, device="cuda")
+        b = torch.randint(-3, 3, (M, M), dtype=torch.int8, device="cuda").t()
+        out["int8_torch_int_mm_tops"] = best_tops(lambda: torch._int_mm(a, b))
+    except Exception as e:                                    # noqa: BLE001 -- context only
+        out["int8_torch_int_mm_tops"] = "unavailable: %s" % type(e).__name__
+    try:
+        a8 = torch.randn(M, M, device="cuda").to(torch.float8_e4m3fn)
+        b8 = torch.randn(M, M, device="cuda").to(torch.float8_e4m3fn).t()
+        one = torch.tensor(1.0, device="cuda")
+        out["fp8_torch_scaled_mm_tflops"] = best_tops(lambda: torch._scaled_mm(a8, b8, scale_a=one, scale_b=one, out_dtype=torch.bfloat16))
+    except Exception as e:                                    # noqa: BLE001
+        out["fp8_torch_scaled_mm_tflops"] = "unavailable: %s" % type(e).__name__
+    out["note"] = "library GEMMs 8192^3 (burst); no fp4 GEMM in this stack -- the peak above is the kernel's own instruction, bare"
+    return out
+
+
 def config_dict(cfg, N, dim, eps, kmax):
     """The `config` object of the JSON line: the same keys and values from both arms (ours / reference)."""
     stride = 4 * ((N + 255) // 256)
@@ -437,7 +471,8 @@ def run_ours(args, cfg, rank, local_rank, world):
                     "hw_rate": "%d MAC/clk/SM x 148 SMs x %.0f MHz (sampled) = %.0f TOP/s" % (16384 if fp4 else 8192, sm_clock_mhz, hw),
                     "frac_of_scaled_bf16": achieved / (ratio * peaks["bf16"]),
                     "scaled_bf16": "%g x bf16 %s = %.0f TOP/s (power-capped cuBLAS figure; context only)" % (ratio, peaks["source"], ratio * peaks["bf16"]),
-                    "kernel_ms": k_ms, "traffic": traffic, "traffic_source": traffic_src}
+                    "kernel_ms": k_ms, "traffic": traffic, "traffic_source": traffic_src,
+                    "library_gemm_context": library_gemm_context(torch)}
     else:
         # LOP3 AND + POPC + IADD per 32 triple tests: peak = measured issue rate of exactly that mix (csg_measure_peak)
         csg.csg_measure_peak(csg.PEAK_ALU_MIX, 2000)

@@ -536,7 +536,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive_cluster(tmem_empty_leader);
-            // Bucketing: one test per value.  Measured alternatives (config 3, ms per launch): this loop 89.65; a
+            // General bucketing (any kmax): one test per value.  Measured alternatives (config 3, ms per launch): this loop 89.65; a
             // branch-free pass that builds a 32-bit mask of passing values (compare + select + add) and then visits the
             // set bits eight at a time 91.80 -- per WARP nearly every group of columns holds a hit, so the second pass
             // branches as often; the same mask with the values copied to a local-memory scratch and a loop over the set
@@ -548,6 +548,38 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 if (n < TC_HIST) atomicAdd(&hist[n], 1u);
                 else atomicAdd(&counts[n], 1ULL);
             };
+            // Local action (kmax <= 3, every BASELINE.json config but the smeared one): no branch and no atomic per value.
+            // Each thread keeps the four bins in the four bytes of one register (it sees 64 values per tile, so a byte
+            // cannot overflow): the accumulator is turned into the shift amount 8 n with one FFMA and one AND (fp4: the
+            // low 23 bits of 4n * 2 + 2^23; int8: a shift), "1 << 8n" is a PTX shl, which clamps shift amounts above 31
+            // and so yields 0 for every n >= 4, and the relation bit predicates the add.  Five instructions per value in
+            // a straight line instead of a bit test, a compare and a BSSY/BRA/BSYNC triple with a divergent slow path;
+            // the four bytes are summed over the warp once per tile (4 REDUX + at most 4 shared-memory atomics per warp).
+            const bool byte_bins = !DUMP && kcap <= 3 && N <= (1LL << 20);
+            if (byte_bins) {
+                uint32_t packed = 0u;
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    if (dbg & 8) break;               // ablation: no bucketing (the accumulators are still read)
+                    const uint32_t rw = relw[e];
+                    if (rw == 0u) continue;           // no related pair among these 32 columns
+#pragma unroll
+                    for (int x = 0; x < 32; ++x) {
+                        const uint32_t v = e == 0 ? v0[x] : v1[x];
+                        const uint32_t sh = KIND == KIND_FP4
+                                                ? (__float_as_uint(fmaf(__uint_as_float(v), 2.0f, 8388608.0f)) & 0x7FFFFFu)
+                                                : (v >> (2 * TB - 3));
+                        uint32_t onehot;
+                        asm("shl.b32 %0, 1, %1;" : "=r"(onehot) : "r"(sh));      // 0 when 8 n > 31
+                        if (rw & (1u << x)) packed += onehot;
+                    }
+                }
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const unsigned int c = __reduce_add_sync(0xFFFFFFFFu, (packed >> (8 * k)) & 0xFFu);
+                    if (lane == 0 && c != 0u && k <= kcap) atomicAdd(&hist[k], c);
+                }
+            } else {
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
                 if (dbg & 8) break;                   // ablation: no bucketing (the accumulators are still read)
@@ -564,6 +596,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                         bucket(v);
                     }
                 }
+            }
             }
             // one count per finished tile of this cluster (throttle of the TMA threads, see below)
             if (progress != nullptr && rank == 0 && tid == 0) atomicAdd(progress, 1u);
