@@ -204,7 +204,7 @@ int csg_effective_variant(int64_t N);
 /*
  * Measurement / test aid like csg_set_variant: the drift throttle of the fp4 tensor kernel (clusters of the
  * persistent grid are kept within one round of each other so that concurrently running tiles share rows in L2).
- * CSG_THROTTLE_AUTO: on for matrices above 4 GiB only; _ON: on whenever a launch has more tiles than clusters;
+ * CSG_THROTTLE_AUTO: on for matrices above 1 GiB only; _ON: on whenever a launch has more tiles than clusters;
  * _OFF: never.  In every mode it is used only if the runtime reports that the whole grid can be resident at once,
  * and a wait that lasts longer than a few ms switches it off inside the kernel.  Results never depend on it.
  */

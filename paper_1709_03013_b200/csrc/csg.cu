@@ -350,13 +350,14 @@ static int launch_tensor(Device* D, int kind, const uint64_t* rel_bits, long lon
     rc = ensure_bits_map(D, kind, rel_bits, N, stride, &map);
     if (rc) return rc;
     const int grid = 2 * std::max(1, std::min(ntiles, D->sm_count / 2));   // one CTA pair per SM pair
-    // Drift throttle (tensor_kernel.cuh, TC_MAX_LEAD).  Measured: config 4 (N = 262144, full histogram) 1022 -> 929 ms,
-    // DRAM reads 2.55 -> 0.67 TB per launch, SM clock under the power cap 1.67 -> 1.86 GHz; config 3 (kmax = 3)
-    // 106.6 -> 107.5 ms, the de Sitter workload (N = 131072, full histogram) 109.9 -> 111.4 ms.  So CSG_THROTTLE_AUTO
-    // switches it on only for matrices of more than 4 GiB, where a cluster walks through thousands of rounds -- and
-    // only if the runtime says that the whole grid can be resident at once (the wait is bounded in the kernel, too).
+    // Drift throttle (tensor_kernel.cuh, TC_MAX_LEAD): fewer DRAM reads, so less power.  Measured (round 2 kernel):
+    // config 4 (N = 262144, 8 GiB, full histogram) 942 -> 847 ms; config 3 (N = 131072, 2 GiB), where the kernel now
+    // runs into the 1 kW power cap: a single launch 88.5 either way, twelve back to back 89.9 (drifting up to 92) ->
+    // 88.85 ms (steady); config 2 (512 MiB, no power cap) 12.02 -> 12.20 ms.  So CSG_THROTTLE_AUTO switches it on for
+    // matrices above 1 GiB -- and in every mode only if the runtime says that the whole grid can be resident at once
+    // (the wait is bounded in the kernel, too).
     unsigned int* progress = nullptr;
-    const bool big = N * stride * 8 > (4LL << 30) && ntiles > 16 * (grid / 2);
+    const bool big = N * stride * 8 > (1LL << 30) && ntiles > 16 * (grid / 2);
     const bool want = g.throttle == CSG_THROTTLE_ON ? ntiles > grid / 2 : (g.throttle == CSG_THROTTLE_AUTO && big);
     if (kind == KIND_FP4 && dump == nullptr && want && D->wait_clusters >= grid / 2) {
         // a ring of counters, one per launch, so that launches in flight on different streams do not share one
