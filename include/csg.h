@@ -149,6 +149,17 @@ int csg_action_host(const uint64_t *rel_bits_host, int64_t N, int dim, double ep
                     int64_t *counts_host, double *S_host);
 
 /*
+ * How csg_action_host overlaps the copy of a large matrix with the kernel.  CSG_HOST_PIPELINE_AUTO: the gated single
+ * launch described above when the driver offers stream memory operations (fp4 kind), else chunked launches;
+ * _CHUNKED: always one launch per copy step behind an event.  The gated launch WAITS inside the kernel for the copy
+ * stream, so it needs copies and kernels to run concurrently: under a tool that serialises the GPU's work (Nsight
+ * Compute replays one kernel at a time and holds every other stream) it cannot make progress -- select _CHUNKED for
+ * such runs (bench.py --host-pipeline chunked).  Results never depend on the mode.
+ */
+enum { CSG_HOST_PIPELINE_AUTO = 0, CSG_HOST_PIPELINE_CHUNKED = 1 };
+int csg_set_host_pipeline(int mode);
+
+/*
  * Linking (Sec. 2.2: "pairwise relations are found by identifying pairs of elements which are
  * timelike separated"; dense, symmetric, topologically sorted adjacency matrix): builds the relation matrix
  * that csg_action reads from the coordinates of the elements.
@@ -210,6 +221,27 @@ int csg_effective_variant(int64_t N);
  */
 enum { CSG_THROTTLE_AUTO = 0, CSG_THROTTLE_ON = 1, CSG_THROTTLE_OFF = 2 };
 int csg_set_throttle(int mode);
+
+/*
+ * Block-sparse K sweep of the fp4 tensor kernel.  The paper's pair loop skips unrelated pairs (Algorithm 5
+ * l.4-5), so its run time depends on the ordering fraction.  A tensor-core tile cannot skip single
+ * pairs, but the stage of tile (I, J) that sweeps column block K multiplies the 256 x 256 block (I, K) of the matrix
+ * with block (J, K) and contributes nothing when either is empty -- and in a time-sorted 3+1 sprinkling the blocks
+ * next to the diagonal are (elements close in time are almost never timelike separated).  One pass over the matrix
+ * marks the empty blocks (csg_block_occupancy) and the kernel skips the dead two-stage groups; results never depend
+ * on it.  CSG_SPARSE_AUTO: matrices of 512 MiB and more (device-resident calls only: csg_action_host streams the
+ * matrix while the kernel runs and stays dense); _ON: every fp4 launch (test aid); _OFF: never.
+ */
+enum { CSG_SPARSE_AUTO = 0, CSG_SPARSE_ON = 1, CSG_SPARSE_OFF = 2 };
+int csg_set_sparse(int mode);
+/*
+ * The occupancy pass on its own (test hook and measurement aid).  occ DEVICE, ceil(N/256) rows of
+ * csg_occupancy_stride_words(N) 32-bit words, every word overwritten: bit (K % 32) of word K / 32 of row I is set iff
+ * some bit of rows 256 I .. 256 I + 255, columns 256 K .. 256 K + 255 of the matrix is set; words beyond the last
+ * column block are zero.  rel_bits as in csg_action.  Enqueued on `stream`, no host synchronisation.
+ */
+int64_t csg_occupancy_stride_words(int64_t N);
+int csg_block_occupancy(const uint64_t *rel_bits, int64_t N, uint32_t *occ, cudaStream_t stream);
 
 /*
  * Measurement aid: the roofline denominators measured on the current device.  Runs a bare kernel (no producers, no

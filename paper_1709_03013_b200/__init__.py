@@ -7,8 +7,8 @@ There is no CPU fallback: if libcsg.so is missing, importing the compute entry p
 Functions carry the C names: csg_action, csg_action_host, csg_interval_sizes, csg_row_stride_words,
 csg_set_variant, csg_effective_variant, csg_set_kernel_timing, csg_last_kernel_ms, csg_kernel_ms_history,
 csg_launch_count, csg_action_partial, csg_action_finish, csg_tile_schedule, csg_link, csg_causet_action_host,
-csg_last_link_ms, csg_action_batch, csg_tile_interval_sizes, csg_set_throttle, csg_measure_peak, csg_strerror,
-csg_shutdown.
+csg_last_link_ms, csg_action_batch, csg_tile_interval_sizes, csg_set_throttle, csg_set_sparse, csg_set_host_pipeline,
+csg_occupancy_stride_words, csg_block_occupancy, csg_measure_peak, csg_strerror, csg_shutdown.
 """
 import ctypes
 import os
@@ -20,6 +20,8 @@ from . import _build
 VARIANT_AUTO, VARIANT_BITSET, VARIANT_TENSOR, VARIANT_TENSOR_FP4 = 0, 1, 2, 3
 GEOM_MINKOWSKI_2D, GEOM_MINKOWSKI_4D, GEOM_DESITTER_2D = 0, 1, 2
 THROTTLE_AUTO, THROTTLE_ON, THROTTLE_OFF = 0, 1, 2
+SPARSE_AUTO, SPARSE_ON, SPARSE_OFF = 0, 1, 2
+HOST_PIPELINE_AUTO, HOST_PIPELINE_CHUNKED = 0, 1
 PEAK_MMA_MXF4, PEAK_MMA_I8, PEAK_ALU_MIX, PEAK_ALU_POPC, PEAK_ALU_LOP3 = 0, 1, 2, 3, 4
 LIB_PATH = _build.LIB_PATH
 
@@ -28,7 +30,8 @@ EXPORTS = [
     "csg_effective_variant", "csg_set_kernel_timing", "csg_last_kernel_ms", "csg_kernel_ms_history",
     "csg_launch_count", "csg_action_partial", "csg_action_finish", "csg_tile_schedule", "csg_link",
     "csg_causet_action_host", "csg_last_link_ms", "csg_action_batch", "csg_tile_interval_sizes", "csg_set_throttle",
-    "csg_measure_peak",
+    "csg_measure_peak", "csg_set_sparse", "csg_occupancy_stride_words", "csg_block_occupancy",
+    "csg_set_host_pipeline",
     "csg_strerror", "csg_shutdown",
 ]
 
@@ -82,6 +85,14 @@ def load():
     lib.csg_tile_interval_sizes.restype = ci
     lib.csg_set_throttle.argtypes = [ci]
     lib.csg_set_throttle.restype = ci
+    lib.csg_set_sparse.argtypes = [ci]
+    lib.csg_set_sparse.restype = ci
+    lib.csg_set_host_pipeline.argtypes = [ci]
+    lib.csg_set_host_pipeline.restype = ci
+    lib.csg_occupancy_stride_words.argtypes = [i64]
+    lib.csg_occupancy_stride_words.restype = i64
+    lib.csg_block_occupancy.argtypes = [vp, i64, vp, vp]
+    lib.csg_block_occupancy.restype = ci
     lib.csg_measure_peak.argtypes = [ci, ci, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_double)]
     lib.csg_measure_peak.restype = ci
     lib.csg_set_variant.argtypes = [ci]
@@ -297,6 +308,29 @@ def csg_tile_interval_sizes(rel_bits, N, tiles_ij, n_out=None, stream=None):
 
 def csg_set_throttle(mode):
     _check(load().csg_set_throttle(int(mode)))
+
+
+def csg_set_sparse(mode):
+    _check(load().csg_set_sparse(int(mode)))
+
+
+def csg_set_host_pipeline(mode):
+    _check(load().csg_set_host_pipeline(int(mode)))
+
+
+def csg_occupancy_stride_words(N):
+    return int(load().csg_occupancy_stride_words(int(N)))
+
+
+def csg_block_occupancy(rel_bits, N, occ=None, stream=None):
+    """int csg_block_occupancy(rel_bits, N, occ, stream): occ = int32 CUDA tensor (ceil(N/256), stride) of bit words."""
+    import torch
+    assert rel_bits.is_cuda and rel_bits.element_size() == 8 and rel_bits.is_contiguous()
+    if occ is None:
+        occ = torch.empty(((int(N) + 255) // 256, csg_occupancy_stride_words(N)), dtype=torch.int32, device=rel_bits.device)
+    assert occ.is_cuda and occ.dtype == torch.int32 and occ.is_contiguous()
+    _check(load().csg_block_occupancy(rel_bits.data_ptr(), int(N), occ.data_ptr(), _stream_handle(stream)))
+    return occ
 
 
 def csg_measure_peak(what, iters):

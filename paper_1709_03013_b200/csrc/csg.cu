@@ -17,6 +17,7 @@
 #include "finish.cuh"
 #include "bitset_kernel.cuh"
 #include "link_kernel.cuh"
+#include "occupancy_kernel.cuh"
 #include "tensor_kernel.cuh"
 #include "peak_kernels.cuh"
 
@@ -42,6 +43,7 @@ finish_action_kernel(const long long* __restrict__ counts, long long N, int dim,
 constexpr int TIMING_RING = 64;
 constexpr int PROGRESS_RING = 64;
 constexpr int MAX_DEVICES = 64;
+constexpr int OCC_RING = 16;
 
 struct TileList {                       // tile schedule of one (N, shard, nshards) on the device
     long long N;
@@ -79,6 +81,12 @@ struct Device {
     unsigned int* d_progress = nullptr; // PROGRESS_RING finished-tile counters, one per launch in flight (drift throttle)
     std::map<cudaStream_t, BitsetFusedWs*> fused_ws;   // fused small-N launch: one zeroed workspace per stream
     unsigned int* d_landed = nullptr;   // chunks of the host matrix delivered so far (gate of csg_action_host)
+    // block-occupancy bitmaps (occupancy_kernel.cuh), one per launch in flight; a slot that is too small for a later N is
+    // replaced and the old buffer kept until csg_shutdown (a launch or a captured graph may still read it)
+    uint32_t* d_occ[OCC_RING] = {};
+    size_t d_occ_words[OCC_RING] = {};
+    std::vector<uint32_t*> occ_retired;
+    long long occ_next = 0;
     // end-to-end (host buffer) path
     cudaStream_t host_stream = nullptr, copy_stream = nullptr;
     uint64_t* d_bits = nullptr;
@@ -98,6 +106,8 @@ struct Global {
     std::mutex mu;
     int variant = CSG_VARIANT_AUTO;
     int throttle = CSG_THROTTLE_AUTO;
+    int sparse = CSG_SPARSE_AUTO;
+    int host_pipeline = CSG_HOST_PIPELINE_AUTO;
     bool timing = false;
     int debug = 0;                      // ablation bits; only the -DCSG_ABLATE build can set it
     long long launches = 0;
@@ -343,7 +353,7 @@ static int ensure_tensor_ready(Device* D) {
 // the host-matrix path (NULL when the matrix is resident); dump: csg_tile_interval_sizes (NULL otherwise).
 static int launch_tensor(Device* D, int kind, const uint64_t* rel_bits, long long N, long long stride, int kmax,
                          long long* counts, const int2* d_tiles, int ntiles, const unsigned int* landed,
-                         const int* tile_need, int* dump, cudaStream_t stream) {
+                         const int* tile_need, int* dump, const uint32_t* occ, cudaStream_t stream) {
     int rc = ensure_tensor_ready(D);
     if (rc) return rc;
     const CUtensorMap* map = nullptr;
@@ -368,7 +378,7 @@ static int launch_tensor(Device* D, int kind, const uint64_t* rel_bits, long lon
     unsigned long long* c64 = reinterpret_cast<unsigned long long*>(counts);
     const int s8 = TcTraits<KIND_I8>::SMEM_BYTES, s4 = TcTraits<KIND_FP4>::SMEM_BYTES;
 #define CSG_LAUNCH(KERNEL, SMEM) \
-    KERNEL<<<grid, TC_THREADS, SMEM, stream>>>(*map, rel_bits, N, stride, kmax, c64, d_tiles, ntiles, g.debug, progress, landed, tile_need, dump)
+    KERNEL<<<grid, TC_THREADS, SMEM, stream>>>(*map, rel_bits, N, stride, kmax, c64, d_tiles, ntiles, g.debug, progress, landed, tile_need, dump, occ, occ_stride_words(N))
     // int8: operand bit TB: the accumulator holds n_ij << 2TB and n_ij <= N-2, so TB is the largest with
     // (N-2) << 2TB < 2^31; TB = 7 turns every unpack shift into a left shift (FMA pipe).
     const int tb = N - 2 < (1LL << 17) ? 7 : N - 2 < (1LL << 19) ? 6 : N - 2 < (1LL << 21) ? 5 : 4;
@@ -390,6 +400,36 @@ static int launch_tensor(Device* D, int kind, const uint64_t* rel_bits, long lon
 #undef CSG_LAUNCH
     CSG_CUDA(cudaGetLastError());
     ++g.launches;
+    return CSG_OK;
+}
+
+// Block-sparse K sweep of the fp4 tensor kernel (occupancy_kernel.cuh): one pass over the matrix marks the empty
+// 256 x 256 blocks, and the kernel skips every two-stage group whose U or L block is empty.  Measured at config 3 (4D,
+// N = 131072): 10.8 % of the groups are dead.  AUTO: matrices of 512 MiB and more (the pass costs one HBM read of the
+// matrix, 0.4 % of the action there; a 1+1 set has no empty block and only pays that); ON: every fp4 launch (tests).
+// *occ = nullptr when the sweep stays dense.
+constexpr long long SPARSE_MIN_BYTES = 512LL << 20;
+
+static int occupancy_pass(Device* D, int kind, const uint64_t* rel_bits, long long N, long long stride,
+                          const uint32_t** occ, cudaStream_t stream) {
+    *occ = nullptr;
+    if (kind != KIND_FP4 || g.sparse == CSG_SPARSE_OFF) return CSG_OK;
+    if (g.sparse == CSG_SPARSE_AUTO && N * stride * 8 < SPARSE_MIN_BYTES) return CSG_OK;
+    const int nB = (int)((N + TC_T - 1) / TC_T);
+    const int ostride = occ_stride_words(N);
+    const size_t words = (size_t)nB * ostride;
+    const int slot = (int)(D->occ_next++ % OCC_RING);
+    if (D->d_occ_words[slot] < words) {
+        if (D->d_occ[slot]) D->occ_retired.push_back(D->d_occ[slot]);
+        D->d_occ[slot] = nullptr;
+        D->d_occ_words[slot] = 0;
+        CSG_CUDA(cudaMalloc(&D->d_occ[slot], words * sizeof(uint32_t)));
+        D->d_occ_words[slot] = words;
+    }
+    occupancy_kernel<<<dim3(ostride / 4, nB), OCC_THREADS, 0, stream>>>(rel_bits, N, stride, D->d_occ[slot], ostride);
+    CSG_CUDA(cudaGetLastError());
+    ++g.launches;
+    *occ = D->d_occ[slot];
     return CSG_OK;
 }
 
@@ -416,7 +456,9 @@ static int interval_device(Device* D, const uint64_t* rel_bits, long long N, int
         CSG_CUDA(cudaEventRecord(D->ev0[slot], stream));
     }
     if (tensor) {
-        rc = launch_tensor(D, kind, rel_bits, N, stride, kmax, counts, tl->d, tl->n, nullptr, nullptr, nullptr, stream);
+        const uint32_t* occ = nullptr;
+        if ((rc = occupancy_pass(D, kind, rel_bits, N, stride, &occ, stream))) return rc;
+        rc = launch_tensor(D, kind, rel_bits, N, stride, kmax, counts, tl->d, tl->n, nullptr, nullptr, nullptr, occ, stream);
         if (rc) return rc;
     } else {
         const long long nb = (N + BS_T - 1) / BS_T;
@@ -597,7 +639,7 @@ static int interval_host_pipelined(Device* D, const uint64_t* rel_bits_host, uin
     // the copies must not overtake work of an earlier call that still reads d_bits on `stream`
     CSG_CUDA(cudaEventRecord(ev_prev, stream));
     CSG_CUDA(cudaStreamWaitEvent(D->copy_stream, ev_prev, 0));
-    WriteValue32Fn write32 = kind == KIND_FP4 ? stream_write_value32() : nullptr;
+    WriteValue32Fn write32 = kind == KIND_FP4 && g.host_pipeline != CSG_HOST_PIPELINE_CHUNKED ? stream_write_value32() : nullptr;
     if (write32) {
         if (!D->d_landed) CSG_CUDA(cudaMalloc(&D->d_landed, sizeof(unsigned int)));
         // reset the gate, then ONE launch that starts at once and follows the copies
@@ -606,7 +648,7 @@ static int interval_host_pipelined(Device* D, const uint64_t* rel_bits_host, uin
         } else {
             CSG_CUDA(cudaEventRecord(ev_reset, D->copy_stream));
             CSG_CUDA(cudaStreamWaitEvent(stream, ev_reset, 0));
-            rc = launch_tensor(D, kind, d_bits, N, stride, kmax, counts, ct->d, ct->n, D->d_landed, ct->d_need, nullptr, stream);
+            rc = launch_tensor(D, kind, d_bits, N, stride, kmax, counts, ct->d, ct->n, D->d_landed, ct->d_need, nullptr, nullptr, stream);
             if (rc) return rc;
         }
     }
@@ -624,7 +666,7 @@ static int interval_host_pipelined(Device* D, const uint64_t* rel_bits_host, uin
             CSG_CUDA(cudaStreamWaitEvent(stream, D->chunk_ev[c], 0));
             const int nt = ct->off[c + 1] - ct->off[c];
             if (nt > 0) {
-                rc = launch_tensor(D, kind, d_bits, N, stride, kmax, counts, ct->d + ct->off[c], nt, nullptr, nullptr, nullptr, stream);
+                rc = launch_tensor(D, kind, d_bits, N, stride, kmax, counts, ct->d + ct->off[c], nt, nullptr, nullptr, nullptr, nullptr, stream);
                 if (rc) return rc;
             }
         }
@@ -687,6 +729,8 @@ static void release_device(Device* D) {
     if (D->d_coords) cudaFree(D->d_coords);
     if (D->d_progress) cudaFree(D->d_progress);
     if (D->d_landed) cudaFree(D->d_landed);
+    for (uint32_t* p : D->d_occ) if (p) cudaFree(p);
+    for (uint32_t* p : D->occ_retired) cudaFree(p);
     for (auto& kv : D->fused_ws) cudaFree(kv.second);
     for (cudaEvent_t e : D->chunk_ev) cudaEventDestroy(e);
     if (D->copy_stream) cudaStreamDestroy(D->copy_stream);
@@ -930,8 +974,12 @@ int csg_tile_interval_sizes(const uint64_t* rel_bits, int64_t N, const int32_t* 
     CSG_CUDA(cudaMalloc(&d_tiles, (size_t)ntiles * sizeof(int2)));
     cudaError_t e = cudaMemcpy(d_tiles, tiles_ij_host, (size_t)ntiles * sizeof(int2), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) {
-        rc = launch_tensor(D, variant == CSG_VARIANT_TENSOR_FP4 ? KIND_FP4 : KIND_I8, rel_bits, N, csg_row_stride_words(N),
-                           0, nullptr, d_tiles, (int)ntiles, nullptr, nullptr, n_out, stream);
+        const int kind = variant == CSG_VARIANT_TENSOR_FP4 ? KIND_FP4 : KIND_I8;
+        const uint32_t* occ = nullptr;
+        rc = occupancy_pass(D, kind, rel_bits, N, csg_row_stride_words(N), &occ, stream);
+        if (rc == CSG_OK)
+            rc = launch_tensor(D, kind, rel_bits, N, csg_row_stride_words(N), 0, nullptr, d_tiles, (int)ntiles, nullptr, nullptr,
+                               n_out, occ, stream);
         e = cudaStreamSynchronize(stream);
     }
     cudaFree(d_tiles);
@@ -956,6 +1004,37 @@ int csg_set_throttle(int mode) {
     std::lock_guard<std::mutex> lock(g.mu);
     if (mode < CSG_THROTTLE_AUTO || mode > CSG_THROTTLE_OFF) return CSG_E_VARIANT;
     g.throttle = mode;
+    return CSG_OK;
+}
+
+int csg_set_sparse(int mode) {
+    std::lock_guard<std::mutex> lock(g.mu);
+    if (mode < CSG_SPARSE_AUTO || mode > CSG_SPARSE_OFF) return CSG_E_VARIANT;
+    g.sparse = mode;
+    return CSG_OK;
+}
+
+int csg_set_host_pipeline(int mode) {
+    std::lock_guard<std::mutex> lock(g.mu);
+    if (mode < CSG_HOST_PIPELINE_AUTO || mode > CSG_HOST_PIPELINE_CHUNKED) return CSG_E_VARIANT;
+    g.host_pipeline = mode;
+    return CSG_OK;
+}
+
+int64_t csg_occupancy_stride_words(int64_t N) { return N < 1 ? 0 : occ_stride_words(N); }
+
+int csg_block_occupancy(const uint64_t* rel_bits, int64_t N, uint32_t* occ, cudaStream_t stream) {
+    std::lock_guard<std::mutex> lock(g.mu);
+    if (!rel_bits || !occ) return CSG_E_NULL;
+    if (N < 1 || N > CSG_MAX_N) return CSG_E_SIZE;
+    if ((reinterpret_cast<uintptr_t>(rel_bits) & 15) || (reinterpret_cast<uintptr_t>(occ) & 3)) return CSG_E_ALIGN;
+    Device* D = nullptr;
+    int rc = current_device(&D);
+    if (rc) return rc;
+    const int nB = (int)((N + TC_T - 1) / TC_T), ostride = occ_stride_words(N);
+    occupancy_kernel<<<dim3(ostride / 4, nB), OCC_THREADS, 0, stream>>>(rel_bits, N, csg_row_stride_words(N), occ, ostride);
+    CSG_CUDA(cudaGetLastError());
+    ++g.launches;
     return CSG_OK;
 }
 

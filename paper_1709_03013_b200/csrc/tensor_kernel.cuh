@@ -387,6 +387,52 @@ __device__ __forceinline__ void tile_k_range(int I, int J, int& kb_begin, int& k
     }
 }
 
+// Live groups of a tile (block-sparse K sweep).  A group = TC_GROUP = 2 consecutive stages, the unit of one packed-bit
+// copy and of a producer set's turn.  occ = block occupancy of the relation matrix (occupancy_kernel.cuh; fp4 kind,
+// 256-column stages, so stage kb of the sweep IS column block kb): stage kb of tile (I, J) multiplies block (I, kb) of
+// U with block (J, kb) of L and is dead when either block is empty; a group is live when one of its two stages is.
+// Returns the live mask of groups 32 gw .. 32 gw + 31 of the tile (group g = stages kb_begin + 2g, + 2g + 1).  With
+// occ == nullptr every group of the range is live (the dense sweep).  All three roles of the kernel (TMA thread,
+// producers, MMA thread) walk the same masks, so they agree on the sequence of groups without talking to each other.
+__device__ __forceinline__ uint32_t live_groups_word(const uint32_t* __restrict__ occI, const uint32_t* __restrict__ occJ,
+                                                     int kb_begin, int kb_end, int gw) {
+    const int rem = ((kb_end - kb_begin) >> 1) - 32 * gw;          // groups left from this word on
+    const uint32_t in_range = rem >= 32 ? 0xFFFFFFFFu : ((1u << rem) - 1u);
+    if (occI == nullptr) return in_range;
+    const int s = kb_begin + 64 * gw;                              // first stage of the word
+    const int w = s >> 5, sh = s & 31;
+    const uint32_t a0 = __ldg(occI + w) & __ldg(occJ + w), a1 = __ldg(occI + w + 1) & __ldg(occJ + w + 1),
+                   a2 = __ldg(occI + w + 2) & __ldg(occJ + w + 2);  // rows are padded with zero words (OCC_PAD_WORDS)
+    uint64_t S = ((uint64_t)__funnelshift_r(a1, a2, sh) << 32) | __funnelshift_r(a0, a1, sh);   // stages s .. s + 63
+    S = (S | (S >> 1)) & 0x5555555555555555ull;                    // bit 2g: group g has a live stage
+    S = (S | (S >> 1)) & 0x3333333333333333ull;                    // compress the even bits
+    S = (S | (S >> 2)) & 0x0F0F0F0F0F0F0F0Full;
+    S = (S | (S >> 4)) & 0x00FF00FF00FF00FFull;
+    S = (S | (S >> 8)) & 0x0000FFFF0000FFFFull;
+    S = (S | (S >> 16)) & 0x00000000FFFFFFFFull;
+    return (uint32_t)S & in_range;
+}
+// Calls body(kb0) for the first stage kb0 of every live group of the tile, in ascending order; a tile without any
+// live group still gets its first group (the MMA of a tile's first stage is what zeroes the accumulators).
+template <class F>
+__device__ __forceinline__ void for_live_groups(const uint32_t* __restrict__ occ, int occ_stride, int I, int J,
+                                                int kb_begin, int kb_end, F&& body) {
+    const uint32_t* occI = occ ? occ + (size_t)I * occ_stride : nullptr;
+    const uint32_t* occJ = occ ? occ + (size_t)J * occ_stride : nullptr;
+    const int nwords = (((kb_end - kb_begin) >> 1) + 31) >> 5;
+    int done = 0;
+    for (int gw = 0; gw <= nwords; ++gw) {
+        uint32_t m = gw < nwords ? live_groups_word(occI, occJ, kb_begin, kb_end, gw) : (done == 0 ? 1u : 0u);
+        const int base = gw < nwords ? kb_begin + 64 * gw : kb_begin;
+        while (m) {
+            const int g = __ffs((int)m) - 1;
+            m &= m - 1;
+            ++done;
+            body(base + 2 * g);
+        }
+    }
+}
+
 // KIND_I8: TB = bit of the operand byte that carries the relation bit: operands are 0 or 2^TB, every product is
 // 4^TB, the accumulator holds n_ij << 2TB; the host picks the largest TB with (N-2) << 2TB < 2^31 (exact in s32).
 // KIND_FP4: TB unused (pass 0); the f32 accumulator holds 4 n_ij, exact for n_ij < 2^22.
@@ -400,10 +446,11 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                      long long stride_words, int kmax, unsigned long long* __restrict__ counts,
                      const int2* __restrict__ tiles, int ntiles, int dbg_arg, unsigned int* __restrict__ progress_arg,
                      const unsigned int* __restrict__ landed_arg, const int* __restrict__ tile_need,
-                     int* __restrict__ dump) {
+                     int* __restrict__ dump, const uint32_t* __restrict__ occ_arg, int occ_stride) {
     constexpr bool ABLATE = (FLAGS & TCF_ABLATE) != 0, WAITS = (FLAGS & TCF_WAIT) != 0, DUMP = (FLAGS & TCF_DUMP) != 0;
     unsigned int* const progress = WAITS ? progress_arg : nullptr;      // compiled out of the instantiations that never wait
     const unsigned int* const landed = WAITS ? landed_arg : nullptr;
+    const uint32_t* const occ = KIND == KIND_FP4 ? occ_arg : nullptr;   // block-sparse sweep: fp4 kind only (stage = column block)
     using T = TcTraits<KIND>;
     const int dbg = ABLATE ? dbg_arg : 0;             // compiled out of every instantiation of libcsg.so
     constexpr int COLS = T::STAGE_COLS, WORDS = T::WORDS;
@@ -624,7 +671,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 epilogue(epi_I, epi_J, epi_t);
                 epi_I = -1;
             }
-            const int epi_at = kb_begin + TC_GROUP * (min(prefill, (kb_end - kb_begin) / TC_GROUP) - 1);
+            int gdone = 0;                            // live groups of this tile expanded so far
             // One stage of one row: open-range mask, expansion, publish of this warp's previous stage, store.
             auto do_stage = [&](int kb, uint32_t stage, uint32_t eparity, uint32_t (&w)[WORDS]) {
                 if (dbg & 256) {                              // ablation: no open-range masks
@@ -670,7 +717,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 }
                 pending = (int)stage;
             };
-            for (int kb0 = kb_begin; kb0 < kb_end; kb0 += TC_GROUP) {
+            for_live_groups(occ, occ_stride, I, J, kb_begin, kb_end, [&](int kb0) {
                 // The packed-bit buffer is released only after the operand stores that consume every word loaded from
                 // it: the hardware has then issued them after the LDS data arrived.  An arrive placed right after the
                 // LDS instructions is NOT ordered after their completion (naming the loaded registers as unused asm
@@ -740,11 +787,15 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                     __syncwarp();
                     if (bits_release != 0 && lane == 0) mbar_arrive(bits_release);
                 }
-                if (epi_I >= 0 && kb0 == epi_at) {             // the previous tile's epilogue, after the prefill
+                if (epi_I >= 0 && ++gdone == prefill) {        // the previous tile's epilogue, after the prefill
                     publish_pending();
                     epilogue(epi_I, epi_J, epi_t);
                     epi_I = -1;
                 }
+            });
+            if (epi_I >= 0) {                                  // this tile had fewer live groups than the prefill
+                publish_pending();
+                epilogue(epi_I, epi_J, epi_t);
             }
             epi_I = I;
             epi_J = J;
@@ -777,7 +828,9 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 }
                 tc_fence_after();
                 uint32_t fresh = 1;                         // the tile's first MMA overwrites the accumulators
-                for (int kb = kb_begin; kb < kb_end; ++kb) {
+                for_live_groups(occ, occ_stride, tile.x, tile.y, kb_begin, kb_end, [&](int) {
+#pragma unroll 1
+                for (int half = 0; half < TC_GROUP; ++half) {
                     mbar_wait(full0 + 8 * stage, sphase);
                     tc_fence_after();
                     if (issuer) {
@@ -797,11 +850,12 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                                 umma_i8_2cta(tmem_base, adesc + 2 * kk, bdesc + 2 * kk, TC_IDESC, acc);
                         }
                         umma_commit_2cta(empty0 + 8 * stage);
-                        if (kb == kb_end - 1) umma_commit_2cta(tmem_full);
                     }
                     fresh = 0;
                     if (++stage == T::STAGES) { stage = 0; sphase ^= 1; }
                 }
+                });
+                if (issuer) umma_commit_2cta(tmem_full);     // arrives when every MMA of the tile has completed
                 ++done_tiles;
             }
         }
@@ -853,7 +907,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                         asm volatile("fence.proxy.async.global;" ::: "memory");   // the bytes are read by the async proxy (TMA)
                     }
                 }
-                for (int kb0 = kb_begin; kb0 < ((dbg & 32) ? kb_begin : kb_end); kb0 += TC_GROUP) {
+                if (!(dbg & 32)) for_live_groups(occ, occ_stride, tile.x, tile.y, kb_begin, kb_end, [&](int kb0) {
                     mbar_wait(bits_empty0 + 8 * bb, bphase ^ 1);
                     const uint32_t bar = bits_full0 + 8 * bb;
                     const uint32_t dst = smem0 + T::OFF_BITS + bb * T::BITS_BUF_BYTES;
@@ -861,7 +915,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                     tma_load_2d(dst, &bits_map, kb0 * (COLS / 8), ia, bar);
                     tma_load_2d(dst + T::BITS_BOX_BYTES, &bits_map, kb0 * (COLS / 8), jb, bar);
                     if (++bb == T::BITS_BUFS) { bb = 0; bphase ^= 1; }
-                }
+                });
             }
         }
     }
