@@ -519,7 +519,7 @@ def run_ours(args, cfg, rank, local_rank, world):
                     "kernel_ms": k_ms, "traffic": traffic, "traffic_source": traffic_src}
     if variant == csg.VARIANT_TENSOR_FP4:
         # block-sparse sweep (csg_set_sparse, AUTO: matrices of 512 MiB and more): what the tensor cores really executed
-        sparse_on = N * csg.csg_row_stride_words(N) * 8 >= (512 << 20)
+        sparse_on = N * csg.csg_row_stride_words(N) * 8 >= (512 << 20) and (dim != 2 or tiles_mode)   # CSG_SPARSE_AUTO
         frac_exec = 1.0
         if sparse_on:
             occ = csg.csg_block_occupancy(d_bits, N)
@@ -527,10 +527,11 @@ def run_ours(args, cfg, rank, local_rank, world):
             frac_exec = executed_group_fraction(occ.cpu().numpy(), N)
         roofline["executed_fraction"] = frac_exec
         roofline["frac_executed"] = roofline["frac"] * frac_exec
-        roofline["executed_note"] = ("block-sparse K sweep: the kernel skips two-stage groups whose U or L block is empty "
-                                     "(occupancy pass inside the timed kernel span); `achieved`/`frac` count all C(N,3) "
-                                     "algorithmic tests, `frac_executed` = frac x executed_fraction is the tensor cores' own "
-                                     "utilisation against the same measured peak")
+        roofline["executed_note"] = ("block-sparse K sweep (occupancy pass inside the timed kernel span): two-stage groups whose "
+                                     "U or L blocks are empty are neither fetched, expanded nor multiplied; executed_fraction "
+                                     "of the dense sweep's groups remains; `achieved`/`frac` count all C(N,3) algorithmic "
+                                     "tests, `frac_executed` = frac x executed_fraction is the tensor cores' own utilisation "
+                                     "against the same measured peak")
     roofline["hbm_gbs_algorithmic"] = (N * csg.csg_row_stride_words(N) * 8) / (k_ms * 1e-3) / 1e9
     # what the paper's method would execute of these tests (it skips unrelated pairs, PAPER.md:407 l.4-5)
     roofline["useful_work_ratio"] = useful_work_ratio(bits, N)

@@ -228,9 +228,11 @@ int csg_set_throttle(int mode);
  * pairs, but the stage of tile (I, J) that sweeps column block K multiplies the 256 x 256 block (I, K) of the matrix
  * with block (J, K) and contributes nothing when either is empty -- and in a time-sorted 3+1 sprinkling the blocks
  * next to the diagonal are (elements close in time are almost never timelike separated).  One pass over the matrix
- * marks the empty blocks (csg_block_occupancy) and the kernel skips the dead two-stage groups; results never depend
- * on it.  CSG_SPARSE_AUTO: matrices of 512 MiB and more (device-resident calls only: csg_action_host streams the
- * matrix while the kernel runs and stays dense); _ON: every fp4 launch (test aid); _OFF: never.
+ * marks the empty blocks (csg_block_occupancy) and the kernel neither fetches, expands nor multiplies the two-stage
+ * groups (2 x 256 columns) in which both stages are dead; results never depend on it.
+ * CSG_SPARSE_AUTO: matrices of 512 MiB and more, unless the call says dim = 2 (a 1+1 order, flat or de Sitter, has
+ * no empty block, and the pass and the mask loop would cost 2 %; csg_action_partial has no dim and uses the sweep);
+ * _ON: every fp4 launch (test aid); _OFF: never.  csg_action_host marks the blocks of every chunk as it lands.
  */
 enum { CSG_SPARSE_AUTO = 0, CSG_SPARSE_ON = 1, CSG_SPARSE_OFF = 2 };
 int csg_set_sparse(int mode);

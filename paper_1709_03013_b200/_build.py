@@ -17,10 +17,11 @@ def _sources():
     return srcs
 
 
-def needs_build():
-    if not os.path.exists(LIB_PATH):
+def needs_build(path=None):
+    path = path or LIB_PATH
+    if not os.path.exists(path):
         return True
-    t = os.path.getmtime(LIB_PATH)
+    t = os.path.getmtime(path)
     return any(os.path.getmtime(s) > t for s in _sources())
 
 
@@ -29,7 +30,7 @@ def build(force=False, verbose=False, ablate=False, defines=()):
     ablate=True builds libcsg_ablate.so instead: the same sources with -DCSG_ABLATE, i.e. with the timing-ablation
     switches of the fp4 kernel and csg_set_debug compiled in (wrong counts when set; never the product library)."""
     out = ABLATE_LIB_PATH if ablate else LIB_PATH
-    if not force and not ablate and not defines and not needs_build():
+    if not force and not defines and not needs_build(out):
         return out
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     cmd = [

@@ -27,6 +27,7 @@ def main():
     ap.add_argument("--config", type=int, default=2, help="index into csg_inputs.CONFIGS")
     ap.add_argument("--debug", default="0,14,9,63,64", help="comma-separated CSG_DEBUG values")
     ap.add_argument("--runs", type=int, default=4)
+    ap.add_argument("--sparse", type=int, default=0, help="csg_set_sparse mode: 0 auto, 1 on, 2 off (dense sweep)")
     args = ap.parse_args()
     csg.LIB_PATH = csg._build.build(ablate=True)       # never the product library
     lib = csg.load()
@@ -36,6 +37,7 @@ def main():
     _, bits = csg_inputs.make_config(cfg)
     d = csg.to_device(bits)
     csg.csg_set_variant(csg.VARIANT_TENSOR_FP4)
+    csg.csg_set_sparse(args.sparse)
     csg.csg_set_kernel_timing(True)
     for dbg in [int(x) for x in args.debug.split(",")]:
         lib.csg_set_debug(dbg)
@@ -44,7 +46,7 @@ def main():
             csg.csg_action(d, N, dim, 1.0, 3)
             torch.cuda.synchronize()
             ms.append(csg.csg_last_kernel_ms())
-        print("%s CSG_DEBUG=%-4d kernel ms %s" % (cfg["name"], dbg, " ".join("%.3f" % m for m in ms)), flush=True)
+        print("%s sparse=%d CSG_DEBUG=%-4d kernel ms %s" % (cfg["name"], args.sparse, dbg, " ".join("%.3f" % m for m in ms)), flush=True)
     lib.csg_set_debug(0)
     csg.csg_set_kernel_timing(False)
     csg.csg_set_variant(csg.VARIANT_AUTO)

@@ -88,7 +88,7 @@ struct Device {
     std::vector<uint32_t*> occ_retired;
     long long occ_next = 0;
     // end-to-end (host buffer) path
-    cudaStream_t host_stream = nullptr, copy_stream = nullptr;
+    cudaStream_t host_stream = nullptr, copy_stream = nullptr, occ_stream = nullptr;
     uint64_t* d_bits = nullptr;
     size_t d_bits_bytes = 0;
     long long* d_counts = nullptr;
@@ -322,7 +322,11 @@ static int ensure_tensor_ready(Device* D) {
     CSG_OPT_IN((tensor_action_kernel<KIND_I8, 4, TCF_DUMP>), s8);
     CSG_OPT_IN((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA>), s4);
     CSG_OPT_IN((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA | TCF_WAIT>), s4);
-    CSG_OPT_IN((tensor_action_kernel<KIND_FP4, 0, TCF_DUMP>), s4);
+    CSG_OPT_IN((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA | TCF_SPARSE>), s4);
+    CSG_OPT_IN((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA | TCF_SPARSE | TCF_WAIT>), s4);
+    CSG_OPT_IN((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA | TCF_GATE>), s4);
+    CSG_OPT_IN((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA | TCF_GATE | TCF_SPARSE>), s4);
+    CSG_OPT_IN((tensor_action_kernel<KIND_FP4, 0, TCF_DUMP | TCF_SPARSE>), s4);
     CSG_OPT_IN((tensor_peak_kernel<KIND_FP4>), s4);
     CSG_OPT_IN((tensor_peak_kernel<KIND_I8>), s8);
 #undef CSG_OPT_IN
@@ -340,7 +344,7 @@ static int ensure_tensor_ready(Device* D) {
     cfg.attrs = &attr;
     cfg.numAttrs = 1;
     int nclusters = 0;
-    if (cudaOccupancyMaxActiveClusters(&nclusters, tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA | TCF_WAIT>, &cfg) != cudaSuccess) {
+    if (cudaOccupancyMaxActiveClusters(&nclusters, tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA | TCF_SPARSE | TCF_WAIT>, &cfg) != cudaSuccess) {
         cudaGetLastError();
         nclusters = 0;
     }
@@ -359,7 +363,11 @@ static int launch_tensor(Device* D, int kind, const uint64_t* rel_bits, long lon
     const CUtensorMap* map = nullptr;
     rc = ensure_bits_map(D, kind, rel_bits, N, stride, &map);
     if (rc) return rc;
-    const int grid = 2 * std::max(1, std::min(ntiles, D->sm_count / 2));   // one CTA pair per SM pair
+    // One CTA pair per SM pair.  The gated launch of the host-matrix pipeline with the block-sparse sweep leaves one SM
+    // pair free: it waits for occupancy kernels that are launched while it runs, and those must find an SM (next to a
+    // CTA of this kernel there is no room: 18 warps x 96 registers fill two of the four register files of an SM).
+    const int clusters = std::max(1, D->sm_count / 2 - ((landed && occ) ? 1 : 0));
+    const int grid = 2 * std::max(1, std::min(ntiles, clusters));
     // Drift throttle (tensor_kernel.cuh, TC_MAX_LEAD): fewer DRAM reads, so less power.  Measured (round 2 kernel):
     // config 4 (N = 262144, 8 GiB, full histogram) 942 -> 847 ms; config 3 (N = 131072, 2 GiB), where the kernel now
     // runs into the 1 kW power cap: a single launch 88.5 either way, twelve back to back 89.9 (drifting up to 92) ->
@@ -383,8 +391,13 @@ static int launch_tensor(Device* D, int kind, const uint64_t* rel_bits, long lon
     // (N-2) << 2TB < 2^31; TB = 7 turns every unpack shift into a left shift (FMA pipe).
     const int tb = N - 2 < (1LL << 17) ? 7 : N - 2 < (1LL << 19) ? 6 : N - 2 < (1LL << 21) ? 5 : 4;
     if (kind == KIND_FP4) {
-        if (dump) CSG_LAUNCH((tensor_action_kernel<KIND_FP4, 0, TCF_DUMP>), s4);
-        else if (progress || landed) CSG_LAUNCH((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA | TCF_WAIT>), s4);
+        // one instantiation per combination in use, so that a launch carries only the code it needs (tensor_kernel.cuh)
+        if (dump) CSG_LAUNCH((tensor_action_kernel<KIND_FP4, 0, TCF_DUMP | TCF_SPARSE>), s4);
+        else if (landed && occ) CSG_LAUNCH((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA | TCF_GATE | TCF_SPARSE>), s4);
+        else if (landed) CSG_LAUNCH((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA | TCF_GATE>), s4);
+        else if (progress && occ) CSG_LAUNCH((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA | TCF_SPARSE | TCF_WAIT>), s4);
+        else if (progress) CSG_LAUNCH((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA | TCF_WAIT>), s4);
+        else if (occ) CSG_LAUNCH((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA | TCF_SPARSE>), s4);
         else CSG_LAUNCH((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA>), s4);
     } else if (dump) {
         if (tb == 7) CSG_LAUNCH((tensor_action_kernel<KIND_I8, 7, TCF_DUMP>), s8);
@@ -404,20 +417,20 @@ static int launch_tensor(Device* D, int kind, const uint64_t* rel_bits, long lon
 }
 
 // Block-sparse K sweep of the fp4 tensor kernel (occupancy_kernel.cuh): one pass over the matrix marks the empty
-// 256 x 256 blocks, and the kernel skips every two-stage group whose U or L block is empty.  Measured at config 3 (4D,
-// N = 131072): 10.8 % of the groups are dead.  AUTO: matrices of 512 MiB and more (the pass costs one HBM read of the
-// matrix, 0.4 % of the action there; a 1+1 set has no empty block and only pays that); ON: every fp4 launch (tests).
-// *occ = nullptr when the sweep stays dense.
+// 256 x 256 blocks, and the kernel skips every two-stage group whose U or L blocks are empty.  Measured at config 3 (4D,
+// N = 131072): 10.8 % of the groups are dead, 88.5 -> 81.8 ms.  A 1+1 set (flat or de Sitter) has no empty block: there
+// the pass and the mask loop cost 2 % (de Sitter N = 131072: 94.0 -> 96.0 ms).  So CSG_SPARSE_AUTO switches it on for
+// matrices of 512 MiB and more unless the caller says dim = 2 (csg_action_partial has no dim: on); ON: every fp4
+// launch (tests).  *occ = nullptr when the sweep stays dense.
 constexpr long long SPARSE_MIN_BYTES = 512LL << 20;
 
-static int occupancy_pass(Device* D, int kind, const uint64_t* rel_bits, long long N, long long stride,
-                          const uint32_t** occ, cudaStream_t stream) {
+// The occupancy map of the next launch (one of OCC_RING buffers), or *occ = nullptr when the sweep stays dense.
+static int occupancy_buffer(Device* D, int kind, long long N, long long stride, int dim_hint, uint32_t** occ) {
     *occ = nullptr;
     if (kind != KIND_FP4 || g.sparse == CSG_SPARSE_OFF) return CSG_OK;
-    if (g.sparse == CSG_SPARSE_AUTO && N * stride * 8 < SPARSE_MIN_BYTES) return CSG_OK;
+    if (g.sparse == CSG_SPARSE_AUTO && (N * stride * 8 < SPARSE_MIN_BYTES || dim_hint == 2)) return CSG_OK;
     const int nB = (int)((N + TC_T - 1) / TC_T);
-    const int ostride = occ_stride_words(N);
-    const size_t words = (size_t)nB * ostride;
+    const size_t words = (size_t)nB * occ_stride_words(N);
     const int slot = (int)(D->occ_next++ % OCC_RING);
     if (D->d_occ_words[slot] < words) {
         if (D->d_occ[slot]) D->occ_retired.push_back(D->d_occ[slot]);
@@ -426,15 +439,34 @@ static int occupancy_pass(Device* D, int kind, const uint64_t* rel_bits, long lo
         CSG_CUDA(cudaMalloc(&D->d_occ[slot], words * sizeof(uint32_t)));
         D->d_occ_words[slot] = words;
     }
-    occupancy_kernel<<<dim3(ostride / 4, nB), OCC_THREADS, 0, stream>>>(rel_bits, N, stride, D->d_occ[slot], ostride);
-    CSG_CUDA(cudaGetLastError());
-    ++g.launches;
     *occ = D->d_occ[slot];
     return CSG_OK;
 }
 
+// Marks row blocks [block0, block0 + nblocks) of the map.
+static int occupancy_launch(const uint64_t* rel_bits, long long N, long long stride, uint32_t* occ, int block0, int nblocks,
+                            cudaStream_t stream) {
+    const int ostride = occ_stride_words(N);
+    occupancy_kernel<<<dim3(ostride / OCC_WORDS_PER_CTA, nblocks), OCC_THREADS, 0, stream>>>(rel_bits, N, stride, occ, ostride, block0);
+    CSG_CUDA(cudaGetLastError());
+    ++g.launches;
+    return CSG_OK;
+}
+
+static int occupancy_pass(Device* D, int kind, const uint64_t* rel_bits, long long N, long long stride, int dim_hint,
+                          const uint32_t** occ, cudaStream_t stream) {
+    uint32_t* buf = nullptr;
+    *occ = nullptr;
+    int rc = occupancy_buffer(D, kind, N, stride, dim_hint, &buf);
+    if (rc || !buf) return rc;
+    if ((rc = occupancy_launch(rel_bits, N, stride, buf, 0, (int)((N + TC_T - 1) / TC_T), stream))) return rc;
+    *occ = buf;
+    return CSG_OK;
+}
+
 // Interval kernel over the tiles of one shard: counts (kmax+1 int64, overwritten) <- this shard's abundances.
-static int interval_device(Device* D, const uint64_t* rel_bits, long long N, int kmax, int shard, int nshards,
+// dim_hint: the caller's dim (2 or 4) or 0 when the entry point has none; only steers CSG_SPARSE_AUTO.
+static int interval_device(Device* D, const uint64_t* rel_bits, long long N, int kmax, int shard, int nshards, int dim_hint,
                            long long* counts, cudaStream_t stream) {
     const long long stride = csg_row_stride_words(N);
     CSG_CUDA(cudaMemsetAsync(counts, 0, (size_t)(kmax + 1) * sizeof(long long), stream));
@@ -457,7 +489,7 @@ static int interval_device(Device* D, const uint64_t* rel_bits, long long N, int
     }
     if (tensor) {
         const uint32_t* occ = nullptr;
-        if ((rc = occupancy_pass(D, kind, rel_bits, N, stride, &occ, stream))) return rc;
+        if ((rc = occupancy_pass(D, kind, rel_bits, N, stride, dim_hint, &occ, stream))) return rc;
         rc = launch_tensor(D, kind, rel_bits, N, stride, kmax, counts, tl->d, tl->n, nullptr, nullptr, nullptr, occ, stream);
         if (rc) return rc;
     } else {
@@ -535,7 +567,7 @@ static int action_fused_small(Device* D, const uint64_t* rel_bits, long long N, 
 static int action_device(Device* D, const uint64_t* rel_bits, long long N, int dim, double eps, int kmax,
                          long long* counts, double* S, cudaStream_t stream) {
     if (fused_small_ok(N, kmax, stream)) return action_fused_small(D, rel_bits, N, dim, eps, kmax, counts, S, stream);
-    int rc = interval_device(D, rel_bits, N, kmax, 0, 1, counts, stream);
+    int rc = interval_device(D, rel_bits, N, kmax, 0, 1, dim, counts, stream);
     if (rc) return rc;
     return finish_device(counts, N, dim, eps, kmax, S, stream);
 }
@@ -602,7 +634,7 @@ static int ensure_chunk_tiles(Device* D, long long N, const ChunkTiles** out) {
         delete c;
         return cuda_fail(e, "tile list of the host pipeline");
     }
-    while ((int)D->chunk_ev.size() < nchunks + 2) {
+    while ((int)D->chunk_ev.size() < 2 * nchunks + 2) {
         cudaEvent_t ev;
         CSG_CUDA(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
         D->chunk_ev.push_back(ev);
@@ -627,7 +659,7 @@ static WriteValue32Fn stream_write_value32() {
 }
 
 static int interval_host_pipelined(Device* D, const uint64_t* rel_bits_host, uint64_t* d_bits, long long N, int kmax,
-                                   int kind, long long* counts, cudaStream_t stream) {
+                                   int kind, int dim_hint, long long* counts, cudaStream_t stream) {
     const long long stride = csg_row_stride_words(N);
     const ChunkTiles* ct = nullptr;
     int rc = ensure_chunk_tiles(D, N, &ct);
@@ -639,6 +671,14 @@ static int interval_host_pipelined(Device* D, const uint64_t* rel_bits_host, uin
     // the copies must not overtake work of an earlier call that still reads d_bits on `stream`
     CSG_CUDA(cudaEventRecord(ev_prev, stream));
     CSG_CUDA(cudaStreamWaitEvent(D->copy_stream, ev_prev, 0));
+    // Block-sparse sweep: the row blocks of a chunk are marked (occupancy kernel) right behind the chunk's copy and BEFORE
+    // the chunk is published, so the two occupancy rows a tile reads are complete when the tile may start.  The kernels
+    // run on a stream of their own (behind an event per copy), so the copies stay back to back; that stream then
+    // publishes the chunks.  A gated launch leaves them one SM pair (launch_tensor).
+    uint32_t* occ = nullptr;
+    if ((rc = occupancy_buffer(D, kind, N, stride, dim_hint, &occ))) return rc;
+    if (occ && !D->occ_stream) CSG_CUDA(cudaStreamCreateWithFlags(&D->occ_stream, cudaStreamNonBlocking));
+    cudaStream_t publish = occ ? D->occ_stream : D->copy_stream;
     WriteValue32Fn write32 = kind == KIND_FP4 && g.host_pipeline != CSG_HOST_PIPELINE_CHUNKED ? stream_write_value32() : nullptr;
     if (write32) {
         if (!D->d_landed) CSG_CUDA(cudaMalloc(&D->d_landed, sizeof(unsigned int)));
@@ -648,7 +688,7 @@ static int interval_host_pipelined(Device* D, const uint64_t* rel_bits_host, uin
         } else {
             CSG_CUDA(cudaEventRecord(ev_reset, D->copy_stream));
             CSG_CUDA(cudaStreamWaitEvent(stream, ev_reset, 0));
-            rc = launch_tensor(D, kind, d_bits, N, stride, kmax, counts, ct->d, ct->n, D->d_landed, ct->d_need, nullptr, nullptr, stream);
+            rc = launch_tensor(D, kind, d_bits, N, stride, kmax, counts, ct->d, ct->n, D->d_landed, ct->d_need, nullptr, occ, stream);
             if (rc) return rc;
         }
     }
@@ -656,17 +696,23 @@ static int interval_host_pipelined(Device* D, const uint64_t* rel_bits_host, uin
         const long long row0 = ct->row_begin[c], row1 = ct->row_end[c];
         CSG_CUDA(cudaMemcpyAsync(d_bits + row0 * stride, rel_bits_host + row0 * stride,
                                  (size_t)(row1 - row0) * stride * sizeof(uint64_t), cudaMemcpyHostToDevice, D->copy_stream));
+        if (occ) {
+            CSG_CUDA(cudaEventRecord(D->chunk_ev[nchunks + 2 + c], D->copy_stream));
+            CSG_CUDA(cudaStreamWaitEvent(D->occ_stream, D->chunk_ev[nchunks + 2 + c], 0));
+            const int b0 = (int)(row0 / TC_T), b1 = (int)((row1 + TC_T - 1) / TC_T);
+            if ((rc = occupancy_launch(d_bits, N, stride, occ, b0, b1 - b0, D->occ_stream))) return rc;
+        }
         if (write32) {
-            if (write32(D->copy_stream, (CUdeviceptr)D->d_landed, (cuuint32_t)(c + 1), 0) != CUDA_SUCCESS) {
+            if (write32(publish, (CUdeviceptr)D->d_landed, (cuuint32_t)(c + 1), 0) != CUDA_SUCCESS) {
                 snprintf(g.cuda_msg, sizeof(g.cuda_msg), "cuStreamWriteValue32 failed while a gated launch is waiting");
                 return CSG_E_CUDA;
             }
         } else {
-            CSG_CUDA(cudaEventRecord(D->chunk_ev[c], D->copy_stream));
+            CSG_CUDA(cudaEventRecord(D->chunk_ev[c], publish));
             CSG_CUDA(cudaStreamWaitEvent(stream, D->chunk_ev[c], 0));
             const int nt = ct->off[c + 1] - ct->off[c];
             if (nt > 0) {
-                rc = launch_tensor(D, kind, d_bits, N, stride, kmax, counts, ct->d + ct->off[c], nt, nullptr, nullptr, nullptr, nullptr, stream);
+                rc = launch_tensor(D, kind, d_bits, N, stride, kmax, counts, ct->d + ct->off[c], nt, nullptr, nullptr, nullptr, occ, stream);
                 if (rc) return rc;
             }
         }
@@ -734,6 +780,7 @@ static void release_device(Device* D) {
     for (auto& kv : D->fused_ws) cudaFree(kv.second);
     for (cudaEvent_t e : D->chunk_ev) cudaEventDestroy(e);
     if (D->copy_stream) cudaStreamDestroy(D->copy_stream);
+    if (D->occ_stream) cudaStreamDestroy(D->occ_stream);
     if (D->host_stream) cudaStreamDestroy(D->host_stream);
     if (D->link_ev0) cudaEventDestroy(D->link_ev0);
     if (D->link_ev1) cudaEventDestroy(D->link_ev1);
@@ -776,7 +823,7 @@ int csg_action_partial(const uint64_t* rel_bits, int64_t N, int kmax, int shard,
     Device* D = nullptr;
     int rc = current_device(&D);
     if (rc) return rc;
-    return interval_device(D, rel_bits, N, kmax, shard, nshards, reinterpret_cast<long long*>(counts), stream);
+    return interval_device(D, rel_bits, N, kmax, shard, nshards, 0, reinterpret_cast<long long*>(counts), stream);
 }
 
 int csg_action_finish(const int64_t* counts, int64_t N, int dim, double eps, int kmax, double* S,
@@ -821,7 +868,7 @@ int csg_action_batch(const uint64_t* rel_bits, int64_t N, int64_t batch, int dim
     } else {
         // large sets fill the machine on their own: one tensor launch per set, back to back on the stream
         for (int64_t b = 0; b < batch; ++b) {
-            rc = interval_device(D, rel_bits + b * set_words, N, kmax, 0, 1, c + b * (kmax + 1), stream);
+            rc = interval_device(D, rel_bits + b * set_words, N, kmax, 0, 1, dim, c + b * (kmax + 1), stream);
             if (rc) return rc;
         }
     }
@@ -860,10 +907,11 @@ int csg_action_host(const uint64_t* rel_bits_host, int64_t N, int dim, double ep
     const int variant = effective_variant(N);
     if (variant != CSG_VARIANT_BITSET && bits_bytes >= (size_t)HOST_PIPELINE_MIN_BYTES) {
         rc = interval_host_pipelined(D, rel_bits_host, D->d_bits, N, kmax,
-                                     variant == CSG_VARIANT_TENSOR_FP4 ? KIND_FP4 : KIND_I8, D->d_counts, D->host_stream);
+                                     variant == CSG_VARIANT_TENSOR_FP4 ? KIND_FP4 : KIND_I8, dim, D->d_counts, D->host_stream);
         if (rc) {
             cudaStreamSynchronize(D->host_stream);     // never leave a gated launch or a copy behind an error return
             cudaStreamSynchronize(D->copy_stream);
+            if (D->occ_stream) cudaStreamSynchronize(D->occ_stream);
             return rc;
         }
         rc = finish_device(D->d_counts, N, dim, eps, kmax, D->d_S, D->host_stream);
@@ -976,7 +1024,7 @@ int csg_tile_interval_sizes(const uint64_t* rel_bits, int64_t N, const int32_t* 
     if (e == cudaSuccess) {
         const int kind = variant == CSG_VARIANT_TENSOR_FP4 ? KIND_FP4 : KIND_I8;
         const uint32_t* occ = nullptr;
-        rc = occupancy_pass(D, kind, rel_bits, N, csg_row_stride_words(N), &occ, stream);
+        rc = occupancy_pass(D, kind, rel_bits, N, csg_row_stride_words(N), 0, &occ, stream);
         if (rc == CSG_OK)
             rc = launch_tensor(D, kind, rel_bits, N, csg_row_stride_words(N), 0, nullptr, d_tiles, (int)ntiles, nullptr, nullptr,
                                n_out, occ, stream);
@@ -1032,7 +1080,7 @@ int csg_block_occupancy(const uint64_t* rel_bits, int64_t N, uint32_t* occ, cuda
     int rc = current_device(&D);
     if (rc) return rc;
     const int nB = (int)((N + TC_T - 1) / TC_T), ostride = occ_stride_words(N);
-    occupancy_kernel<<<dim3(ostride / 4, nB), OCC_THREADS, 0, stream>>>(rel_bits, N, csg_row_stride_words(N), occ, ostride);
+    occupancy_kernel<<<dim3(ostride / OCC_WORDS_PER_CTA, nB), OCC_THREADS, 0, stream>>>(rel_bits, N, csg_row_stride_words(N), occ, ostride, 0);
     CSG_CUDA(cudaGetLastError());
     ++g.launches;
     return CSG_OK;

@@ -10,16 +10,17 @@
 //
 // occ: nB rows (nB = ceil(N / 256)) of occ_stride 32-bit words; bit (K mod 32) of word K / 32 of row I is set iff
 // some bit of rows 256 I .. 256 I + 255, columns 256 K .. 256 K + 255 is set.  Every word of a row is written (words
-// beyond the last column block as zero), so the buffer needs no memset.  HBM-bound: one coalesced read of the matrix.
+// beyond the last column block as zero), so the buffer needs no memset.  HBM-bound: one coalesced read of the matrix
+// (0.295 ms for 2 GiB).
 #pragma once
 #include <cstdint>
 
 namespace csg {
 
 constexpr int OCC_THREADS = 256;                       // 8 warps; a thread owns 16 bytes (128 columns) of every row
-constexpr int OCC_BLOCKS_PER_CTA = OCC_THREADS / 2;    // 128 column blocks = 4 output words per CTA
+constexpr int OCC_WORDS_PER_CTA = OCC_THREADS / 64;    // 128 column blocks = 4 output words per CTA
 constexpr int OCC_ROWS = 256;
-constexpr int OCC_PAD_WORDS = 4;                       // zero words after the last column block (the kernel reads ahead)
+constexpr int OCC_PAD_WORDS = 4;                       // zero words after the last column block (the kernel reads 2 ahead)
 
 // occ_stride for N: a multiple of 4 words (one CTA writes 4), at least ceil(nB / 32) + OCC_PAD_WORDS.
 __host__ __device__ inline int occ_stride_words(long long N) {
@@ -27,12 +28,13 @@ __host__ __device__ inline int occ_stride_words(long long N) {
     return (((nB + 31) / 32 + OCC_PAD_WORDS + 3) / 4) * 4;
 }
 
-// grid = (occ_stride / 4, nB): CTA (c, I) reduces rows of block I over column blocks 128 c .. 128 c + 127.
+// grid = (occ_stride / 4, number of row blocks): CTA (c, y) reduces the rows of block I = block0 + y over column blocks
+// 128 c .. 128 c + 127.  block0 > 0: the host-matrix pipeline marks the row blocks of one chunk as soon as it has landed.
 __global__ void __launch_bounds__(OCC_THREADS)
 occupancy_kernel(const uint64_t* __restrict__ rel, long long N, long long stride_words, uint32_t* __restrict__ occ,
-                 int occ_stride) {
+                 int occ_stride, int block0) {
     __shared__ uint32_t part[OCC_THREADS / 32];
-    const int I = blockIdx.y;
+    const int I = block0 + blockIdx.y;
     const long long row0 = (long long)I * OCC_ROWS;
     const int nrows = (int)min((long long)OCC_ROWS, N - row0);
     const long long q = (long long)blockIdx.x * OCC_THREADS + threadIdx.x;     // 16-byte chunk of the row
@@ -63,8 +65,8 @@ occupancy_kernel(const uint64_t* __restrict__ rel, long long N, long long stride
     b = (b | (b >> 8)) & 0x0000FFFFu;
     if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = b;                    // 16 blocks per warp
     __syncthreads();
-    if (threadIdx.x < 4) {
-        const int w = 4 * blockIdx.x + threadIdx.x;
+    if (threadIdx.x < OCC_WORDS_PER_CTA) {
+        const int w = OCC_WORDS_PER_CTA * blockIdx.x + threadIdx.x;
         if (w < occ_stride) occ[(long long)I * occ_stride + w] = part[2 * threadIdx.x] | (part[2 * threadIdx.x + 1] << 16);
     }
 }

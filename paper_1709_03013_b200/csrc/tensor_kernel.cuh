@@ -28,14 +28,17 @@
 //   * the open range i<k<j costs nothing in the steady state: only the stages that overlap block I need the k>i
 //     mask and only those that overlap block J the k<j mask;
 //   * fused epilogue by the producer warps: tcgen05.ld of their CTA's accumulators, bit R[i][j] (and i<j), n_ij
-//     into a privatised shared-memory histogram (bins < 2048) or straight into the global counts (higher bins,
+//     into a privatised shared-memory histogram (bins < TC_HIST) or straight into the global counts (higher bins,
 //     smeared action only).  The first two groups of the NEXT tile are expanded before the epilogue of a tile, so
 //     the tensor cores restart as soon as the accumulators are drained.  No N x N count matrix ever reaches HBM.
 //
-// Template FLAGS select what else is compiled in: TCF_WAIT (the TMA thread may wait on two global words before it
-// starts a tile: the drift throttle and the host-copy gate, see below), TCF_DUMP (test hook csg_tile_interval_sizes:
-// the epilogue writes every n_ij of the listed tiles instead of bucketing it), TCF_ABLATE (only in the separate
-// -DCSG_ABLATE build of paper_1709_03013_b200/ablate.py, never in libcsg.so).
+// Template FLAGS select what else is compiled in, so that a launch pays only for what it uses: TCF_WAIT (drift
+// throttle: the TMA thread may wait for the finished-tile counter before it starts a tile), TCF_GATE (host-copy gate of
+// csg_action_host: tiles wait for the chunks of the matrix they read; implies the throttle code), TCF_SPARSE
+// (block-sparse K sweep: the roles walk the live-group masks of the occupancy map instead of a counted loop; fp4
+// kind), TCF_DUMP (test hook csg_tile_interval_sizes: the epilogue writes every n_ij of the listed tiles instead of
+// bucketing it), TCF_ABLATE (only in the separate -DCSG_ABLATE build of paper_1709_03013_b200/ablate.py, never in
+// libcsg.so).
 // `dbg` (csg_set_debug of the ABLATE build; 0 and compiled out everywhere else) switches parts of the kernel off
 // for timing ablations (1: no MMA issue, 2: no
 // expansion arithmetic, 4: no operand stores, 8: no bucketing in the epilogue, 16: no fence before publishing a stage, 32: no
@@ -75,9 +78,16 @@ constexpr int TC_THREADS = TC_PRODUCERS + 64;  // + the MMA warp + the TMA warp
 constexpr bool TC_WHOLE_GROUP = CSG_WHOLE_GROUP != 0;   // a producer set expands both stages of every second group
 constexpr int TC_MAX_LEAD = 1;                 // rounds a cluster may run ahead of the average (L2 sharing inside a patch)
 constexpr int TC_THROTTLE_MAX_POLLS = 1 << 15; // polls of >= 200 ns in ONE wait before a cluster stops throttling for good (see the TMA warp)
-constexpr int TCF_ABLATE = 1, TCF_WAIT = 2, TCF_DUMP = 4;   // template FLAGS of tensor_action_kernel
+constexpr int TCF_ABLATE = 1, TCF_WAIT = 2, TCF_DUMP = 4, TCF_GATE = 8, TCF_SPARSE = 16;   // template FLAGS of tensor_action_kernel
 constexpr int TC_PREFILL_GROUPS = 2;           // groups (2 stages each) of the next tile expanded before a tile's epilogue
-constexpr int TC_HIST = 2048;              // privatised low bins per CTA
+#ifndef CSG_TC_HIST
+#define CSG_TC_HIST 2048
+#endif
+// Privatised low bins per CTA (u32, shared memory); higher bins (full-histogram epilogue only) go to the global histogram
+// with one red.add per value.  Measured with 12288 bins (48 KiB, all that is left beside the operand ring): the
+// full-histogram configs gain < 1 % and config 3 loses 2 % (81.8 -> 83.5 ms: the L1 that remains next to 213 KiB of
+// shared memory is too small for the epilogue's relation words and the per-tile loads), so 2048 stays.
+constexpr int TC_HIST = CSG_TC_HIST;
 
 // The two operand encodings of the kernel.
 //   KIND_I8 : one relation bit -> one u8 (0 or 1 << TB); tcgen05.mma kind::i8, K = 32 per instruction, s32
@@ -387,13 +397,49 @@ __device__ __forceinline__ void tile_k_range(int I, int J, int& kb_begin, int& k
     }
 }
 
-// Live groups of a tile (block-sparse K sweep).  A group = TC_GROUP = 2 consecutive stages, the unit of one packed-bit
-// copy and of a producer set's turn.  occ = block occupancy of the relation matrix (occupancy_kernel.cuh; fp4 kind,
-// 256-column stages, so stage kb of the sweep IS column block kb): stage kb of tile (I, J) multiplies block (I, kb) of
-// U with block (J, kb) of L and is dead when either block is empty; a group is live when one of its two stages is.
-// Returns the live mask of groups 32 gw .. 32 gw + 31 of the tile (group g = stages kb_begin + 2g, + 2g + 1).  With
-// occ == nullptr every group of the range is live (the dense sweep).  All three roles of the kernel (TMA thread,
-// producers, MMA thread) walk the same masks, so they agree on the sequence of groups without talking to each other.
+// Host-copy gate (csg_action_host): the matrix arrives in row chunks on a copy stream, which publishes the number of chunks
+// delivered after each one (and after that chunk's rows of the occupancy map are complete); tile (I, J) reads the rows
+// of blocks I and J only, and the host has worked out how many chunks that takes in its copy order.  The wait depends
+// on the copy stream alone, never on another CTA.  The TMA thread waits before it fetches the tile's bits; with the
+// block-sparse sweep the producers and the MMA thread wait, too, before they read the tile's occupancy rows (when the
+// TMA thread is held up they catch up with it and would otherwise read rows that are not written yet).
+__device__ __forceinline__ void wait_landed(const unsigned int* landed, unsigned int need, unsigned int& chunks_seen) {
+    if (chunks_seen >= need) return;
+    unsigned int got;
+    while (true) {
+        asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(got) : "l"(landed) : "memory");
+        if (got >= need) break;
+        __nanosleep(500);
+    }
+    chunks_seen = got;
+}
+
+// Live groups of a tile (block-sparse K sweep, template flag TCF_SPARSE).  A group = TC_GROUP = 2 consecutive stages, the
+// unit of one packed-bit copy and of a producer set's turn.  occ = block occupancy of the relation matrix
+// (occupancy_kernel.cuh; fp4 kind, 256-column stages, so stage kb of the sweep IS column block kb): stage kb of tile
+// (I, J) multiplies block (I, kb) of U with block (J, kb) of L and is dead when either block is empty; a group is live
+// when one of its two stages is.  live_groups_word returns the live mask of groups 32 gw .. 32 gw + 31 of the tile
+// (group g = stages kb_begin + 2g, + 2g + 1); with occ == nullptr every group of the range is live.  All three roles of
+// the kernel (TMA thread, producers, MMA thread) walk the same masks, so they agree on the sequence of groups without
+// talking to each other.  Without TCF_SPARSE the sweep is the plain counted loop over all groups.
+// Tried and dropped (measured at config 3, same box): an occupancy map in half-stages of 128 columns with the MMA thread
+// skipping the dead half-stages inside live groups (6 % fewer MMAs): 83.7 ms against 81.8 -- the producers still expand
+// them, they sit in the few groups at both ends of a sweep where the kernel is then producer-bound, and the longer
+// issue loop costs every stage; running the dense configs through the mask loop with a null map: +4 % at config 1;
+// one inlined call site for the epilogue through an end-of-tile call of the loop body: 87.6 ms (more loop state, spills);
+// the MMA warp computing a tile's first mask word before it waits for the accumulators: no change (81.8 ms).
+// COHERENT (TCF_GATE): the occupancy rows are written by another kernel WHILE this one runs (host-matrix pipeline: a
+// row block is marked when its chunk has landed, before the chunk count that lets a tile start is published), so they
+// are read from L2 (ld.relaxed.gpu) -- a row that shares a 128-byte line with one read earlier could otherwise come
+// stale from L1.
+template <bool COHERENT>
+__device__ __forceinline__ uint32_t occ_load(const uint32_t* p) {
+    if (!COHERENT) return __ldg(p);
+    uint32_t v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+template <bool COHERENT>
 __device__ __forceinline__ uint32_t live_groups_word(const uint32_t* __restrict__ occI, const uint32_t* __restrict__ occJ,
                                                      int kb_begin, int kb_end, int gw) {
     const int rem = ((kb_end - kb_begin) >> 1) - 32 * gw;          // groups left from this word on
@@ -401,8 +447,9 @@ __device__ __forceinline__ uint32_t live_groups_word(const uint32_t* __restrict_
     if (occI == nullptr) return in_range;
     const int s = kb_begin + 64 * gw;                              // first stage of the word
     const int w = s >> 5, sh = s & 31;
-    const uint32_t a0 = __ldg(occI + w) & __ldg(occJ + w), a1 = __ldg(occI + w + 1) & __ldg(occJ + w + 1),
-                   a2 = __ldg(occI + w + 2) & __ldg(occJ + w + 2);  // rows are padded with zero words (OCC_PAD_WORDS)
+    const uint32_t a0 = occ_load<COHERENT>(occI + w) & occ_load<COHERENT>(occJ + w),
+                   a1 = occ_load<COHERENT>(occI + w + 1) & occ_load<COHERENT>(occJ + w + 1),
+                   a2 = occ_load<COHERENT>(occI + w + 2) & occ_load<COHERENT>(occJ + w + 2);  // rows end in zero words (OCC_PAD_WORDS)
     uint64_t S = ((uint64_t)__funnelshift_r(a1, a2, sh) << 32) | __funnelshift_r(a0, a1, sh);   // stages s .. s + 63
     S = (S | (S >> 1)) & 0x5555555555555555ull;                    // bit 2g: group g has a live stage
     S = (S | (S >> 1)) & 0x3333333333333333ull;                    // compress the even bits
@@ -413,16 +460,20 @@ __device__ __forceinline__ uint32_t live_groups_word(const uint32_t* __restrict_
     return (uint32_t)S & in_range;
 }
 // Calls body(kb0) for the first stage kb0 of every live group of the tile, in ascending order; a tile without any
-// live group still gets its first group (the MMA of a tile's first stage is what zeroes the accumulators).
-template <class F>
+// live group still gets its first group (the MMA of a tile's first stage is what clears the accumulators).
+template <bool SPARSE, bool COHERENT, class F>
 __device__ __forceinline__ void for_live_groups(const uint32_t* __restrict__ occ, int occ_stride, int I, int J,
                                                 int kb_begin, int kb_end, F&& body) {
+    if (!SPARSE) {
+        for (int kb0 = kb_begin; kb0 < kb_end; kb0 += TC_GROUP) body(kb0);
+        return;
+    }
     const uint32_t* occI = occ ? occ + (size_t)I * occ_stride : nullptr;
     const uint32_t* occJ = occ ? occ + (size_t)J * occ_stride : nullptr;
     const int nwords = (((kb_end - kb_begin) >> 1) + 31) >> 5;
     int done = 0;
     for (int gw = 0; gw <= nwords; ++gw) {
-        uint32_t m = gw < nwords ? live_groups_word(occI, occJ, kb_begin, kb_end, gw) : (done == 0 ? 1u : 0u);
+        uint32_t m = gw < nwords ? live_groups_word<COHERENT>(occI, occJ, kb_begin, kb_end, gw) : (done == 0 ? 1u : 0u);
         const int base = gw < nwords ? kb_begin + 64 * gw : kb_begin;
         while (m) {
             const int g = __ffs((int)m) - 1;
@@ -437,7 +488,7 @@ __device__ __forceinline__ void for_live_groups(const uint32_t* __restrict__ occ
 // 4^TB, the accumulator holds n_ij << 2TB; the host picks the largest TB with (N-2) << 2TB < 2^31 (exact in s32).
 // KIND_FP4: TB unused (pass 0); the f32 accumulator holds 4 n_ij, exact for n_ij < 2^22.
 // tiles[t] = {I, J}: 256-row blocks, I <= J.  Grid = 2 x (number of SM pairs), cluster (2,1,1).
-// progress (TCF_WAIT, may be NULL): zeroed counter of finished tiles, the drift throttle.  landed / tile_need (TCF_WAIT,
+// progress (TCF_WAIT or TCF_GATE, may be NULL): zeroed counter of finished tiles, the drift throttle.  landed / tile_need (TCF_GATE,
 // may be NULL): the host-copy gate -- *landed = number of row chunks of `rel` the copy stream has delivered so far,
 // tile_need[t] = how many must be there before tile t may start.  dump (TCF_DUMP): ntiles x 256 x 256 int32, n_ij or -1.
 template <int KIND, int TB, int FLAGS = 0>
@@ -447,10 +498,12 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                      const int2* __restrict__ tiles, int ntiles, int dbg_arg, unsigned int* __restrict__ progress_arg,
                      const unsigned int* __restrict__ landed_arg, const int* __restrict__ tile_need,
                      int* __restrict__ dump, const uint32_t* __restrict__ occ_arg, int occ_stride) {
-    constexpr bool ABLATE = (FLAGS & TCF_ABLATE) != 0, WAITS = (FLAGS & TCF_WAIT) != 0, DUMP = (FLAGS & TCF_DUMP) != 0;
+    constexpr bool ABLATE = (FLAGS & TCF_ABLATE) != 0, DUMP = (FLAGS & TCF_DUMP) != 0, GATE = (FLAGS & TCF_GATE) != 0;
+    constexpr bool WAITS = (FLAGS & (TCF_WAIT | TCF_GATE)) != 0;        // the TMA thread may wait on global words
+    constexpr bool SPARSE = (FLAGS & TCF_SPARSE) != 0 && KIND == KIND_FP4;   // block-sparse sweep: fp4 kind only (stage = column block)
     unsigned int* const progress = WAITS ? progress_arg : nullptr;      // compiled out of the instantiations that never wait
-    const unsigned int* const landed = WAITS ? landed_arg : nullptr;
-    const uint32_t* const occ = KIND == KIND_FP4 ? occ_arg : nullptr;   // block-sparse sweep: fp4 kind only (stage = column block)
+    const unsigned int* const landed = GATE ? landed_arg : nullptr;
+    const uint32_t* const occ = SPARSE ? occ_arg : nullptr;
     using T = TcTraits<KIND>;
     const int dbg = ABLATE ? dbg_arg : 0;             // compiled out of every instantiation of libcsg.so
     constexpr int COLS = T::STAGE_COLS, WORDS = T::WORDS;
@@ -537,6 +590,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
         const int cq = warp >> 2;                     // which 64 accumulator columns it drains
         uint32_t tphase = 0;                          // parity of tmem_full
         int epi_I = -1, epi_J = -1, epi_t = -1;       // tile whose accumulators still wait for their epilogue
+        unsigned int chunks_seen = 0;                 // host-copy gate: chunks known to have landed
 
         // Publish this set's stage that is written but not yet visible to the MMA thread.
         auto publish_pending = [&]() {
@@ -672,6 +726,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 epi_I = -1;
             }
             int gdone = 0;                            // live groups of this tile expanded so far
+            if (GATE && SPARSE && landed != nullptr && occ != nullptr) wait_landed(landed, (unsigned int)tile_need[t], chunks_seen);
             // One stage of one row: open-range mask, expansion, publish of this warp's previous stage, store.
             auto do_stage = [&](int kb, uint32_t stage, uint32_t eparity, uint32_t (&w)[WORDS]) {
                 if (dbg & 256) {                              // ablation: no open-range masks
@@ -717,7 +772,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 }
                 pending = (int)stage;
             };
-            for_live_groups(occ, occ_stride, I, J, kb_begin, kb_end, [&](int kb0) {
+            for_live_groups<SPARSE, GATE>(occ, occ_stride, I, J, kb_begin, kb_end, [&](int kb0) {
                 // The packed-bit buffer is released only after the operand stores that consume every word loaded from
                 // it: the hardware has then issued them after the LDS data arrived.  An arrive placed right after the
                 // LDS instructions is NOT ordered after their completion (naming the loaded registers as unused asm
@@ -814,6 +869,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
             const bool issuer = elect_one();
             uint32_t stage = 0, sphase = 0, ephase = 0;
             int done_tiles = 0;
+            unsigned int chunks_seen = 0;
             const uint32_t tmem_sfa = tmem_base + T::TMEM_SF, tmem_sfb = tmem_base + T::TMEM_SFB;
             const uint64_t adesc0 = make_kmajor_sw128_desc(smem0), bdesc0 = make_kmajor_sw128_desc(smem0 + T::OFF_B);
             for (int rd = 0; rd < rounds; ++rd) {
@@ -828,9 +884,10 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 }
                 tc_fence_after();
                 uint32_t fresh = 1;                         // the tile's first MMA overwrites the accumulators
-                for_live_groups(occ, occ_stride, tile.x, tile.y, kb_begin, kb_end, [&](int) {
+                if (GATE && SPARSE && landed != nullptr && occ != nullptr) wait_landed(landed, (unsigned int)tile_need[t], chunks_seen);
+                for_live_groups<SPARSE, GATE>(occ, occ_stride, tile.x, tile.y, kb_begin, kb_end, [&](int) {
 #pragma unroll 1
-                for (int half = 0; half < TC_GROUP; ++half) {
+                for (int st = 0; st < TC_GROUP; ++st) {
                     mbar_wait(full0 + 8 * stage, sphase);
                     tc_fence_after();
                     if (issuer) {
@@ -890,24 +947,13 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                         __nanosleep(200);
                     }
                 }
-                // Host-copy gate (csg_action_host): the matrix arrives in row chunks on a copy stream, which publishes the
-                // number of chunks delivered after each one; tile (I, J) reads the rows of blocks I and J only, and the
-                // host has worked out how many chunks that takes in its copy order.  The wait depends on the copy engine
-                // alone, never on another CTA.
-                if (WAITS && landed != nullptr) {
-                    const unsigned int need = (unsigned int)tile_need[t];
-                    if (chunks_seen < need) {
-                        unsigned int got;
-                        while (true) {
-                            asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(got) : "l"(landed) : "memory");
-                            if (got >= need) break;
-                            __nanosleep(500);
-                        }
-                        chunks_seen = got;
-                        asm volatile("fence.proxy.async.global;" ::: "memory");   // the bytes are read by the async proxy (TMA)
-                    }
+                // Host-copy gate (wait_landed above).
+                if (GATE && landed != nullptr) {
+                    const unsigned int before = chunks_seen;
+                    wait_landed(landed, (unsigned int)tile_need[t], chunks_seen);
+                    if (chunks_seen != before) asm volatile("fence.proxy.async.global;" ::: "memory");   // the bytes are read by the async proxy (TMA)
                 }
-                if (!(dbg & 32)) for_live_groups(occ, occ_stride, tile.x, tile.y, kb_begin, kb_end, [&](int kb0) {
+                if (!(dbg & 32)) for_live_groups<SPARSE, GATE>(occ, occ_stride, tile.x, tile.y, kb_begin, kb_end, [&](int kb0) {
                     mbar_wait(bits_empty0 + 8 * bb, bphase ^ 1);
                     const uint32_t bar = bits_full0 + 8 * bb;
                     const uint32_t dst = smem0 + T::OFF_BITS + bb * T::BITS_BUF_BYTES;

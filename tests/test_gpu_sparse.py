@@ -28,12 +28,14 @@ def csg():
 def block_sparse_poset(N, density, keep_prob, seed):
     """Index-compatible random relation matrix (not transitively closed: the definition does not need it, DESIGN.md
     A12, and a closure would refill the blocks) whose 256 x 256 blocks (I, K), I <= K, survive with probability
-    keep_prob.  Returns the packed bitset and the dense upper-triangular 0/1 matrix."""
+    keep_prob, and of the survivors' 256 x 128 and 128 x 256 half-blocks another quarter is emptied.  Returns the packed bitset and the dense upper-triangular 0/1 matrix."""
     rng = np.random.default_rng(seed)
     U = np.triu(rng.random((N, N)) < density, 1)
     nB = (N + 255) // 256
     keep = rng.random((nB, nB)) < keep_prob
     U &= np.kron(keep, np.ones((256, 256), dtype=bool))[:N, :N]
+    U &= np.kron(rng.random((nB, 2 * nB)) < 0.75, np.ones((256, 128), dtype=bool))[:N, :N]
+    U &= np.kron(rng.random((2 * nB, nB)) < 0.75, np.ones((128, 256), dtype=bool))[:N, :N]
     return csg_inputs.pack_dense(U.astype(np.uint8)), U
 
 
@@ -166,5 +168,27 @@ def test_sparse_sweep_sprinkled_sets(csg, dim, N, kmax):
             total += csg.csg_action_partial(d, N, kmax, s, 3).cpu().numpy()
         assert (total == want).all()
     finally:
+        csg.csg_set_sparse(csg.SPARSE_AUTO)
+        csg.csg_set_variant(csg.VARIANT_AUTO)
+
+
+@pytest.mark.parametrize("pipeline", ["auto", "chunked"])
+@pytest.mark.parametrize("dim,N,kmax", [(4, 20001, 3), (2, 16384, 16382), (4, 33000, 3)])
+def test_sparse_sweep_in_the_host_pipeline(csg, dim, N, kmax, pipeline):
+    """csg_action_host with the sweep forced on: the copy stream marks the occupancy rows of every chunk behind its copy,
+    while the (gated or chunked) interval kernel already runs; pinned and pageable host memory, repeated calls."""
+    _, bits = csg_inputs.make_causet(dim, N, 5 + N)
+    want = oracle.alg5_counts(bits, N, kmax)
+    pinned = torch.from_numpy(bits.view(np.int64)).pin_memory()
+    csg.csg_set_variant(csg.VARIANT_TENSOR_FP4)
+    csg.csg_set_sparse(csg.SPARSE_ON)
+    csg.csg_set_host_pipeline(csg.HOST_PIPELINE_CHUNKED if pipeline == "chunked" else csg.HOST_PIPELINE_AUTO)
+    try:
+        for host in (pinned, bits, pinned):
+            c, S = csg.csg_action_host(host, N, dim, 1.0, kmax)
+            assert (np.asarray(c) == want).all()
+            assert S == oracle.action_local(dim, N, want)
+    finally:
+        csg.csg_set_host_pipeline(csg.HOST_PIPELINE_AUTO)
         csg.csg_set_sparse(csg.SPARSE_AUTO)
         csg.csg_set_variant(csg.VARIANT_AUTO)
