@@ -651,11 +651,20 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
             };
             // Local action (kmax <= 3, every BASELINE.json config but the smeared one): no branch and no atomic per value.
             // Each thread keeps the four bins in the four bytes of one register (it sees 64 values per tile, so a byte
-            // cannot overflow): the accumulator is turned into the shift amount 8 n with one FFMA and one AND (fp4: the
-            // low 23 bits of 4n * 2 + 2^23; int8: a shift), "1 << 8n" is a PTX shl, which clamps shift amounts above 31
-            // and so yields 0 for every n >= 4, and the relation bit predicates the add.  Five instructions per value in
-            // a straight line instead of a bit test, a compare and a BSSY/BRA/BSYNC triple with a divergent slow path;
-            // the four bytes are summed over the warp once per tile (4 REDUX + at most 4 shared-memory atomics per warp).
+            // cannot overflow) and adds "1 << 8n" for every related pair; PTX shl clamps shift amounts above 31, so the
+            // term is 0 for every n >= 4.  The pass is bound by the ALU pipe (16 lanes per scheduler, 4 warps each), so
+            // what counts is ALU instructions per value -- 2.5 now, from 4:
+            //   * 8n straight from the accumulator's bit pattern by ONE multiplication (FMA pipe): the f32 accumulator
+            //     holds 4n, and 4n * 2^-148 = 8n * 2^-149 is a subnormal whose bit pattern IS the integer 8n (exact;
+            //     for 8n >= 2^23 the product is a normal number with a pattern >= 2^23, which the shift clamps away like
+            //     every other n >= 4).  Needs subnormals, i.e. no -ftz / fast-math (the build has neither).  Before:
+            //     FFMA with 2^23 + AND with the mantissa mask;
+            //   * the relation bit goes into bit 31 of the shift amount (x-th bit of ~rw moved up by an IMAD.SHL on the
+            //     FMA pipe, merged by one LOP3), so an unrelated pair shifts the 1 out as well -- no mask, no predicate;
+            //   * int8 kind: a shift of the s32 accumulator instead of the multiplication.
+            // Measured on one box, config 1 / 2 / 3: 0.2525 / 10.85 / 81.67 ms -> 0.2382 / 10.66 / 80.83 ms; without any
+            // bucketing (wrong counts) 0.200 / - / 78.3.  The four bytes are summed over the warp once per tile (4 REDUX +
+            // at most 4 shared-memory atomics per warp).
             const bool byte_bins = !DUMP && kcap <= 3 && N <= (1LL << 20);
             if (byte_bins) {
                 uint32_t packed = 0u;
@@ -667,12 +676,12 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
 #pragma unroll
                     for (int x = 0; x < 32; ++x) {
                         const uint32_t v = e == 0 ? v0[x] : v1[x];
-                        const uint32_t sh = KIND == KIND_FP4
-                                                ? (__float_as_uint(fmaf(__uint_as_float(v), 2.0f, 8388608.0f)) & 0x7FFFFFu)
-                                                : (v >> (2 * TB - 3));
+                        const uint32_t sh = KIND == KIND_FP4 ? __float_as_uint(__fmul_rn(__uint_as_float(v), __uint_as_float(2u)))
+                                                             : (v >> (2 * TB - 3));
+                        const uint32_t amt = sh | ((~rw << (31 - x)) & 0x80000000u);   // bit 31: not a related pair
                         uint32_t onehot;
-                        asm("shl.b32 %0, 1, %1;" : "=r"(onehot) : "r"(sh));      // 0 when 8 n > 31
-                        if (rw & (1u << x)) packed += onehot;
+                        asm("shl.b32 %0, 1, %1;" : "=r"(onehot) : "r"(amt));     // 0 when 8 n > 31 or unrelated
+                        packed += onehot;
                     }
                 }
 #pragma unroll
