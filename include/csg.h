@@ -62,7 +62,7 @@ enum {
 #define CSG_MAX_BATCH 65535
 
 enum {
-    CSG_VARIANT_AUTO = 0,   /* fp4 tensor variant when N > 1024, else bitset (csg_action_batch: N >= 2048) */
+    CSG_VARIANT_AUTO = 0,   /* fp4 tensor variant when N > 1024, else bitset (csg_action_batch: N > 128) */
     CSG_VARIANT_BITSET = 1, /* LOP3 AND + POPC over packed 32-bit words, register micro-tiles */
     CSG_VARIANT_TENSOR = 2, /* bits unpacked to u8 in shared memory, tcgen05.mma kind::i8, s32 accumulators in TMEM */
     CSG_VARIANT_TENSOR_FP4 = 3 /* bits unpacked to e2m1 nibbles, tcgen05.mma kind::mxf4 with unit block scales, f32
@@ -120,8 +120,11 @@ int csg_action_finish(const int64_t *counts, int64_t N, int dim, double eps, int
  * A batch of causal sets of the same size in one call (Monte-Carlo chains and ensemble averages work on many
  * sets of modest size: PAPER.md:35, 457, 490).  rel_bits DEVICE: `batch` matrices back to back, each
  * N*csg_row_stride_words(N) words; counts DEVICE: batch x (kmax+1) int64, row b = abundances of set b; S DEVICE:
- * batch doubles.  Other arguments as csg_action.  1 <= batch <= CSG_MAX_BATCH.  Sets of N < 2048 elements (under
- * CSG_VARIANT_AUTO) share ONE bitset-kernel launch (grid.y = set), larger ones run back to back on the tensor cores.
+ * batch doubles.  Other arguments as csg_action.  1 <= batch <= CSG_MAX_BATCH, batch * N < 2^31.  The whole batch is
+ * ONE launch of the interval kernel: under CSG_VARIANT_AUTO the bitset kernel (grid.y = set) for N <= 128, above that
+ * one persistent tensor-core launch that works through the tiles of all sets, deepest first across the batch (no
+ * launch and no tail per set).  Only sets whose matrix exceeds 48 MiB run back to back, one launch each (they fill
+ * the machine on their own and take the patch schedule and the block-sparse sweep).
  */
 int csg_action_batch(const uint64_t *rel_bits, int64_t N, int64_t batch, int dim, double eps, int kmax,
                      int64_t *counts, double *S, cudaStream_t stream);

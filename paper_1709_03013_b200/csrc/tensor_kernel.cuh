@@ -56,6 +56,7 @@
 namespace csg {
 
 constexpr int TC_T = 256;                  // tile edge in pairs (UMMA M = N = 256 over the CTA pair)
+constexpr int TC_SET_SHIFT = 14;           // tiles[t].x = I | set << 14: which causal set of a batch the tile belongs to (csg_action_batch)
 constexpr int TC_ROWS_A = 128;             // A rows per CTA
 constexpr int TC_ROWS_B = 128;             // B rows per CTA
 constexpr int TC_ROWS = TC_ROWS_A + TC_ROWS_B;
@@ -487,7 +488,13 @@ __device__ __forceinline__ void for_live_groups(const uint32_t* __restrict__ occ
 // KIND_I8: TB = bit of the operand byte that carries the relation bit: operands are 0 or 2^TB, every product is
 // 4^TB, the accumulator holds n_ij << 2TB; the host picks the largest TB with (N-2) << 2TB < 2^31 (exact in s32).
 // KIND_FP4: TB unused (pass 0); the f32 accumulator holds 4 n_ij, exact for n_ij < 2^22.
-// tiles[t] = {I, J}: 256-row blocks, I <= J.  Grid = 2 x (number of SM pairs), cluster (2,1,1).
+// tiles[t] = {I | set << TC_SET_SHIFT, J}: 256-row blocks, I <= J, of causal set `set` of a batch (0 for a single set).
+// A batch (csg_action_batch) is `batch` matrices of N rows back to back: set b's row i is row b N + i of the TMA view
+// and of `rel`, and its abundances go to counts + b * counts_stride with one global atomic per warp, bin and tile
+// (counts_stride = 0: a single set, bins collected in the CTA's shared-memory histogram).  The rows that a tile's
+// 256-row blocks hold beyond N belong to the next set instead of being zero-filled; they only reach accumulators of
+// rows i >= N, which the epilogue drops, and of columns j >= N, where row i's relation bits are zero padding.
+// Grid = 2 x (number of SM pairs), cluster (2,1,1).
 // progress (TCF_WAIT or TCF_GATE, may be NULL): zeroed counter of finished tiles, the drift throttle.  landed / tile_need (TCF_GATE,
 // may be NULL): the host-copy gate -- *landed = number of row chunks of `rel` the copy stream has delivered so far,
 // tile_need[t] = how many must be there before tile t may start.  dump (TCF_DUMP): ntiles x 256 x 256 int32, n_ij or -1.
@@ -497,7 +504,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                      long long stride_words, int kmax, unsigned long long* __restrict__ counts,
                      const int2* __restrict__ tiles, int ntiles, int dbg_arg, unsigned int* __restrict__ progress_arg,
                      const unsigned int* __restrict__ landed_arg, const int* __restrict__ tile_need,
-                     int* __restrict__ dump, const uint32_t* __restrict__ occ_arg, int occ_stride) {
+                     int* __restrict__ dump, const uint32_t* __restrict__ occ_arg, int occ_stride, int counts_stride) {
     constexpr bool ABLATE = (FLAGS & TCF_ABLATE) != 0, DUMP = (FLAGS & TCF_DUMP) != 0, GATE = (FLAGS & TCF_GATE) != 0;
     constexpr bool WAITS = (FLAGS & (TCF_WAIT | TCF_GATE)) != 0;        // the TMA thread may wait on global words
     constexpr bool SPARSE = (FLAGS & TCF_SPARSE) != 0 && KIND == KIND_FP4;   // block-sparse sweep: fp4 kind only (stage = column block)
@@ -605,12 +612,15 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
             if (lane == 0 && !(dbg & 64)) mbar_arrive_cluster(full_leader0 + 8 * pending);
             pending = -1;
         };
-        // Fused epilogue of tile (eI, eJ): TMEM -> registers -> mask by R[i][j], i<j -> histogram.
-        auto epilogue = [&](int eI, int eJ, int et) {
+        // Fused epilogue of tile (eI, eJ) (eI still carries the set index of a batch): TMEM -> registers -> mask by
+        // R[i][j], i<j -> histogram.
+        auto epilogue = [&](int eIs, int eJ, int et) {
             if (dbg & 64) return;
+            const int eI = eIs & ((1 << TC_SET_SHIFT) - 1), eset = eIs >> TC_SET_SHIFT;
             const long long i0 = (long long)eI * TC_T, j0 = (long long)eJ * TC_T;
             const long long i = i0 + 128 * (int)rank + 32 * q4 + lane;
-            const uint32_t* relrow32 = reinterpret_cast<const uint32_t*>(rel + (i < N ? i : 0) * stride_words);
+            const uint32_t* relrow32 = reinterpret_cast<const uint32_t*>(rel + ((long long)eset * N + (i < N ? i : 0)) * stride_words);
+            unsigned long long* const set_counts = counts + (long long)eset * counts_stride;   // batch: this set's abundances
             uint32_t relw[2];
 #pragma unroll
             for (int e = 0; e < 2; ++e) {             // relation bits first: their latency hides behind the wait
@@ -646,8 +656,8 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 // fp4: 4 n < 2^24 is an exact f32; n = low 23 bits of (4n * 0.25 + 2^23)
                 const int n = KIND == KIND_FP4 ? (int)(__float_as_uint(fmaf(__uint_as_float(v), 0.25f, 8388608.0f)) & 0x7FFFFFu)
                                                : (int)(v >> (2 * TB));
-                if (n < TC_HIST) atomicAdd(&hist[n], 1u);
-                else atomicAdd(&counts[n], 1ULL);
+                if (n < TC_HIST && counts_stride == 0) atomicAdd(&hist[n], 1u);
+                else atomicAdd(&set_counts[n], 1ULL);
             };
             // Local action (kmax <= 3, every BASELINE.json config but the smeared one): no branch and no atomic per value.
             // Each thread keeps the four bins in the four bytes of one register (it sees 64 values per tile, so a byte
@@ -687,7 +697,10 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
                     const unsigned int c = __reduce_add_sync(0xFFFFFFFFu, (packed >> (8 * k)) & 0xFFu);
-                    if (lane == 0 && c != 0u && k <= kcap) atomicAdd(&hist[k], c);
+                    if (lane == 0 && c != 0u && k <= kcap) {
+                        if (counts_stride == 0) atomicAdd(&hist[k], c);
+                        else atomicAdd(&set_counts[k], (unsigned long long)c);
+                    }
                 }
             } else {
 #pragma unroll
@@ -716,7 +729,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
             const int t = rd * G + ((rd & 1) ? (G - 1 - cl) : cl);
             if (t >= ntiles) continue;
             const int2 tile = tiles[t];
-            const int I = tile.x, J = tile.y;
+            const int I = tile.x & ((1 << TC_SET_SHIFT) - 1), J = tile.y;
             int kb_begin, kb_end;                     // stages of COLS columns, [begin, end): even count
             tile_k_range<COLS>(I, J, kb_begin, kb_end);
             const int kbA = (256 * I + 255) / COLS;   // stages kb <= kbA can hold columns k <= i
@@ -861,7 +874,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 publish_pending();
                 epilogue(epi_I, epi_J, epi_t);
             }
-            epi_I = I;
+            epi_I = tile.x;                                    // with the set index of a batch
             epi_J = J;
             epi_t = t;
         }
@@ -886,7 +899,8 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 if (t >= ntiles) continue;
                 const int2 tile = tiles[t];
                 int kb_begin, kb_end;
-                tile_k_range<COLS>(tile.x, tile.y, kb_begin, kb_end);
+                const int tI = tile.x & ((1 << TC_SET_SHIFT) - 1);
+                tile_k_range<COLS>(tI, tile.y, kb_begin, kb_end);
                 if (done_tiles > 0) {                       // both CTAs' accumulators must have been drained
                     mbar_wait(tmem_empty, ephase);
                     ephase ^= 1;
@@ -894,7 +908,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 tc_fence_after();
                 uint32_t fresh = 1;                         // the tile's first MMA overwrites the accumulators
                 if (GATE && SPARSE && landed != nullptr && occ != nullptr) wait_landed(landed, (unsigned int)tile_need[t], chunks_seen);
-                for_live_groups<SPARSE, GATE>(occ, occ_stride, tile.x, tile.y, kb_begin, kb_end, [&](int) {
+                for_live_groups<SPARSE, GATE>(occ, occ_stride, tI, tile.y, kb_begin, kb_end, [&](int) {
 #pragma unroll 1
                 for (int st = 0; st < TC_GROUP; ++st) {
                     mbar_wait(full0 + 8 * stage, sphase);
@@ -935,9 +949,11 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 const int t = rd * G + ((rd & 1) ? (G - 1 - cl) : cl);
                 if (t >= ntiles) continue;
                 const int2 tile = tiles[t];
-                const int ia = tile.x * TC_T + 128 * (int)rank, jb = tile.y * TC_T + 128 * (int)rank;
+                const int tI = tile.x & ((1 << TC_SET_SHIFT) - 1);
+                const int set_row0 = (tile.x >> TC_SET_SHIFT) * (int)N;        // first row of the tile's causal set (batch)
+                const int ia = set_row0 + tI * TC_T + 128 * (int)rank, jb = set_row0 + tile.y * TC_T + 128 * (int)rank;
                 int kb_begin, kb_end;
-                tile_k_range<COLS>(tile.x, tile.y, kb_begin, kb_end);
+                tile_k_range<COLS>(tI, tile.y, kb_begin, kb_end);
                 // Keep the clusters within TC_MAX_LEAD rounds of the average: the schedule has no barrier between rounds,
                 // and with a slow, variable epilogue (full histogram) the clusters of a patch drift apart until none of
                 // them shares row segments in L2 any more (config 4: 2.55 TB of DRAM reads per launch, L2 hit rate
@@ -962,7 +978,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                     wait_landed(landed, (unsigned int)tile_need[t], chunks_seen);
                     if (chunks_seen != before) asm volatile("fence.proxy.async.global;" ::: "memory");   // the bytes are read by the async proxy (TMA)
                 }
-                if (!(dbg & 32)) for_live_groups<SPARSE, GATE>(occ, occ_stride, tile.x, tile.y, kb_begin, kb_end, [&](int kb0) {
+                if (!(dbg & 32)) for_live_groups<SPARSE, GATE>(occ, occ_stride, tI, tile.y, kb_begin, kb_end, [&](int kb0) {
                     mbar_wait(bits_empty0 + 8 * bb, bphase ^ 1);
                     const uint32_t bar = bits_full0 + 8 * bb;
                     const uint32_t dst = smem0 + T::OFF_BITS + bb * T::BITS_BUF_BYTES;
