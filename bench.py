@@ -599,14 +599,18 @@ def run_ours(args, cfg, rank, local_rank, world):
     }
     l_ms = sum(link_ms) / len(link_ms)
     pairs = N * (N - 1) // 2
-    fp64_ops = {csg.GEOM_MINKOWSKI_4D: 11, csg.GEOM_MINKOWSKI_2D: 2, csg.GEOM_DESITTER_2D: 5}[geom]   # DADD/DMUL/DSETP per pair test (dt>0 is an integer compare)
-    fp64_peak = 64 * 148 * 1.965e9                                           # FP64 lanes/clk/SM x SMs x max clock
+    # arithmetic instructions per pair test.  3+1 Minkowski: the single-precision filter (4 FADD + 1 FMUL + 3 FFMA; the
+    # double-precision code only decides the ~1e-4 of the pairs next to the light cone) on the 128-lane FP32 pipe; the
+    # two (1+1) geometries: DADD/DMUL/DSETP on the 64-lane FP64 pipe
+    fp64_ops = {csg.GEOM_MINKOWSKI_4D: 8, csg.GEOM_MINKOWSKI_2D: 2, csg.GEOM_DESITTER_2D: 5}[geom]
+    fp64_peak = (128 if geom == csg.GEOM_MINKOWSKI_4D else 64) * 148 * 1.965e9   # lanes/clk/SM x SMs x max clock
     line["link"] = {
         "kernel": "link_kernel<%s>" % {0: "GEOM_M2", 1: "GEOM_M4", 2: "GEOM_DS2"}[geom], "kernel_ms": l_ms,
         "pair_tests_per_s": pairs / (l_ms * 1e-3), "write_gbs": N * csg.csg_row_stride_words(N) * 8 / (l_ms * 1e-3) / 1e9,
         "roofline": {"bound": "alu", "achieved": pairs * fp64_ops / (l_ms * 1e-3) / 1e12, "peak": fp64_peak / 1e12,
-                     "unit": "T fp64 instr/s", "frac": pairs * fp64_ops / (l_ms * 1e-3) / fp64_peak,
-                     "peak_source": "derived: 64 FP64 lanes/clk/SM x 148 SMs x 1.965 GHz (DESIGN.md)",
+                     "unit": "T fp32 instr/s" if geom == csg.GEOM_MINKOWSKI_4D else "T fp64 instr/s",
+                     "frac": pairs * fp64_ops / (l_ms * 1e-3) / fp64_peak,
+                     "peak_source": "derived: %d lanes/clk/SM x 148 SMs x 1.965 GHz (DESIGN.md 5.5)" % (128 if geom == csg.GEOM_MINKOWSKI_4D else 64),
                      "traffic": read_traffic("link_kernel<%s>" % {0: "GEOM_M2", 1: "GEOM_M4", 2: "GEOM_DS2"}[geom], cfg["index"])[0]},
         "e2e_from_coords": {"value": multigpu.whole_job_rate(world * triples, e2e_steps, e2e_coords_ms), "unit": UNIT,
                             "ms_per_step": e2e_coords_ms / e2e_steps, "h2d_bytes_per_step": N * dim * 8,

@@ -43,7 +43,7 @@ finish_action_kernel(const long long* __restrict__ counts, long long N, int dim,
 constexpr int TIMING_RING = 64;
 constexpr int PROGRESS_RING = 64;
 constexpr int MAX_DEVICES = 64;
-constexpr int OCC_RING = 16;
+constexpr int OCC_RING = 64;
 
 struct TileList {                       // tile schedule of one (N, shard, nshards) on the device; nshards = -batch for a batch of sets
     long long N;
@@ -357,6 +357,8 @@ static int ensure_tensor_ready(Device* D) {
     CSG_OPT_IN((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA | TCF_GATE>), s4);
     CSG_OPT_IN((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA | TCF_GATE | TCF_SPARSE>), s4);
     CSG_OPT_IN((tensor_action_kernel<KIND_FP4, 0, TCF_DUMP | TCF_SPARSE>), s4);
+    CSG_OPT_IN((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA | TCF_BATCH>), s4);
+    CSG_OPT_IN((tensor_action_kernel<KIND_I8, 7, TCF_BATCH>), s8);
     CSG_OPT_IN((tensor_peak_kernel<KIND_FP4>), s4);
     CSG_OPT_IN((tensor_peak_kernel<KIND_I8>), s8);
 #undef CSG_OPT_IN
@@ -425,13 +427,20 @@ static int launch_tensor(Device* D, int kind, const uint64_t* rel_bits, long lon
     const int tb = N - 2 < (1LL << 17) ? 7 : N - 2 < (1LL << 19) ? 6 : N - 2 < (1LL << 21) ? 5 : 4;
     if (kind == KIND_FP4) {
         // one instantiation per combination in use, so that a launch carries only the code it needs (tensor_kernel.cuh)
-        if (dump) CSG_LAUNCH((tensor_action_kernel<KIND_FP4, 0, TCF_DUMP | TCF_SPARSE>), s4);
+        if (batch > 1) CSG_LAUNCH((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA | TCF_BATCH>), s4);
+        else if (dump) CSG_LAUNCH((tensor_action_kernel<KIND_FP4, 0, TCF_DUMP | TCF_SPARSE>), s4);
         else if (landed && occ) CSG_LAUNCH((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA | TCF_GATE | TCF_SPARSE>), s4);
         else if (landed) CSG_LAUNCH((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA | TCF_GATE>), s4);
         else if (progress && occ) CSG_LAUNCH((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA | TCF_SPARSE | TCF_WAIT>), s4);
         else if (progress) CSG_LAUNCH((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA | TCF_WAIT>), s4);
         else if (occ) CSG_LAUNCH((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA | TCF_SPARSE>), s4);
         else CSG_LAUNCH((tensor_action_kernel<KIND_FP4, 0, FP4_EXTRA>), s4);
+    } else if (batch > 1) {
+        if (tb != 7) {      // batches are sets within L2 (N < 2^17), for which the int8 kind always has TB = 7
+            snprintf(g.cuda_msg, sizeof(g.cuda_msg), "batched int8 launch with N = %lld", N);
+            return CSG_E_CUDA;
+        }
+        CSG_LAUNCH((tensor_action_kernel<KIND_I8, 7, TCF_BATCH>), s8);
     } else if (dump) {
         if (tb == 7) CSG_LAUNCH((tensor_action_kernel<KIND_I8, 7, TCF_DUMP>), s8);
         else if (tb == 6) CSG_LAUNCH((tensor_action_kernel<KIND_I8, 6, TCF_DUMP>), s8);

@@ -36,7 +36,7 @@
 // throttle: the TMA thread may wait for the finished-tile counter before it starts a tile), TCF_GATE (host-copy gate of
 // csg_action_host: tiles wait for the chunks of the matrix they read; implies the throttle code), TCF_SPARSE
 // (block-sparse K sweep: the roles walk the live-group masks of the occupancy map instead of a counted loop; fp4
-// kind), TCF_DUMP (test hook csg_tile_interval_sizes: the epilogue writes every n_ij of the listed tiles instead of
+// kind), TCF_BATCH (csg_action_batch: tiles of many sets in one launch), TCF_DUMP (test hook csg_tile_interval_sizes: the epilogue writes every n_ij of the listed tiles instead of
 // bucketing it), TCF_ABLATE (only in the separate -DCSG_ABLATE build of paper_1709_03013_b200/ablate.py, never in
 // libcsg.so).
 // `dbg` (csg_set_debug of the ABLATE build; 0 and compiled out everywhere else) switches parts of the kernel off
@@ -79,7 +79,7 @@ constexpr int TC_THREADS = TC_PRODUCERS + 64;  // + the MMA warp + the TMA warp
 constexpr bool TC_WHOLE_GROUP = CSG_WHOLE_GROUP != 0;   // a producer set expands both stages of every second group
 constexpr int TC_MAX_LEAD = 1;                 // rounds a cluster may run ahead of the average (L2 sharing inside a patch)
 constexpr int TC_THROTTLE_MAX_POLLS = 1 << 15; // polls of >= 200 ns in ONE wait before a cluster stops throttling for good (see the TMA warp)
-constexpr int TCF_ABLATE = 1, TCF_WAIT = 2, TCF_DUMP = 4, TCF_GATE = 8, TCF_SPARSE = 16;   // template FLAGS of tensor_action_kernel
+constexpr int TCF_ABLATE = 1, TCF_WAIT = 2, TCF_DUMP = 4, TCF_GATE = 8, TCF_SPARSE = 16, TCF_BATCH = 32;   // template FLAGS of tensor_action_kernel
 constexpr int TC_PREFILL_GROUPS = 2;           // groups (2 stages each) of the next tile expanded before a tile's epilogue
 #ifndef CSG_TC_HIST
 #define CSG_TC_HIST 2048
@@ -491,7 +491,8 @@ __device__ __forceinline__ void for_live_groups(const uint32_t* __restrict__ occ
 // tiles[t] = {I | set << TC_SET_SHIFT, J}: 256-row blocks, I <= J, of causal set `set` of a batch (0 for a single set).
 // A batch (csg_action_batch) is `batch` matrices of N rows back to back: set b's row i is row b N + i of the TMA view
 // and of `rel`, and its abundances go to counts + b * counts_stride with one global atomic per warp, bin and tile
-// (counts_stride = 0: a single set, bins collected in the CTA's shared-memory histogram).  The rows that a tile's
+// (template flag TCF_BATCH; without it: a single set, bins collected in the CTA's shared-memory histogram -- the
+// decode and the second flush path cost 0.5 - 3 % when they were compiled into every instantiation).  The rows that a tile's
 // 256-row blocks hold beyond N belong to the next set instead of being zero-filled; they only reach accumulators of
 // rows i >= N, which the epilogue drops, and of columns j >= N, where row i's relation bits are zero padding.
 // Grid = 2 x (number of SM pairs), cluster (2,1,1).
@@ -508,6 +509,8 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
     constexpr bool ABLATE = (FLAGS & TCF_ABLATE) != 0, DUMP = (FLAGS & TCF_DUMP) != 0, GATE = (FLAGS & TCF_GATE) != 0;
     constexpr bool WAITS = (FLAGS & (TCF_WAIT | TCF_GATE)) != 0;        // the TMA thread may wait on global words
     constexpr bool SPARSE = (FLAGS & TCF_SPARSE) != 0 && KIND == KIND_FP4;   // block-sparse sweep: fp4 kind only (stage = column block)
+    constexpr bool BATCH = (FLAGS & TCF_BATCH) != 0;                    // tiles carry a set index (csg_action_batch)
+    constexpr int TILE_I_MASK = BATCH ? (1 << TC_SET_SHIFT) - 1 : -1;   // single set: tiles[t].x is the block index itself
     unsigned int* const progress = WAITS ? progress_arg : nullptr;      // compiled out of the instantiations that never wait
     const unsigned int* const landed = GATE ? landed_arg : nullptr;
     const uint32_t* const occ = SPARSE ? occ_arg : nullptr;
@@ -616,11 +619,11 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
         // R[i][j], i<j -> histogram.
         auto epilogue = [&](int eIs, int eJ, int et) {
             if (dbg & 64) return;
-            const int eI = eIs & ((1 << TC_SET_SHIFT) - 1), eset = eIs >> TC_SET_SHIFT;
+            const int eI = eIs & TILE_I_MASK, eset = BATCH ? eIs >> TC_SET_SHIFT : 0;
             const long long i0 = (long long)eI * TC_T, j0 = (long long)eJ * TC_T;
             const long long i = i0 + 128 * (int)rank + 32 * q4 + lane;
             const uint32_t* relrow32 = reinterpret_cast<const uint32_t*>(rel + ((long long)eset * N + (i < N ? i : 0)) * stride_words);
-            unsigned long long* const set_counts = counts + (long long)eset * counts_stride;   // batch: this set's abundances
+            unsigned long long* const set_counts = counts + (long long)eset * (BATCH ? counts_stride : 0);   // batch: this set's abundances
             uint32_t relw[2];
 #pragma unroll
             for (int e = 0; e < 2; ++e) {             // relation bits first: their latency hides behind the wait
@@ -656,7 +659,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 // fp4: 4 n < 2^24 is an exact f32; n = low 23 bits of (4n * 0.25 + 2^23)
                 const int n = KIND == KIND_FP4 ? (int)(__float_as_uint(fmaf(__uint_as_float(v), 0.25f, 8388608.0f)) & 0x7FFFFFu)
                                                : (int)(v >> (2 * TB));
-                if (n < TC_HIST && counts_stride == 0) atomicAdd(&hist[n], 1u);
+                if (n < TC_HIST && !BATCH) atomicAdd(&hist[n], 1u);
                 else atomicAdd(&set_counts[n], 1ULL);
             };
             // Local action (kmax <= 3, every BASELINE.json config but the smeared one): no branch and no atomic per value.
@@ -698,7 +701,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 for (int k = 0; k < 4; ++k) {
                     const unsigned int c = __reduce_add_sync(0xFFFFFFFFu, (packed >> (8 * k)) & 0xFFu);
                     if (lane == 0 && c != 0u && k <= kcap) {
-                        if (counts_stride == 0) atomicAdd(&hist[k], c);
+                        if (!BATCH) atomicAdd(&hist[k], c);
                         else atomicAdd(&set_counts[k], (unsigned long long)c);
                     }
                 }
@@ -729,7 +732,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
             const int t = rd * G + ((rd & 1) ? (G - 1 - cl) : cl);
             if (t >= ntiles) continue;
             const int2 tile = tiles[t];
-            const int I = tile.x & ((1 << TC_SET_SHIFT) - 1), J = tile.y;
+            const int I = tile.x & TILE_I_MASK, J = tile.y;
             int kb_begin, kb_end;                     // stages of COLS columns, [begin, end): even count
             tile_k_range<COLS>(I, J, kb_begin, kb_end);
             const int kbA = (256 * I + 255) / COLS;   // stages kb <= kbA can hold columns k <= i
@@ -899,7 +902,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 if (t >= ntiles) continue;
                 const int2 tile = tiles[t];
                 int kb_begin, kb_end;
-                const int tI = tile.x & ((1 << TC_SET_SHIFT) - 1);
+                const int tI = tile.x & TILE_I_MASK;
                 tile_k_range<COLS>(tI, tile.y, kb_begin, kb_end);
                 if (done_tiles > 0) {                       // both CTAs' accumulators must have been drained
                     mbar_wait(tmem_empty, ephase);
@@ -949,8 +952,8 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 const int t = rd * G + ((rd & 1) ? (G - 1 - cl) : cl);
                 if (t >= ntiles) continue;
                 const int2 tile = tiles[t];
-                const int tI = tile.x & ((1 << TC_SET_SHIFT) - 1);
-                const int set_row0 = (tile.x >> TC_SET_SHIFT) * (int)N;        // first row of the tile's causal set (batch)
+                const int tI = tile.x & TILE_I_MASK;
+                const int set_row0 = BATCH ? (tile.x >> TC_SET_SHIFT) * (int)N : 0;   // first row of the tile's causal set
                 const int ia = set_row0 + tI * TC_T + 128 * (int)rank, jb = set_row0 + tile.y * TC_T + 128 * (int)rank;
                 int kb_begin, kb_end;
                 tile_k_range<COLS>(tI, tile.y, kb_begin, kb_end);

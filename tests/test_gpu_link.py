@@ -162,3 +162,51 @@ def test_de_sitter_mean_action_approaches_einstein_hilbert(csg):
     sem = S.std(ddof=1) / math.sqrt(len(S))
     print("de Sitter N=%d: mean S = %.3f +- %.3f (S_EH = %.3f), sigma = %.3f" % (N, S.mean(), sem, s_eh, S.std(ddof=1)))
     assert abs(S.mean() - s_eh) <= 4 * sem + 0.15 * s_eh
+
+
+# --------------------------------------------------------------------------- the single-precision filter of the 4D kernel
+def _sorted_by_time(c):
+    return np.ascontiguousarray(c[np.argsort(c[:, 0], kind="stable")])
+
+
+@pytest.mark.parametrize("offset,scale", [(0.0, 1.0), (1000.0, 1.0), (-3.0e6, 1.0), (0.0, 1.0e-12), (0.0, 1.0e9),
+                                          (0.0, 1.0e17), (7.0, 3.0e-5)])
+def test_link_4d_filter_near_the_light_cone(csg, offset, scale):
+    """Pairs exactly on the cone, one ulp inside and one ulp outside it, among ordinary events; every coordinate
+    shifted and scaled so that the certainty bound of the single-precision test is tiny, huge or switched off.  The
+    kernel must take the double-precision decision for every pair: word for word equal to the linking oracle."""
+    rng = np.random.default_rng(int(abs(offset)) + 17)
+    base = csg_inputs.sprinkle(4, 700, 4242)
+    extra = []
+    for k in range(120):
+        a = base[rng.integers(0, 700)].copy()
+        d = rng.normal(size=3)
+        d /= np.linalg.norm(d)
+        r = rng.uniform(0.01, 0.3)
+        b = a.copy()
+        b[1:] += r * d
+        dist = math.sqrt(float(((b[1:] - a[1:]) ** 2).sum()))
+        dt = [dist, np.nextafter(dist, 2.0), np.nextafter(dist, 0.0), dist * (1 + 3e-8), dist * (1 - 3e-8)][k % 5]
+        b[0] = a[0] + dt
+        extra.append(b)
+    # pythagorean displacements: exactly on the cone in exact arithmetic
+    for q in range(1, 9):
+        extra.append(np.array([0.125 + 5.0 / 64 * q / 8, 3.0 / 64 * q / 8, 4.0 / 64 * q / 8, 0.0]))
+    extra.append(np.array([0.125, 0.0, 0.0, 0.0]))
+    coords = _sorted_by_time(np.vstack([base, np.array(extra)]) * scale + offset * scale)
+    want = csg_inputs.pack_dense(np.triu(oracle.link(M4, coords), 1))
+    got = gpu_link(csg, coords, M4)
+    assert (got == want).all(), np.argwhere(got != want)[:5]
+
+
+def test_link_4d_filter_nan_and_inf(csg):
+    """NaN and infinite coordinates never relate anything under the strict double-precision tests; the filter must not
+    decide them either."""
+    coords = _sorted_by_time(csg_inputs.sprinkle(4, 520, 99))
+    coords[100, 1] = np.nan
+    coords[300, 0] = np.inf
+    coords[301, 2] = -np.inf
+    with np.errstate(invalid="ignore"):
+        want = csg_inputs.pack_dense(np.triu(oracle.link(M4, coords), 1))
+    got = gpu_link(csg, coords, M4)
+    assert (got == want).all(), np.argwhere(got != want)[:5]
