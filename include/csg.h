@@ -29,8 +29,8 @@
  * csg_shutdown() must not be called while work of this library is still in flight, and it invalidates every CUDA
  * graph that captured a call of this library (the graph holds pointers into the cached workspace).
  * Per-launch scratch (the finished-tile counter of the drift throttle, the occupancy map of the block-sparse sweep)
- * comes from rings of 64 slots per device: at most 64 launches that use them may be in flight at once, and a graph
- * that captured such a launch (matrices above 512 MiB) keeps its slot, so it must not be replayed while 64 or more
+ * comes from rings of 32 slots per device: at most 32 launches that use them may be in flight at once, and a graph
+ * that captured such a launch (matrices above 512 MiB) keeps its slot, so it must not be replayed while 32 or more
  * later launches of the same kind are still running.
  */
 #ifndef CSG_H_

@@ -43,7 +43,7 @@ finish_action_kernel(const long long* __restrict__ counts, long long N, int dim,
 constexpr int TIMING_RING = 64;
 constexpr int PROGRESS_RING = 64;
 constexpr int MAX_DEVICES = 64;
-constexpr int OCC_RING = 64;
+constexpr int OCC_RING = 32;
 
 struct TileList {                       // tile schedule of one (N, shard, nshards) on the device; nshards = -batch for a batch of sets
     long long N;
@@ -475,11 +475,16 @@ static int occupancy_buffer(Device* D, int kind, long long N, long long stride, 
     const size_t words = (size_t)nB * occ_stride_words(N);
     const int slot = (int)(D->occ_next++ % OCC_RING);
     if (D->d_occ_words[slot] < words) {
-        if (D->d_occ[slot]) D->occ_retired.push_back(D->d_occ[slot]);
-        D->d_occ[slot] = nullptr;
-        D->d_occ_words[slot] = 0;
-        CSG_CUDA(cudaMalloc(&D->d_occ[slot], words * sizeof(uint32_t)));
-        D->d_occ_words[slot] = words;
+        // the whole ring at once, so that after ONE warm-up call of a size no later call of that size allocates (a call
+        // that is being captured into a CUDA graph must not)
+        for (int k = 0; k < OCC_RING; ++k) {
+            if (D->d_occ_words[k] >= words) continue;
+            if (D->d_occ[k]) D->occ_retired.push_back(D->d_occ[k]);
+            D->d_occ[k] = nullptr;
+            D->d_occ_words[k] = 0;
+            CSG_CUDA(cudaMalloc(&D->d_occ[k], words * sizeof(uint32_t)));
+            D->d_occ_words[k] = words;
+        }
     }
     *occ = D->d_occ[slot];
     return CSG_OK;

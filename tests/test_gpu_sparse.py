@@ -192,3 +192,52 @@ def test_sparse_sweep_in_the_host_pipeline(csg, dim, N, kmax, pipeline):
         csg.csg_set_host_pipeline(csg.HOST_PIPELINE_AUTO)
         csg.csg_set_sparse(csg.SPARSE_AUTO)
         csg.csg_set_variant(csg.VARIANT_AUTO)
+
+
+def test_sparse_and_batched_launches_in_a_cuda_graph(csg):
+    """After one warm-up call per size the block-sparse call (occupancy kernel + interval kernel; its occupancy map comes
+    from a ring that is allocated as a whole by the warm-up) and the batched call (one persistent launch over all sets)
+    only enqueue stream-ordered work: captured in a CUDA graph and replayed twice, with other calls in between."""
+    N, dim, kmax = 5000, 4, 3
+    sets = [csg_inputs.make_causet(dim, N, 40 + b)[1] for b in range(3)]
+    want = [oracle.alg5_counts(b, N, kmax) for b in sets]
+    d = [csg.to_device(b) for b in sets]
+    nb, Nb = 12, 700
+    small = np.stack([csg_inputs.make_causet(2, Nb, 300 + b)[1] for b in range(nb)])
+    d_small = csg.to_device(small)
+    want_small = [oracle.counts_from_bits(small[b], Nb, 3) for b in range(nb)]
+    other = csg_inputs.make_causet(dim, 1300, 77)[1]
+    d_other, want_other = csg.to_device(other), oracle.alg5_counts(other, 1300, kmax)
+    counts = [torch.zeros(kmax + 1, dtype=torch.int64, device="cuda") for _ in sets]
+    S = [torch.zeros(1, dtype=torch.float64, device="cuda") for _ in sets]
+    bc = torch.zeros((nb, 4), dtype=torch.int64, device="cuda")
+    bS = torch.zeros(nb, dtype=torch.float64, device="cuda")
+    csg.csg_set_variant(csg.VARIANT_TENSOR_FP4)
+    csg.csg_set_sparse(csg.SPARSE_ON)
+    try:
+        csg.csg_action(d[0], N, dim, 1.0, kmax, counts[0], S[0])                     # warm-ups outside the capture
+        csg.csg_action_batch(d_small, Nb, nb, 2, 1.0, 3, bc, bS)
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):
+            for b in range(3):
+                csg.csg_action(d[b], N, dim, 1.0, kmax, counts[b], S[b])
+            csg.csg_action_batch(d_small, Nb, nb, 2, 1.0, 3, bc, bS)
+        for rep in range(2):
+            for c in counts:
+                c.fill_(-1)
+            bc.fill_(-1)
+            graph.replay()
+            torch.cuda.synchronize()
+            for b in range(3):
+                assert (counts[b].cpu().numpy() == want[b]).all(), (rep, b)
+                assert float(S[b].item()) == oracle.action_local(dim, N, want[b])
+            got = bc.cpu().numpy()
+            for b in range(nb):
+                assert (got[b] == want_small[b]).all(), (rep, b)
+            c2, _ = csg.csg_action(d_other, 1300, dim, 1.0, kmax)                       # another size in between
+            torch.cuda.synchronize()
+            assert (c2.cpu().numpy() == want_other).all()
+    finally:
+        csg.csg_set_sparse(csg.SPARSE_AUTO)
+        csg.csg_set_variant(csg.VARIANT_AUTO)
