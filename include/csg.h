@@ -80,7 +80,7 @@ int64_t csg_row_stride_words(int64_t N);
  * Interval abundances and action of one causal set.  All work is enqueued on `stream`.  The FIRST call for a new
  * (device, N) builds that size's tile schedule and copies it to the device with one blocking cudaMemcpy; every later
  * call with that N -- whatever other sizes were run in between, on whatever stream -- only enqueues a memset and
- * two kernels, synchronises nothing, and can be captured in a CUDA graph.
+ * two or three kernels (small sets: one), synchronises nothing, and can be captured in a CUDA graph.
  *
  *   rel_bits DEVICE, N*csg_row_stride_words(N) words, layout above, 16-byte aligned, read only.
  *   N        number of elements, 1 <= N <= CSG_MAX_N (N = 1, 2 are valid: no triples).
@@ -150,7 +150,9 @@ int64_t csg_tile_schedule(int64_t N, int shard, int nshards, int32_t *tiles_ij, 
  * Matrices of 32 MiB and more go over in 64 row chunks, outermost chunks first, on a copy stream while ONE
  * persistent launch of the interval kernel already runs: after each chunk the copy stream publishes how many have
  * been delivered (cuStreamWriteValue32) and a tile starts when the two row blocks it reads are there
- * (overlap of the transfer with the computation).
+ * (overlap of the transfer with the computation).  With the block-sparse sweep (csg_set_sparse) the
+ * blocks of a chunk are marked by a small kernel on a third stream before the chunk is published, and the persistent
+ * launch leaves one SM pair free for those kernels.
  */
 int csg_action_host(const uint64_t *rel_bits_host, int64_t N, int dim, double eps, int kmax,
                     int64_t *counts_host, double *S_host);
