@@ -124,11 +124,12 @@ int csg_action_finish(const int64_t *counts, int64_t N, int dim, double eps, int
  * A batch of causal sets of the same size in one call (Monte-Carlo chains and ensemble averages work on many
  * sets of modest size: PAPER.md:35, 457, 490).  rel_bits DEVICE: `batch` matrices back to back, each
  * N*csg_row_stride_words(N) words; counts DEVICE: batch x (kmax+1) int64, row b = abundances of set b; S DEVICE:
- * batch doubles.  Other arguments as csg_action.  1 <= batch <= CSG_MAX_BATCH, batch * N < 2^31.  The whole batch is
- * ONE launch of the interval kernel: under CSG_VARIANT_AUTO the bitset kernel (grid.y = set) for N <= 128, above that
- * one persistent tensor-core launch that works through the tiles of all sets, deepest first across the batch (no
- * launch and no tail per set).  Only sets whose matrix exceeds 48 MiB run back to back, one launch each (they fill
- * the machine on their own and take the patch schedule and the block-sparse sweep).
+ * batch doubles.  Other arguments as csg_action.  1 <= batch <= CSG_MAX_BATCH, batch * N < 2^31.  Under
+ * CSG_VARIANT_AUTO: N <= 128: one launch of the bitset kernel (grid.y = set); above that persistent tensor-core
+ * launches that each work through the tiles of a power-of-two number of sets, deepest first across those sets (64
+ * sets: one launch; 100 sets: 64 + 32 + 4; no launch and no tail per set, and one cached tile list per power of two).
+ * Only sets whose matrix exceeds 48 MiB run back to back, one launch each (they fill the machine on their own and
+ * take the patch schedule and the block-sparse sweep).
  */
 int csg_action_batch(const uint64_t *rel_bits, int64_t N, int64_t batch, int dim, double eps, int kmax,
                      int64_t *counts, double *S, cudaStream_t stream);

@@ -705,6 +705,21 @@ static WriteValue32Fn stream_write_value32() {
     return reinterpret_cast<WriteValue32Fn>(g.write_value32);
 }
 
+// A gated launch waits inside the kernel for the chunk count; if feeding it fails half-way (a copy, an occupancy launch
+// or a stream write returns an error) the count would never arrive and the caller's synchronize would hang.  The guard
+// opens the gate on every early return: the launch then runs to its end on whatever has landed (the call returns the
+// error, its counts are not used).
+struct GateGuard {
+    unsigned int* d_landed = nullptr;
+    bool armed = false;
+    ~GateGuard() {
+        if (!armed) return;
+        const unsigned int open = 0x7FFFFFFFu;
+        cudaMemcpy(d_landed, &open, sizeof(open), cudaMemcpyHostToDevice);   // legacy default stream: does not wait for the non-blocking streams
+        cudaGetLastError();
+    }
+};
+
 static int interval_host_pipelined(Device* D, const uint64_t* rel_bits_host, uint64_t* d_bits, long long N, int kmax,
                                    int kind, int dim_hint, long long* counts, cudaStream_t stream) {
     const long long stride = csg_row_stride_words(N);
@@ -727,6 +742,7 @@ static int interval_host_pipelined(Device* D, const uint64_t* rel_bits_host, uin
     if (occ && !D->occ_stream) CSG_CUDA(cudaStreamCreateWithFlags(&D->occ_stream, cudaStreamNonBlocking));
     cudaStream_t publish = occ ? D->occ_stream : D->copy_stream;
     WriteValue32Fn write32 = kind == KIND_FP4 && g.host_pipeline != CSG_HOST_PIPELINE_CHUNKED ? stream_write_value32() : nullptr;
+    GateGuard gate;
     if (write32) {
         if (!D->d_landed) CSG_CUDA(cudaMalloc(&D->d_landed, sizeof(unsigned int)));
         // reset the gate, then ONE launch that starts at once and follows the copies
@@ -737,6 +753,8 @@ static int interval_host_pipelined(Device* D, const uint64_t* rel_bits_host, uin
             CSG_CUDA(cudaStreamWaitEvent(stream, ev_reset, 0));
             rc = launch_tensor(D, kind, d_bits, N, stride, kmax, counts, ct->d, ct->n, D->d_landed, ct->d_need, nullptr, occ, stream);
             if (rc) return rc;
+            gate.d_landed = D->d_landed;
+            gate.armed = true;
         }
     }
     for (int c = 0; c < nchunks; ++c) {
@@ -764,6 +782,7 @@ static int interval_host_pipelined(Device* D, const uint64_t* rel_bits_host, uin
             }
         }
     }
+    gate.armed = false;                 // every chunk has been published (or nothing was gated)
     return CSG_OK;
 }
 
@@ -920,15 +939,18 @@ int csg_action_batch(const uint64_t* rel_bits, int64_t N, int64_t batch, int dim
             if (rc) return rc;
         }
     } else {
-        // sets within L2: ONE persistent tensor launch over the tiles of all sets, deepest first across the batch, so
-        // that the machine is full whatever the size of a single set and there is no launch tail per set; groups of
-        // sets when the tile list would pass BATCH_MAX_TILES entries
+        // sets within L2: persistent tensor launches over the tiles of MANY sets at once, deepest first across the sets, so
+        // that the machine is full whatever the size of a single set and there is no launch tail per set.  A launch
+        // takes a power-of-two number of sets (64 sets: one launch; 100 sets: 64 + 32 + 4), so that the cached tile
+        // lists are one per power of two and N -- not one per batch size a Monte-Carlo code happens to use -- and at
+        // most BATCH_MAX_TILES entries each.
         const int kind = variant == CSG_VARIANT_TENSOR_FP4 ? KIND_FP4 : KIND_I8;
         const long long nB = (N + TC_T - 1) / TC_T, tiles_per_set = nB * (nB + 1) / 2;
-        const long long group = std::max<long long>(1, std::min<long long>(batch, BATCH_MAX_TILES / tiles_per_set));
+        const long long max_group = std::max<long long>(1, BATCH_MAX_TILES / tiles_per_set);
         CSG_CUDA(cudaMemsetAsync(c, 0, (size_t)batch * (kmax + 1) * sizeof(long long), stream));
-        for (int64_t b0 = 0; b0 < batch; b0 += group) {
-            const int nb = (int)std::min<long long>(group, batch - b0);
+        for (int64_t b0 = 0; b0 < batch;) {
+            long long nb = 1;
+            while (2 * nb <= std::min<long long>(batch - b0, max_group)) nb *= 2;
             if (nb == 1) {          // a single set left over: the ordinary launch adds into its (zeroed) histogram
                 const TileList* tl = nullptr;
                 if ((rc = ensure_tiles(D, N, 0, 1, &tl))) return rc;
@@ -936,11 +958,12 @@ int csg_action_batch(const uint64_t* rel_bits, int64_t N, int64_t batch, int dim
                                    nullptr, nullptr, nullptr, stream);
             } else {
                 const TileList* tl = nullptr;
-                if ((rc = ensure_batch_tiles(D, N, nb, &tl))) return rc;
+                if ((rc = ensure_batch_tiles(D, N, (int)nb, &tl))) return rc;
                 rc = launch_tensor(D, kind, rel_bits + b0 * set_words, N, stride, kmax, c + b0 * (kmax + 1), tl->d, tl->n, nullptr,
-                                   nullptr, nullptr, nullptr, stream, nb);
+                                   nullptr, nullptr, nullptr, stream, (int)nb);
             }
             if (rc) return rc;
+            b0 += nb;
         }
     }
     finish_action_kernel<<<(unsigned)batch, FIN_THREADS, 0, stream>>>(c, N, dim, eps, kmax, S);

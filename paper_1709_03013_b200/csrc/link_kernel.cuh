@@ -61,7 +61,7 @@ __device__ __forceinline__ bool timelike(const double* a, const double* b) {
 // 2^-16 M^2 fixes the sign of the exact expression and of the double test (and s_f > E implies |dt| > 2^-8.5 M, far
 // above the 2^-22 M uncertainty of dt_f, so the sign of dt_f is the sign of dt); everything else -- about one pair in 10^4, NaNs
 // included -- is decided by the double-precision code above, for the whole warp step.  Bit-identical by construction;
-// checked word for word against the oracle and the host generator (tests/test_gpu_link.py).  M outside [1e-10, 1e15]
+// checked word for word against the plain CPU linking code of the tests and the host generator (tests/test_gpu_link.py).  M outside [1e-10, 1e15]
 // (single-precision underflow or overflow of the squares) switches the fast path off for the tile (E = +inf).
 __device__ __forceinline__ void timelike_m4_fast(const float4& r, const float4& a, float E, bool& related, bool& unsure) {
     const float dt = __fsub_rn(a.x, r.x), dx = __fsub_rn(a.y, r.y), dy = __fsub_rn(a.z, r.z), dz = __fsub_rn(a.w, r.w);

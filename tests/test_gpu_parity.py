@@ -175,7 +175,9 @@ def test_batch_of_causal_sets(csg, dim, N, batch, eps, variant):
     counts, S = csg.csg_action_batch(d, N, batch, dim, eps, kmax)
     torch.cuda.synchronize()
     launches = csg.csg_launch_count() - launches0
-    assert launches == 2                               # interval kernel + finishing kernel, whatever the batch
+    tensor = csg.csg_effective_variant(2000) != csg.VARIANT_BITSET if variant else N > 128
+    # bitset: one launch for the batch; tensor: one per power of two in the batch size; + the finishing kernel
+    assert launches == (bin(batch).count("1") if tensor else 1) + 1
     counts, S = counts.cpu().numpy(), S.cpu().numpy()
     for b in range(batch):
         want = reference_counts(sets[b], N, kmax)
