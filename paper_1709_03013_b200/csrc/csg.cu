@@ -340,7 +340,7 @@ constexpr int FP4_EXTRA = 0;
 // Dynamic shared memory opt-in of the tensor kernels and the occupancy of the instantiation that may wait.
 static int ensure_tensor_ready(Device* D) {
     if (D->attr_set) return CSG_OK;
-    const int s8 = TcTraits<KIND_I8>::SMEM_BYTES, s4 = TcTraits<KIND_FP4>::SMEM_BYTES;
+    const int s8 = TcTraits<KIND_I8>::smem_bytes(TC_HIST_WHOLE), s4 = TcTraits<KIND_FP4>::smem_bytes(TC_HIST_WHOLE);   // the most a launch may ask for
 #define CSG_OPT_IN(kernel, bytes) CSG_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes))
     CSG_OPT_IN((tensor_action_kernel<KIND_I8, 7>), s8);
     CSG_OPT_IN((tensor_action_kernel<KIND_I8, 6>), s8);
@@ -419,9 +419,12 @@ static int launch_tensor(Device* D, int kind, const uint64_t* rel_bits, long lon
         CSG_CUDA(cudaMemsetAsync(progress, 0, sizeof(unsigned int), stream));
     }
     unsigned long long* c64 = reinterpret_cast<unsigned long long*>(counts);
-    const int s8 = TcTraits<KIND_I8>::SMEM_BYTES, s4 = TcTraits<KIND_FP4>::SMEM_BYTES;
+    // private histogram: the large one only for launches that can reach bins beyond the small one (tensor_kernel.cuh: TC_HIST)
+    const long long kcap = std::min<long long>(kmax, std::max<long long>(N - 2, 0));
+    const int hist_bins = (dump == nullptr && batch == 1 && kcap >= TC_HIST) ? TC_HIST_WHOLE : TC_HIST;
+    const int s8 = TcTraits<KIND_I8>::smem_bytes(hist_bins), s4 = TcTraits<KIND_FP4>::smem_bytes(hist_bins);
 #define CSG_LAUNCH(KERNEL, SMEM) \
-    KERNEL<<<grid, TC_THREADS, SMEM, stream>>>(*map, rel_bits, N, stride, kmax, c64, d_tiles, ntiles, g.debug, progress, landed, tile_need, dump, occ, occ_stride_words(N), counts_stride)
+    KERNEL<<<grid, TC_THREADS, SMEM, stream>>>(*map, rel_bits, N, stride, kmax, c64, d_tiles, ntiles, g.debug, progress, landed, tile_need, dump, occ, occ_stride_words(N), counts_stride, hist_bins)
     // int8: operand bit TB: the accumulator holds n_ij << 2TB and n_ij <= N-2, so TB is the largest with
     // (N-2) << 2TB < 2^31; TB = 7 turns every unpack shift into a left shift (FMA pipe).
     const int tb = N - 2 < (1LL << 17) ? 7 : N - 2 < (1LL << 19) ? 6 : N - 2 < (1LL << 21) ? 5 : 4;

@@ -28,7 +28,7 @@
 //   * the open range i<k<j costs nothing in the steady state: only the stages that overlap block I need the k>i
 //     mask and only those that overlap block J the k<j mask;
 //   * fused epilogue by the producer warps: tcgen05.ld of their CTA's accumulators, bit R[i][j] (and i<j), n_ij
-//     into a privatised shared-memory histogram (bins < TC_HIST) or straight into the global counts (higher bins,
+//     into a privatised shared-memory histogram (the launch's hist_bins) or straight into the global counts (higher bins,
 //     smeared action only).  The first two groups of the NEXT tile are expanded before the epilogue of a tile, so
 //     the tensor cores restart as soon as the accumulators are drained.  No N x N count matrix ever reaches HBM.
 //
@@ -81,14 +81,16 @@ constexpr int TC_MAX_LEAD = 1;                 // rounds a cluster may run ahead
 constexpr int TC_THROTTLE_MAX_POLLS = 1 << 15; // polls of >= 200 ns in ONE wait before a cluster stops throttling for good (see the TMA warp)
 constexpr int TCF_ABLATE = 1, TCF_WAIT = 2, TCF_DUMP = 4, TCF_GATE = 8, TCF_SPARSE = 16, TCF_BATCH = 32;   // template FLAGS of tensor_action_kernel
 constexpr int TC_PREFILL_GROUPS = 2;           // groups (2 stages each) of the next tile expanded before a tile's epilogue
-#ifndef CSG_TC_HIST
-#define CSG_TC_HIST 2048
-#endif
-// Privatised low bins per CTA (u32, shared memory); higher bins (full-histogram epilogue only) go to the global histogram
-// with one red.add per value.  Measured with 12288 bins (48 KiB, all that is left beside the operand ring): the
-// full-histogram configs gain < 1 % and config 3 loses 2 % (81.8 -> 83.5 ms: the L1 that remains next to 213 KiB of
-// shared memory is too small for the epilogue's relation words and the per-tile loads), so 2048 stays.
-constexpr int TC_HIST = CSG_TC_HIST;
+// Privatised low bins per CTA (u32, shared memory, the last region of the dynamic window; the launch says how many).
+// Higher bins -- whole-histogram launches (smeared action) only -- go to the global histogram with one red.add per
+// value, and scattered global atomics run at 185 G/s on the device (1.57 clk each per SM, measured; u32 and u64
+// alike): a 2D set at N = 262144 sends 1.5e10 of them, 8 % of the launch.  In a 2D order the share of related pairs with
+// n_ij < B is about 4x(-ln x - 1), x = B/N: 12 % at B = 2048, 39 % at B = 12288 (48 KiB: what is left of the 227 KiB
+// beside the operand ring).  Measured: config 4 835.6 -> 819.6 ms, config 5 94.1 -> 92.4 ms with 12288 bins -- but
+// config 3, whose epilogue needs four bins, 81.8 -> 83.5 ms (too little L1 is left beside 213 KiB of shared memory).  So
+// the host gives 12288 bins to launches that can reach bins >= 2048 and 2048 to all others.
+constexpr int TC_HIST = 2048;              // every launch has at least these
+constexpr int TC_HIST_WHOLE = 12288;       // launches with kmax >= TC_HIST
 
 // The two operand encodings of the kernel.
 //   KIND_I8 : one relation bit -> one u8 (0 or 1 << TB); tcgen05.mma kind::i8, K = 32 per instruction, s32
@@ -121,9 +123,10 @@ struct TcTraits {
     static constexpr int BITS_BUFS = 4;
     static constexpr int NUM_BARS = 2 * STAGES + 2 + 2 * BITS_BUFS;
     static constexpr int OFF_BITS = STAGES * STAGE_BYTES;
-    static constexpr int OFF_HIST = OFF_BITS + BITS_BUFS * BITS_BUF_BYTES;
-    static constexpr int OFF_BARS = OFF_HIST + TC_HIST * 4;
-    static constexpr int SMEM_BYTES = OFF_BARS + 8 * NUM_BARS + 16 + 1024;    // + TMEM slot + alignment slack
+    static constexpr int OFF_BARS = OFF_BITS + BITS_BUFS * BITS_BUF_BYTES;
+    static constexpr int OFF_HIST = (OFF_BARS + 8 * NUM_BARS + 16 + 15) & ~15;  // after the barriers and the TMEM slot
+    static constexpr int smem_bytes(int hist_bins) { return OFF_HIST + hist_bins * 4 + 1024; }   // + alignment slack
+    static constexpr int SMEM_BYTES = smem_bytes(TC_HIST);
     static constexpr int TMEM_COLS = KIND == KIND_FP4 ? 512 : 256;            // fp4: + scale factors + the A ring
     // fp4: the A operand never touches shared memory.  The A producers write their expanded rows straight into
     // TMEM (lane = row, 32-bit column j of a K=64 slice = bytes 4j..4j+3 of the row's 32-byte slice, the same
@@ -496,6 +499,8 @@ __device__ __forceinline__ void for_live_groups(const uint32_t* __restrict__ occ
 // 256-row blocks hold beyond N belong to the next set instead of being zero-filled; they only reach accumulators of
 // rows i >= N, which the epilogue drops, and of columns j >= N, where row i's relation bits are zero padding.
 // Grid = 2 x (number of SM pairs), cluster (2,1,1).
+// hist_bins: bins of the CTA's private histogram (TC_HIST or TC_HIST_WHOLE; the launch's dynamic shared memory is
+// TcTraits::smem_bytes(hist_bins)).
 // progress (TCF_WAIT or TCF_GATE, may be NULL): zeroed counter of finished tiles, the drift throttle.  landed / tile_need (TCF_GATE,
 // may be NULL): the host-copy gate -- *landed = number of row chunks of `rel` the copy stream has delivered so far,
 // tile_need[t] = how many must be there before tile t may start.  dump (TCF_DUMP): ntiles x 256 x 256 int32, n_ij or -1.
@@ -505,7 +510,8 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                      long long stride_words, int kmax, unsigned long long* __restrict__ counts,
                      const int2* __restrict__ tiles, int ntiles, int dbg_arg, unsigned int* __restrict__ progress_arg,
                      const unsigned int* __restrict__ landed_arg, const int* __restrict__ tile_need,
-                     int* __restrict__ dump, const uint32_t* __restrict__ occ_arg, int occ_stride, int counts_stride) {
+                     int* __restrict__ dump, const uint32_t* __restrict__ occ_arg, int occ_stride, int counts_stride,
+                     int hist_bins) {
     constexpr bool ABLATE = (FLAGS & TCF_ABLATE) != 0, DUMP = (FLAGS & TCF_DUMP) != 0, GATE = (FLAGS & TCF_GATE) != 0;
     constexpr bool WAITS = (FLAGS & (TCF_WAIT | TCF_GATE)) != 0;        // the TMA thread may wait on global words
     constexpr bool SPARSE = (FLAGS & TCF_SPARSE) != 0 && KIND == KIND_FP4;   // block-sparse sweep: fp4 kind only (stage = column block)
@@ -531,7 +537,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
     const uint32_t tmem_full = empty0 + 8 * T::STAGES, tmem_empty = tmem_full + 8;
     const uint32_t bits_full0 = tmem_empty + 8, bits_empty0 = bits_full0 + 8 * T::BITS_BUFS;
 
-    for (int b = tid; b < TC_HIST; b += TC_THREADS) hist[b] = 0u;
+    for (int b = tid; b < hist_bins; b += TC_THREADS) hist[b] = 0u;
     if (tid == 0) {
         for (int s = 0; s < T::STAGES; ++s) {
             mbar_init(full0 + 8 * s, TC_PRODUCER_WARPS);       // leader's copy is used: 8 warps of one producer set x 2 CTAs
@@ -659,7 +665,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
                 // fp4: 4 n < 2^24 is an exact f32; n = low 23 bits of (4n * 0.25 + 2^23)
                 const int n = KIND == KIND_FP4 ? (int)(__float_as_uint(fmaf(__uint_as_float(v), 0.25f, 8388608.0f)) & 0x7FFFFFu)
                                                : (int)(v >> (2 * TB));
-                if (n < TC_HIST && !BATCH) atomicAdd(&hist[n], 1u);
+                if (n < hist_bins && !BATCH) atomicAdd(&hist[n], 1u);
                 else atomicAdd(&set_counts[n], 1ULL);
             };
             // Local action (kmax <= 3, every BASELINE.json config but the smeared one): no branch and no atomic per value.
@@ -997,7 +1003,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
     // ---- teardown: flush the privatised histogram, release TMEM once neither CTA can touch the other any more
     tc_fence_before();
     __syncthreads();
-    for (int b = tid; b < TC_HIST && b <= kmax; b += TC_THREADS)
+    for (int b = tid; b < hist_bins && b <= kmax; b += TC_THREADS)
         if (hist[b]) atomicAdd(&counts[b], (unsigned long long)hist[b]);
     cluster_sync_all();
     tc_fence_after();
