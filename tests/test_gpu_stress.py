@@ -23,17 +23,21 @@ def csg():
     return m
 
 
+@pytest.mark.parametrize("sparse", [0, 1])
 @pytest.mark.parametrize("throttle", [0, 1])
 @pytest.mark.parametrize("dim,N,reps", [(2, 16384, 12), (4, 16384, 8), (2, 9000, 12)])
-def test_repeated_full_histograms(csg, dim, N, reps, throttle):
+def test_repeated_full_histograms(csg, dim, N, reps, throttle, sparse):
     """throttle = 1 (CSG_THROTTLE_ON): the instantiation of the fp4 kernel whose TMA threads wait on the finished-tile
     counter -- the one BASELINE.json configs[4] runs -- on the device-resident call, and together with the copy gate
-    on the host call."""
+    on the host call.  sparse = 1 (CSG_SPARSE_ON): the instantiations in which the three roles of the kernel each walk
+    the live-group masks of the occupancy map (the headline launch), incl. the gated host pipeline whose occupancy rows
+    are written while the kernel runs."""
     _, bits = csg_inputs.make_causet(dim, N, 777 + N)
     want = oracle.alg5_counts(bits, N, N - 2)
     d = csg.to_device(bits)
     pinned = torch.from_numpy(bits.view(np.int64)).pin_memory()
     csg.csg_set_throttle(throttle)
+    csg.csg_set_sparse(sparse)
     try:
         for r in range(reps):
             c, _ = csg.csg_action(d, N, dim, 1.0, N - 2)
@@ -43,6 +47,7 @@ def test_repeated_full_histograms(csg, dim, N, reps, throttle):
             assert (ch == want).all(), ("host", r)
     finally:
         csg.csg_set_throttle(0)
+        csg.csg_set_sparse(0)
 
 
 @pytest.mark.slow
