@@ -58,7 +58,8 @@ enum {
     CSG_E_CUDA = -8,        /* a CUDA call failed; csg_strerror(CSG_E_CUDA) carries its text */
     CSG_E_VARIANT = -9,     /* unknown variant id or mode */
     CSG_E_SHARD = -10,      /* nshards < 1 or shard outside [0, nshards) */
-    CSG_E_GEOMETRY = -11    /* unknown geometry id */
+    CSG_E_GEOMETRY = -11,   /* unknown geometry id */
+    CSG_E_NOALLOC_LIMIT = -12 /* csg_action_noalloc: N > CSG_NOALLOC_MAX_N or kmax > CSG_NOALLOC_MAX_KMAX */
 };
 
 #define CSG_MAX_N (1 << 22)
@@ -99,6 +100,29 @@ int64_t csg_row_stride_words(int64_t N);
  */
 int csg_action(const uint64_t *rel_bits, int64_t N, int dim, double eps, int kmax, int64_t *counts,
                double *S, cudaStream_t stream);
+
+/*
+ * csg_action for callers that cannot allocate: code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc.  Same arguments, same results (counts bit-identical, S identical) as csg_action, for small causal
+ * sets only:  N <= CSG_NOALLOC_MAX_N and kmax <= CSG_NOALLOC_MAX_KMAX, else CSG_E_NOALLOC_LIMIT (nothing is enqueued).
+ * It runs the fused small-set launch of the bitset variant (AND + POPC tiles, histogram and action in ONE kernel,
+ * whatever csg_set_variant says) with that launch's workspace -- 1024 accumulator bins and the last-CTA ticket -- in a
+ * file-scope `static __device__` array of 8448 bytes instead of a cudaMalloc'ed buffer; every GPU that loads
+ * libcsg.so holds those bytes until the process exits.  The call enqueues one memset of that array (it keeps the last
+ * call's contents) and one kernel on `stream`, synchronises nothing, and calls no cudaMalloc, cudaFree or allocating
+ * library routine, on its first use either.
+ * ALL calls on a device share the one array: calls that overlap on the GPU (two streams, two host threads' launches
+ * in flight together, a captured graph replayed next to an eager call) race on it and return garbage.  Keep them on one
+ * stream or otherwise ordered.
+ * csg_noalloc_setup(): optional; resolves the array's device address (cudaGetSymbolAddress) and reads the SM count for
+ * the CURRENT device, once per device.  csg_action_noalloc does the same on its first call per device; call the
+ * set-up yourself, with the device current, before a capture or a loop that must not touch the CUDA module loader.
+ */
+#define CSG_NOALLOC_MAX_N 4096
+#define CSG_NOALLOC_MAX_KMAX 1023
+int csg_noalloc_setup(void);
+int csg_action_noalloc(const uint64_t *rel_bits, int64_t N, int dim, double eps, int kmax, int64_t *counts,
+                       double *S, cudaStream_t stream);
 
 /*
  * The same path in two halves, for one causal set whose pair tiles are split over several GPUs (the paper

@@ -8,7 +8,8 @@ Functions carry the C names: csg_action, csg_action_host, csg_interval_sizes, cs
 csg_set_variant, csg_effective_variant, csg_set_kernel_timing, csg_last_kernel_ms, csg_kernel_ms_history,
 csg_launch_count, csg_action_partial, csg_action_finish, csg_tile_schedule, csg_link, csg_causet_action_host,
 csg_last_link_ms, csg_action_batch, csg_tile_interval_sizes, csg_set_throttle, csg_set_sparse, csg_set_host_pipeline,
-csg_occupancy_stride_words, csg_block_occupancy, csg_measure_peak, csg_strerror, csg_shutdown.
+csg_occupancy_stride_words, csg_block_occupancy, csg_measure_peak, csg_noalloc_setup, csg_action_noalloc,
+csg_strerror, csg_shutdown.
 """
 import ctypes
 import os
@@ -31,7 +32,7 @@ EXPORTS = [
     "csg_launch_count", "csg_action_partial", "csg_action_finish", "csg_tile_schedule", "csg_link",
     "csg_causet_action_host", "csg_last_link_ms", "csg_action_batch", "csg_tile_interval_sizes", "csg_set_throttle",
     "csg_measure_peak", "csg_set_sparse", "csg_occupancy_stride_words", "csg_block_occupancy",
-    "csg_set_host_pipeline",
+    "csg_set_host_pipeline", "csg_noalloc_setup", "csg_action_noalloc",
     "csg_strerror", "csg_shutdown",
 ]
 
@@ -87,6 +88,10 @@ def load():
     lib.csg_set_throttle.restype = ci
     lib.csg_set_sparse.argtypes = [ci]
     lib.csg_set_sparse.restype = ci
+    lib.csg_noalloc_setup.argtypes = []
+    lib.csg_noalloc_setup.restype = ci
+    lib.csg_action_noalloc.argtypes = [vp, i64, ci, dbl, ci, vp, vp, vp]
+    lib.csg_action_noalloc.restype = ci
     lib.csg_set_host_pipeline.argtypes = [ci]
     lib.csg_set_host_pipeline.restype = ci
     lib.csg_occupancy_stride_words.argtypes = [i64]
@@ -158,6 +163,25 @@ def csg_action(rel_bits, N, dim, eps, kmax, counts=None, S=None, stream=None):
         S = torch.empty(1, dtype=torch.float64, device=rel_bits.device)
     _check(lib.csg_action(rel_bits.data_ptr(), int(N), int(dim), float(eps), int(kmax), counts.data_ptr(),
                           S.data_ptr(), _stream_handle(stream)))
+    return counts, S
+
+
+NOALLOC_MAX_N, NOALLOC_MAX_KMAX = 4096, 1023
+
+
+def csg_noalloc_setup():
+    _check(load().csg_noalloc_setup())
+
+
+def csg_action_noalloc(rel_bits, N, dim, eps, kmax, counts, S, stream=None):
+    """int csg_action_noalloc(rel_bits, N, dim, eps, kmax, counts, S, stream): csg_action for small sets with its scratch
+    in a static device array (include/csg.h).  The caller passes every buffer (device tensors): nothing is allocated
+    here either.  Returns (counts, S); nothing is synchronised."""
+    lib = load()
+    assert rel_bits.is_cuda and rel_bits.element_size() == 8 and rel_bits.is_contiguous()
+    assert counts.is_cuda and counts.element_size() == 8 and S.is_cuda and S.element_size() == 8
+    _check(lib.csg_action_noalloc(rel_bits.data_ptr(), int(N), int(dim), float(eps), int(kmax), counts.data_ptr(),
+                                  S.data_ptr(), _stream_handle(stream)))
     return counts, S
 
 

@@ -860,6 +860,52 @@ static void release_device(Device* D) {
     delete D;
 }
 
+// ---------------------------------------------------------------------------------------------- csg_action_noalloc
+// Scratch of the entry point that allocates nothing (include/csg.h): the workspace of the fused small-set launch
+// (bitset_kernel.cuh: BitsetFusedWs = 1024 bins + the last-CTA ticket, 8200 bytes) in a file-scope device array instead of
+// a cudaMalloc'ed buffer.  Every GPU that loads libcsg.so holds these 8448 bytes until the process exits.  In host
+// code the NAME of the array is a host-side stand-in, not a device address: the kernel gets the address that
+// cudaGetSymbolAddress returned for the device it runs on (noalloc_setup, once per device, with that device current).
+constexpr size_t NOALLOC_SCRATCH_BYTES = 8448;
+static_assert(sizeof(BitsetFusedWs) <= NOALLOC_SCRATCH_BYTES, "static scratch too small for the fused workspace");
+static __device__ __align__(256) unsigned char csg_noalloc_scratch[NOALLOC_SCRATCH_BYTES];
+
+struct NoallocDevice {                  // plain static table: this path must not touch the heap-allocated Device state
+    BitsetFusedWs* ws = nullptr;        // device address of csg_noalloc_scratch on this device
+    int sm_count = 0;
+};
+static NoallocDevice g_noalloc[MAX_DEVICES];
+
+// Set-up for the CURRENT device: device address of the scratch array and the SM count.  No allocation.
+static int noalloc_setup(NoallocDevice** out) {
+    int ord = 0;
+    CSG_CUDA(cudaGetDevice(&ord));
+    if (ord < 0 || ord >= MAX_DEVICES) {
+        snprintf(g.cuda_msg, sizeof(g.cuda_msg), "device ordinal %d out of range", ord);
+        return CSG_E_CUDA;
+    }
+    NoallocDevice& nd = g_noalloc[ord];
+    if (!nd.ws) {
+        int major = 0, sms = 0;
+        CSG_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, ord));
+        CSG_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, ord));
+        if (major != 10) {
+            snprintf(g.cuda_msg, sizeof(g.cuda_msg), "device is sm_%dx; libcsg is built for sm_100a only", major);
+            return CSG_E_CUDA;
+        }
+        void* ptr = nullptr;
+        CSG_CUDA(cudaGetSymbolAddress(&ptr, csg_noalloc_scratch));
+        if (!ptr || (reinterpret_cast<uintptr_t>(ptr) & 255)) {
+            snprintf(g.cuda_msg, sizeof(g.cuda_msg), "cudaGetSymbolAddress returned an unusable address for the static scratch");
+            return CSG_E_CUDA;
+        }
+        nd.sm_count = sms;
+        nd.ws = reinterpret_cast<BitsetFusedWs*>(ptr);
+    }
+    *out = &nd;
+    return CSG_OK;
+}
+
 }  // namespace csg
 
 using namespace csg;
@@ -1132,6 +1178,38 @@ int csg_tile_interval_sizes(const uint64_t* rel_bits, int64_t N, const int32_t* 
     return rc;
 }
 
+int csg_noalloc_setup(void) {
+    std::lock_guard<std::mutex> lock(g.mu);
+    NoallocDevice* nd = nullptr;
+    return noalloc_setup(&nd);
+}
+
+int csg_action_noalloc(const uint64_t* rel_bits, int64_t N, int dim, double eps, int kmax, int64_t* counts, double* S,
+                       cudaStream_t stream) {
+    std::lock_guard<std::mutex> lock(g.mu);
+    int rc = validate(rel_bits, N, dim, eps, kmax, counts, S);
+    if (rc) return rc;
+    if (N > CSG_NOALLOC_MAX_N || kmax > CSG_NOALLOC_MAX_KMAX) return CSG_E_NOALLOC_LIMIT;
+    if ((reinterpret_cast<uintptr_t>(rel_bits) & 15) || (reinterpret_cast<uintptr_t>(counts) & 7) ||
+        (reinterpret_cast<uintptr_t>(S) & 7))
+        return CSG_E_ALIGN;
+    NoallocDevice* nd = nullptr;
+    if ((rc = noalloc_setup(&nd))) return rc;          // a lookup after the first call on this device
+    // Every call shares the scratch and it keeps what the last call left there (zeros after a completed launch, anything
+    // after a failed or aborted one): clear the bins and the ticket on the caller's stream first.
+    CSG_CUDA(cudaMemsetAsync(nd->ws, 0, sizeof(BitsetFusedWs), stream));
+    const long long stride = csg_row_stride_words(N);
+    const long long nb = (N + BS_T - 1) / BS_T;
+    const long long ntiles = nb * (nb + 1) / 2;
+    const int grid = (int)std::max<long long>(1, std::min<long long>(ntiles, (long long)nd->sm_count * 2));
+    bitset_action_kernel<<<grid, BS_THREADS, 0, stream>>>(reinterpret_cast<const uint32_t*>(rel_bits), N, stride * 2, kmax,
+                                                           reinterpret_cast<unsigned long long*>(counts), nb, ntiles, 0, 1, 0,
+                                                           0, nd->ws, dim, eps, S);
+    CSG_CUDA(cudaGetLastError());
+    ++g.launches;
+    return CSG_OK;
+}
+
 int csg_set_variant(int variant) {
     std::lock_guard<std::mutex> lock(g.mu);
     if (variant < CSG_VARIANT_AUTO || variant > CSG_VARIANT_TENSOR_FP4)
@@ -1288,6 +1366,8 @@ const char* csg_strerror(int code) {
         case CSG_E_VARIANT: return "unknown variant or mode";
         case CSG_E_GEOMETRY: return "geometry must be CSG_GEOM_MINKOWSKI_2D, _MINKOWSKI_4D or _DESITTER_2D";
         case CSG_E_SHARD: return "shard must satisfy 0 <= shard < nshards";
+        case CSG_E_NOALLOC_LIMIT:
+            return "csg_action_noalloc: N > CSG_NOALLOC_MAX_N (4096) or kmax > CSG_NOALLOC_MAX_KMAX (1023): beyond its static scratch; use csg_action";
         default: return "unknown error code";
     }
 }

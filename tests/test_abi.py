@@ -57,8 +57,8 @@ def test_row_stride(lib):
 
 
 def test_strerror_distinct(lib):
-    texts = {csg.csg_strerror(c) for c in range(0, -12, -1)}
-    assert len(texts) == 12 and "unknown" in csg.csg_strerror(-99)
+    texts = {csg.csg_strerror(c) for c in range(0, -13, -1)}
+    assert len(texts) == 13 and "unknown" in csg.csg_strerror(-99)
 
 
 def test_variant_setter(lib):
