@@ -362,6 +362,16 @@ static int ensure_tensor_ready(Device* D) {
     CSG_OPT_IN((tensor_peak_kernel<KIND_FP4>), s4);
     CSG_OPT_IN((tensor_peak_kernel<KIND_I8>), s8);
 #undef CSG_OPT_IN
+    // Kernels that the host-matrix pipeline launches WHILE its gated interval kernel is already running (and waiting for
+    // the chunks the host is still enqueueing) must be loaded beforehand: with CUDA's lazy module loading the first
+    // launch of a kernel loads it, loading may synchronise the context, and that would wait for the gated kernel, which
+    // waits for the host -- csg_action_host as the FIRST call of a process hung exactly there.  cudaFuncGetAttributes
+    // forces the load.
+    {
+        cudaFuncAttributes fa;
+        CSG_CUDA(cudaFuncGetAttributes(&fa, occupancy_kernel));
+        CSG_CUDA(cudaFuncGetAttributes(&fa, finish_action_kernel));
+    }
     // The drift throttle makes clusters wait for tiles finished by OTHER clusters, which is only safe when the whole
     // grid is resident at once: ask the runtime how many CTA pairs of that instantiation fit on the device right now.
     cudaLaunchConfig_t cfg = {};

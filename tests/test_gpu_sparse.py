@@ -241,3 +241,37 @@ def test_sparse_and_batched_launches_in_a_cuda_graph(csg):
     finally:
         csg.csg_set_sparse(csg.SPARSE_AUTO)
         csg.csg_set_variant(csg.VARIANT_AUTO)
+
+
+FIRST_CALL_SCRIPT = r"""
+import sys
+sys.path.insert(0, sys.argv[1])
+import numpy as np, torch
+import csg_inputs, paper_1709_03013_b200 as csg
+csg.load()
+N, dim, kmax = 16384, 4, 3
+_, bits = csg_inputs.make_causet(dim, N, 4711)
+csg.csg_set_variant(csg.VARIANT_TENSOR_FP4)
+csg.csg_set_sparse(csg.SPARSE_ON)
+c_host, S_host = csg.csg_action_host(bits, N, dim, 1.0, kmax)          # the FIRST call of this process into the library
+c_dev, S_dev = csg.csg_action(csg.to_device(bits), N, dim, 1.0, kmax)
+torch.cuda.synchronize()
+assert (np.asarray(c_host) == c_dev.cpu().numpy()).all() and S_host == float(S_dev.item())
+print("FIRST_CALL_OK", [int(x) for x in c_host])
+"""
+
+
+def test_host_pipeline_as_the_first_call_of_a_process(csg):
+    """csg_action_host with the block-sparse sweep as the very first library call of a fresh process: the occupancy
+    kernels it launches while the gated interval kernel already waits for the copies must have been loaded before that
+    kernel starts (CUDA loads kernels lazily, loading may synchronise the context: this call once hung for good).  Run
+    in a subprocess under a timeout, so that a hang fails instead of stalling the suite."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, "-c", FIRST_CALL_SCRIPT, root], capture_output=True, text=True, timeout=240)
+    assert r.returncode == 0 and "FIRST_CALL_OK" in r.stdout, (r.returncode, r.stdout[-500:], r.stderr[-1500:])
+    _, bits = csg_inputs.make_causet(4, 16384, 4711)
+    want = oracle.alg5_counts(bits, 16384, 3)
+    assert str([int(x) for x in want]) in r.stdout
