@@ -546,11 +546,13 @@ def run_ours(args, cfg, rank, local_rank, world):
             frac_exec = executed_group_fraction(occ.cpu().numpy(), N)
         roofline["executed_fraction"] = frac_exec
         roofline["frac_executed"] = roofline["frac"] * frac_exec
+        roofline["frac_of_hw_executed"] = roofline["frac_of_hw"] * frac_exec
         roofline["executed_note"] = ("block-sparse K sweep (occupancy pass inside the timed kernel span): two-stage groups whose "
                                      "U or L blocks are empty are neither fetched, expanded nor multiplied; executed_fraction "
                                      "of the dense sweep's groups remains; `achieved`/`frac` count all C(N,3) algorithmic "
                                      "tests, `frac_executed` = frac x executed_fraction is the tensor cores' own utilisation "
-                                     "against the same measured peak")
+                                     "against the same measured peak (never above 1), `frac_of_hw_executed` the same against "
+                                     "16384 MAC/clk/SM at the sampled clock")
     roofline["hbm_gbs_algorithmic"] = (N * csg.csg_row_stride_words(N) * 8) / (k_ms * 1e-3) / 1e9
     # what the paper's method would execute of these tests (it skips unrelated pairs, PAPER.md:407 l.4-5)
     roofline["useful_work_ratio"] = useful_work_ratio(bits, N)
