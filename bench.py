@@ -327,7 +327,10 @@ def run_ours(args, cfg, rank, local_rank, world):
         raise SystemExit("bench.py: no CUDA device; libcsg has no CPU fallback")
     torch.cuda.set_device(local_rank)
     dist = None
-    if world > 1:
+    # `--shard tiles` under torchrun with ONE rank still takes the sharded code path (partial -> all-reduce -> finish in a
+    # one-rank NCCL group): all that a single GPU can show of it
+    under_torchrun = "RANK" in os.environ and "MASTER_ADDR" in os.environ
+    if world > 1 or (args.shard == "tiles" and under_torchrun):
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     if csg._build.needs_build():
@@ -341,7 +344,7 @@ def run_ours(args, cfg, rank, local_rank, world):
     csg.csg_set_host_pipeline(csg.HOST_PIPELINE_CHUNKED if args.host_pipeline == "chunked" else csg.HOST_PIPELINE_AUTO)
 
     N, dim, eps, kmax = cfg["N"], cfg["dim"], cfg["eps"], cfg["kmax"]
-    tiles_mode = args.shard == "tiles" and world > 1
+    tiles_mode = args.shard == "tiles" and dist is not None
     seed = cfg["seed"] if tiles_mode else multigpu.ensemble_seed(cfg["seed"], rank)
     t0 = time.perf_counter()
     coords, bits = csg_inputs.make_config(cfg, seed)
