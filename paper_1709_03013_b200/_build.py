@@ -28,9 +28,15 @@ def needs_build(path=None):
 def build(force=False, verbose=False, ablate=False, defines=()):
     """nvcc -gencode arch=compute_100a,code=sm_100a -lineinfo -O3 -> paper_1709_03013_b200/libcsg.so
     ablate=True builds libcsg_ablate.so instead: the same sources with -DCSG_ABLATE, i.e. with the timing-ablation
-    switches of the fp4 kernel and csg_set_debug compiled in (wrong counts when set; never the product library)."""
+    switches of the fp4 kernel and csg_set_debug compiled in (wrong counts when set; never the product library).
+    defines: extra -D macros of a measurement build (ablate.py --static); such a build goes to
+    libcsg_variant_<macros>.so, NEVER to libcsg.so."""
     out = ABLATE_LIB_PATH if ablate else LIB_PATH
-    if not force and not defines and not needs_build(out):
+    if defines:
+        tag = "_".join(sorted(defines)).replace("=", "-")
+        tag = "".join(ch if (ch.isalnum() or ch in "-_") else "_" for ch in tag)
+        out = os.path.join(_HERE, "libcsg_variant_%s%s.so" % ("ablate_" if ablate else "", tag))
+    if not force and not needs_build(out):
         return out
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     cmd = [

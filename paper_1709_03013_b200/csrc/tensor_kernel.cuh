@@ -80,7 +80,16 @@ constexpr bool TC_WHOLE_GROUP = CSG_WHOLE_GROUP != 0;   // a producer set expand
 constexpr int TC_MAX_LEAD = 1;                 // rounds a cluster may run ahead of the average (L2 sharing inside a patch)
 constexpr int TC_THROTTLE_MAX_POLLS = 1 << 15; // polls of >= 200 ns in ONE wait before a cluster stops throttling for good (see the TMA warp)
 constexpr int TCF_ABLATE = 1, TCF_WAIT = 2, TCF_DUMP = 4, TCF_GATE = 8, TCF_SPARSE = 16, TCF_BATCH = 32;   // template FLAGS of tensor_action_kernel
-constexpr int TC_PREFILL_GROUPS = 2;           // groups (2 stages each) of the next tile expanded before a tile's epilogue
+#ifndef CSG_PREFILL_GROUPS
+#define CSG_PREFILL_GROUPS 2
+#endif
+#ifndef CSG_BITS_BUFS
+#define CSG_BITS_BUFS 4
+#endif
+#ifndef CSG_STATIC_DBG
+#define CSG_STATIC_DBG 0                   // measurement builds only (ablate.py --static): the dbg switches as a compile-time constant
+#endif
+constexpr int TC_PREFILL_GROUPS = CSG_PREFILL_GROUPS;   // groups (2 stages each) of the next tile expanded before a tile's epilogue
 // Privatised low bins per CTA (u32, shared memory, the last region of the dynamic window; the launch says how many).
 // Higher bins -- whole-histogram launches (smeared action) only -- go to the global histogram with one red.add per
 // value, and scattered global atomics run at 185 G/s on the device (1.57 clk each per SM, measured; u32 and u64
@@ -120,7 +129,7 @@ struct TcTraits {
     // ~1400 clk with everything else switched off, so 4 slots cap the pace at one stage per ~340 clk before any
     // work is done; fp4 has room for 6 (B only in shared memory, A ring = 6 x 32 TMEM columns).
     static constexpr int STAGES = A_IN_TMEM ? 6 : 4;
-    static constexpr int BITS_BUFS = 4;
+    static constexpr int BITS_BUFS = CSG_BITS_BUFS;
     static constexpr int NUM_BARS = 2 * STAGES + 2 + 2 * BITS_BUFS;
     static constexpr int OFF_BITS = STAGES * STAGE_BYTES;
     static constexpr int OFF_BARS = OFF_BITS + BITS_BUFS * BITS_BUF_BYTES;
@@ -521,7 +530,10 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
     const unsigned int* const landed = GATE ? landed_arg : nullptr;
     const uint32_t* const occ = SPARSE ? occ_arg : nullptr;
     using T = TcTraits<KIND>;
-    const int dbg = ABLATE ? dbg_arg : 0;             // compiled out of every instantiation of libcsg.so
+    // 0 and compiled out of every instantiation of libcsg.so.  Two measurement builds exist (paper_1709_03013_b200/ablate.py):
+    // -DCSG_ABLATE (run-time switches through csg_set_debug; the tests in the hot loops make that build 28 % slower than the
+    // product) and -DCSG_STATIC_DBG=<bits> (the same switches as a compile-time constant: what is left runs at product speed).
+    const int dbg = CSG_STATIC_DBG != 0 ? CSG_STATIC_DBG : (ABLATE ? dbg_arg : 0);
     constexpr int COLS = T::STAGE_COLS, WORDS = T::WORDS;
     extern __shared__ uint8_t smem_raw[];
     // the dynamic shared window starts at the same offset in both CTAs, so this rounding is identical in both
@@ -750,7 +762,7 @@ tensor_action_kernel(const __grid_constant__ CUtensorMap bits_map, const uint64_
             // rest of tile t+1 ...  While the accumulators of tile t are drained (the MMA thread waits for tmem_empty)
             // the ring already holds the first stages of tile t+1, so the tensor cores restart at once and the
             // producers get those stages' time to refill their pipeline.
-            const int prefill = (ABLATE && (dbg & 128)) ? 0 : TC_PREFILL_GROUPS;    // dbg 128: epilogue before any next stage
+            const int prefill = (dbg & 128) ? 0 : TC_PREFILL_GROUPS;    // dbg 128: epilogue before any next stage
             if (prefill == 0 && epi_I >= 0) {
                 publish_pending();
                 epilogue(epi_I, epi_J, epi_t);
