@@ -188,7 +188,12 @@ int csg_action_host(const uint64_t *rel_bits_host, int64_t N, int dim, double ep
  * _CHUNKED: always one launch per copy step behind an event.  The gated launch WAITS inside the kernel for the copy
  * stream, so it needs copies and kernels to run concurrently: under a tool that serialises the GPU's work (Nsight
  * Compute replays one kernel at a time and holds every other stream) it cannot make progress -- select _CHUNKED for
- * such runs (bench.py --host-pipeline chunked).  Results never depend on the mode.
+ * such runs (bench.py --host-pipeline chunked).  The same holds for anything else that synchronises the whole context
+ * while csg_action_host is running: CUDA loads kernels lazily, and the first launch of a not-yet-loaded kernel from
+ * ANOTHER host thread may have to wait for the gated kernel, which waits for copies this call is still enqueueing.
+ * (The library force-loads its own kernels before it launches a gated kernel.)  A process in which other threads may
+ * launch new kernels during csg_action_host should select _CHUNKED or run with CUDA_MODULE_LOADING=EAGER.
+ * Results never depend on the mode.
  */
 enum { CSG_HOST_PIPELINE_AUTO = 0, CSG_HOST_PIPELINE_CHUNKED = 1 };
 int csg_set_host_pipeline(int mode);
