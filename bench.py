@@ -540,8 +540,8 @@ def run_ours(args, cfg, rank, local_rank, world):
                                    "(%.1f lane-steps/clk/SM at %.0f MHz: the POPC pipe)" % (p_units / (p_ms * 1e-3) / 148 / (sm_clock_mhz * 1e6), sm_clock_mhz),
                     "kernel_ms": k_ms, "traffic": traffic, "traffic_source": traffic_src}
     if variant == csg.VARIANT_TENSOR_FP4:
-        # block-sparse sweep (csg_set_sparse, AUTO: matrices of 512 MiB and more): what the tensor cores really executed
-        sparse_on = N * csg.csg_row_stride_words(N) * 8 >= (512 << 20) and (dim != 2 or tiles_mode)   # CSG_SPARSE_AUTO
+        # block-sparse sweep (csg_set_sparse, AUTO: matrices of 96 MiB and more): what the tensor cores really executed
+        sparse_on = N * csg.csg_row_stride_words(N) * 8 >= (96 << 20) and (dim != 2 or tiles_mode)   # CSG_SPARSE_AUTO
         frac_exec = 1.0
         if sparse_on:
             occ = csg.csg_block_occupancy(d_bits, N)

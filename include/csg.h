@@ -30,7 +30,7 @@
  * graph that captured a call of this library (the graph holds pointers into the cached workspace).
  * Per-launch scratch (the finished-tile counter of the drift throttle, the occupancy map of the block-sparse sweep)
  * comes from rings of 32 slots per device: at most 32 launches that use them may be in flight at once, and a graph
- * that captured such a launch (matrices above 512 MiB) keeps its slot, so it must not be replayed while 32 or more
+ * that captured such a launch (matrices of 96 MiB and more) keeps its slot, so it must not be replayed while 32 or more
  * later launches of the same kind are still running.
  */
 #ifndef CSG_H_
@@ -269,7 +269,8 @@ int csg_set_throttle(int mode);
  * next to the diagonal are (elements close in time are almost never timelike separated).  One pass over the matrix
  * marks the empty blocks (csg_block_occupancy) and the kernel neither fetches, expands nor multiplies the two-stage
  * groups (2 x 256 columns) in which both stages are dead; results never depend on it.
- * CSG_SPARSE_AUTO: matrices of 512 MiB and more, unless the call says dim = 2 (a 1+1 order, flat or de Sitter, has
+ * CSG_SPARSE_AUTO: matrices of 96 MiB and more (N >= 28000; below, the extra launch costs more than the dead
+ * groups), unless the call says dim = 2 (a 1+1 order, flat or de Sitter, has
  * no empty block, and the pass and the mask loop would cost 2 %; csg_action_partial has no dim and uses the sweep);
  * _ON: every fp4 launch (test aid); _OFF: never.  csg_action_host marks the blocks of every chunk as it lands.
  */

@@ -475,9 +475,12 @@ static int launch_tensor(Device* D, int kind, const uint64_t* rel_bits, long lon
 // 256 x 256 blocks, and the kernel skips every two-stage group whose U or L blocks are empty.  Measured at config 3 (4D,
 // N = 131072): 10.8 % of the groups are dead, 88.5 -> 81.8 ms.  A 1+1 set (flat or de Sitter) has no empty block: there
 // the pass and the mask loop cost 2 % (de Sitter N = 131072: 94.0 -> 96.0 ms).  So CSG_SPARSE_AUTO switches it on for
-// matrices of 512 MiB and more unless the caller says dim = 2 (csg_action_partial has no dim: on); ON: every fp4
+// matrices of 96 MiB and more unless the caller says dim = 2 (csg_action_partial has no dim: on); ON: every fp4
 // launch (tests).  *occ = nullptr when the sweep stays dense.
-constexpr long long SPARSE_MIN_BYTES = 512LL << 20;
+// The threshold: 3+1 sprinklings have 11-12 % dead groups from N = 16384 on (5 % at 8192), but the occupancy pass is one
+// more dependent launch: measured dense / sparse ms at N = 8192: 0.047 / 0.063, 16384 (32 MiB): 0.234 / 0.244, 24576
+// (72 MiB): 0.706 / 0.708, 32768 (128 MiB): 1.603 / 1.551, 49152 (288 MiB): 4.94 / 4.64, 65536: 11.6 / 10.7.
+constexpr long long SPARSE_MIN_BYTES = 96LL << 20;
 
 // The occupancy map of the next launch (one of OCC_RING buffers), or *occ = nullptr when the sweep stays dense.
 static int occupancy_buffer(Device* D, int kind, long long N, long long stride, int dim_hint, uint32_t** occ) {
