@@ -135,3 +135,30 @@ def test_noalloc_leaves_device_memory_alone(csg):
     free1, _ = torch.cuda.mem_get_info()
     assert free1 == free0, (free0, free1)
     assert (counts.cpu().numpy() == oracle.alg5_counts(bits, 2000, 3)).all()
+
+
+def test_noalloc_inside_a_cuda_graph(csg):
+    """The case the entry point is for: captured into a CUDA graph WITHOUT any warm-up call of that size (csg_action needs
+    one, it allocates on first use), replayed twice.  The two captured calls run one after the other in the graph's
+    single stream, as the shared scratch requires."""
+    csg.csg_noalloc_setup()                                               # module loading and address look-up outside the capture
+    sets = [csg_inputs.make_causet(4, 1700 + 100 * b, 400 + b)[1] for b in range(2)]
+    Ns = [1700, 1800]
+    d = [csg.to_device(b) for b in sets]
+    counts = [torch.zeros(4, dtype=torch.int64, device="cuda") for _ in sets]
+    S = [torch.zeros(1, dtype=torch.float64, device="cuda") for _ in sets]
+    csg.csg_action_noalloc(d[0], 64, 4, 1.0, 3, counts[0], S[0])           # loads the kernel; a DIFFERENT size on purpose
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        for b in range(2):
+            csg.csg_action_noalloc(d[b], Ns[b], 4, 1.0, 3, counts[b], S[b])
+    for rep in range(2):
+        for c in counts:
+            c.fill_(-1)
+        graph.replay()
+        torch.cuda.synchronize()
+        for b in range(2):
+            want = oracle.alg5_counts(sets[b], Ns[b], 3)
+            assert (counts[b].cpu().numpy() == want).all(), (rep, b)
+            assert float(S[b].item()) == oracle.action_local(4, Ns[b], want)
